@@ -1,0 +1,140 @@
+/* xc_b200.h -- C ABI of the B200 (sm_100a) exchange-correlation integrator.
+ *
+ * Computes, on ONE GPU and in fp64, the numerical quadrature of the XC energy and
+ * potential matrix in a contracted Cartesian Gaussian basis over an atom-centred, partition-weighted
+ * molecular grid -- the "local integration" of arxiv 2007.03143 (Alg. 2 Input/Output, PAPER.md:L192:
+ * "Input: density matrix P, basis functions S, atomic centers A.  Output: V^xc, E^xc"; Alg. 4,
+ * PAPER.md:L255-L283):
+ *
+ *     E_xc = sum_i w_i f(rho_i, sigma_i)                         Eq. (2),(16)
+ *     V_mn = sum_i Z_mi Phi_ni + Phi_mi Z_ni                     Eq. (5),(17),(18)
+ *     Z_mi = 1/2 (w v_rho)_i Phi_mi + 2 (w v_sigma)_i grad rho_i . grad Phi_mi      Eq. (6),(20)
+ *     rho_i = sum_m Phi_mi X_mi,  grad rho_i = 2 sum_m grad Phi_mi X_mi,  X = P^j Phi^j   Eqs. (13)-(15)
+ *     N_el = sum_i w_i rho_i
+ *
+ * with w_i = w_i^q p_A(r_i) the SSF (or Becke-88) partition weights, Eq. (9), points
+ * grouped into spatial batches of <= max_batch_pts points with per-batch shell screening by the
+ * cuboid/sphere test of Alg. 1 and the cutoff radius of Eq. (10).
+ * Readings of ambiguous passages are listed in DESIGN.md (A1..A18).
+ *
+ * Conventions
+ *   - units: bohr / hartree.  All floating point is IEEE double.
+ *   - function order in P and V: shells in input order; inside a shell the Cartesian components
+ *     (l,m,n), l descending then m descending: p = x,y,z; d = xx,xy,xz,yy,yz,zz ((L+1)(L+2)/2 of them).
+ *   - coefficients are used as given (primitive norms included by the caller); nothing is renormalised.
+ *   - every entry point returns 0 (XC_OK) or a negative XC_E* code; nothing throws or aborts across the
+ *     ABI.  xc_last_error() returns a thread-local text for the last failure (CUDA error string included).
+ *   - HOST pointers are marked [host], DEVICE pointers [device].  The library never frees caller memory
+ *     and keeps no caller pointer after a call returns.
+ *   - there is no CPU fallback: without a CUDA device every compute entry point fails with XC_ECUDA.
+ */
+#ifndef XC_B200_H
+#define XC_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define XC_OK            0
+#define XC_EINVAL       -1  /* null pointer, bad size, ld < n_basis, non-positive exponent, bad enum */
+#define XC_EUNSUPPORTED -2  /* L > 2, nprim > 16, batch cannot be screened below the kernel's limit */
+#define XC_ENOMEM       -3  /* host or device allocation failed */
+#define XC_ECUDA        -4  /* CUDA runtime error (text in xc_last_error) */
+
+typedef struct { double x, y, z; int32_t Z; int32_t _pad; } xc_atom;           /* position (bohr), atomic number */
+typedef struct { int32_t atom; int32_t L; int32_t nprim; int32_t prim_off; } xc_shell; /* Cartesian shell, Eq. (7) */
+
+typedef struct {
+  int32_t n_rad, n_ang;   /* radial x angular points per atom (Table 2) */
+  int32_t radial;         /* 0 = Mura-Knowles, m = 3 (reading A3) */
+  int32_t angular;        /* 0 = Fibonacci sphere; 1 = Gauss-Legendre(cos theta) x trapezoid(phi), n_ang = 2 n_theta^2 (reading A4) */
+  int32_t partition;      /* 0 = SSF, a = 0.64; 1 = Becke-1988, 3 iterations, no size adjustment (reading A1/A2) */
+  int32_t functional;     /* 0 = LDA Slater+VWN5; 1 = GGA PBE */
+  int32_t max_batch_pts;  /* <= 512 */
+  int32_t flags;          /* bit 0: reserved */
+  double  eta;            /* Eq. (10) tolerance, 1e-10 */
+  double  mk_alpha;       /* Mura-Knowles scale, bohr (5.0) */
+  double  rho_tol;        /* points with rho <= rho_tol contribute nothing (1e-15, reading A12) */
+} xc_grid_spec;
+
+typedef struct xc_plan xc_plan;   /* opaque: owns host + device copies of grid, batches, basis, workspaces */
+
+/* Step (b) of the hot path + all uploads: builds the atom-centred grid (O1-O3), batches the points into
+ * cuboids of <= max_batch_pts points by recursive median bisection of the whole point cloud (the batching
+ * scheme is free; it satisfies Eq. (11)), screens shells per batch with Alg. 1
+ * on the batch's tight bounding box, and uploads everything to `device`.
+ *   atoms   [host] natoms entries;  shells [host] nshells entries;  exps, coefs [host] nprim_total each.
+ * device = -1 builds a HOST-ONLY plan (no CUDA call is made): xc_plan_info / xc_plan_stats / xc_plan_export work on
+ * it, every compute entry point returns XC_ECUDA.  It exists so that the planner can be validated without a GPU.
+ * On success *out owns the plan (free with xc_plan_destroy).  Errors: XC_EINVAL, XC_EUNSUPPORTED, XC_ENOMEM, XC_ECUDA. */
+int xc_plan_create(const xc_atom* atoms, int32_t natoms, const xc_shell* shells, int32_t nshells,
+                   const double* exps, const double* coefs, int32_t nprim_total,
+                   const xc_grid_spec* spec, int32_t device, xc_plan** out);
+
+/* Sizes of a plan.  Any output pointer may be NULL.  n_shell_entries = sum_j |S_j| (shells, not functions);
+ * algorithmic_flops = sum_j 4 (N_b^j)^2 N_q^j (Eq. (22) PAPER.md:L196 with each MAC = 2 flop). */
+int xc_plan_info(const xc_plan* plan, int64_t* n_points, int64_t* n_batches, int32_t* n_basis,
+                 int64_t* n_shell_entries, double* algorithmic_flops);
+
+/* The plan as DATA, for the oracle (reading A9).  All [host], caller-allocated with the sizes of xc_plan_info:
+ *   pts 3*n_points (x,y,z per point, batch-contiguous order), wq n_points (base weights w^q),
+ *   parent n_points (parent atom), orig n_points (index of the point in the canonical atom-major /
+ *   radial / angular grid order), batch_off n_batches+1, shell_off n_batches+1, shells n_shell_entries
+ *   (global shell ids, ascending inside a batch).  Any pointer may be NULL to skip it. */
+int xc_plan_export(const xc_plan* plan, double* pts, double* wq, int32_t* parent, int64_t* orig,
+                   int64_t* batch_off, int64_t* shell_off, int32_t* shells);
+
+/* Steps (a),(c)-(g): one full E_xc / V_xc / N_el build, stream-ordered on `cuda_stream` (a cudaStream_t, may be 0).
+ *   dP [device] n_basis x n_basis, leading dimension ldp >= n_basis, symmetric (assumed, not checked), read only.
+ *   dV [device] n_basis x n_basis, leading dimension ldv >= n_basis: OVERWRITTEN (Alg. 2 l.2.4),
+ *      both triangles written, exactly symmetric, bit-identical from run to run.
+ *   E_xc, N_el [host] scalars, valid when the call returns (the call synchronises the stream once, at the end).
+ *   flags: bit 0 = reuse the partition weights of the previous xc_eval on this plan (skip step (a);
+ *          "cached-weights build", reading A16); 0 = full build. */
+int xc_eval(xc_plan* plan, const double* dP, int64_t ldp, double* dV, int64_t ldv,
+            double* E_xc, double* N_el, int32_t flags, void* cuda_stream);
+
+/* Same build with HOST buffers: copies P to the device, runs xc_eval, copies V back.  hP, hV [host]. */
+int xc_eval_host(xc_plan* plan, const double* hP, int64_t ldp, double* hV, int64_t ldv,
+                 double* E_xc, double* N_el, int32_t flags);
+
+/* Diagnostics of the last xc_eval on this plan, for parity tests at full size.  All [host], may be NULL:
+ *   w n_points final partition weights (plan order);  rho n_points;  grad_rho 3*n_points (zeros for LDA);
+ *   E_batch, N_batch n_batches: per-batch partial sums of w f and w rho. */
+int xc_eval_diagnostics(xc_plan* plan, double* w, double* rho, double* grad_rho, double* E_batch, double* N_batch);
+
+/* Device time in milliseconds of each stage of the last xc_eval (CUDA events on the eval stream):
+ * ms[0] weights (a), ms[1] density kernel (c,d1,e,f,Z), ms[2] potential kernel (d2 + scatter g), ms[3] finalise, ms[4] total.
+ * launches: number of kernel launches of that xc_eval. */
+int xc_eval_timings(const xc_plan* plan, float ms[5], int32_t* launches);
+
+/* Algorithmic sizes of the plan used by the roofline report: [0] sum_j N_b^j N_q^j (function-points),
+ * [1] sum_j (N_b^j)^2, [2] sum_j 4 (N_b^j)^2 N_q^j, [3] max N_b^j, [4] mean N_q^j, [5] bytes of Phi/Z workspace. */
+int xc_plan_stats(const xc_plan* plan, double stats[6]);
+
+int xc_plan_destroy(xc_plan* plan);
+
+/* One-shot form named by BASELINE.json:north_star = create + eval + destroy. */
+int xc_integrate(const xc_atom* atoms, int32_t natoms, const xc_shell* shells, int32_t nshells,
+                 const double* exps, const double* coefs, int32_t nprim_total, const xc_grid_spec* spec,
+                 int32_t device, const double* dP, int64_t ldp, double* dV, int64_t ldv,
+                 double* E_xc, double* N_el, void* cuda_stream);
+
+/* Stand-alone kernels of single steps, for element-wise parity tests (device pointers, stream-ordered):
+ *   xc_partition_weights: step (a) on arbitrary points. pts [device] 3 arrays x,y,z; parent, wq, w_out [device] npts.
+ *   xc_functional: step (f) point values. rho, sigma, f, vrho, vsigma [device] n each. */
+int xc_partition_weights(const xc_atom* atoms /*[host]*/, int32_t natoms, int32_t partition, int64_t npts,
+                         const double* dx, const double* dy, const double* dz, const double* dwq,
+                         const int32_t* dparent, double* dw_out, void* cuda_stream);
+int xc_functional(int32_t functional, int64_t n, const double* drho, const double* dsigma, double rho_tol,
+                  double* df, double* dvrho, double* dvsigma, void* cuda_stream);
+
+const char* xc_strerror(int code);
+const char* xc_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* XC_B200_H */

@@ -1,0 +1,263 @@
+"""Thin ctypes binding of libxc_b200.so (include/xc_b200.h): argument marshalling only -- every step of
+the hot path runs in the library's CUDA kernels.  torch is used for device memory and streams.
+There is no fallback: if the shared library is missing or cannot be loaded, importing this module fails."""
+from __future__ import annotations
+
+import ctypes as C
+import dataclasses
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libxc_b200.so")
+
+XC_OK, XC_EINVAL, XC_EUNSUPPORTED, XC_ENOMEM, XC_ECUDA = 0, -1, -2, -3, -4
+
+
+class XcAtom(C.Structure):
+    _fields_ = [("x", C.c_double), ("y", C.c_double), ("z", C.c_double), ("Z", C.c_int32), ("_pad", C.c_int32)]
+
+
+class XcShell(C.Structure):
+    _fields_ = [("atom", C.c_int32), ("L", C.c_int32), ("nprim", C.c_int32), ("prim_off", C.c_int32)]
+
+
+class XcGridSpec(C.Structure):
+    _fields_ = [("n_rad", C.c_int32), ("n_ang", C.c_int32), ("radial", C.c_int32), ("angular", C.c_int32),
+                ("partition", C.c_int32), ("functional", C.c_int32), ("max_batch_pts", C.c_int32), ("flags", C.c_int32),
+                ("eta", C.c_double), ("mk_alpha", C.c_double), ("rho_tol", C.c_double)]
+
+
+def grid_spec(n_rad, n_ang, functional, angular=0, partition=0, max_batch_pts=512, eta=1e-10, mk_alpha=5.0,
+              rho_tol=1e-15) -> XcGridSpec:
+    return XcGridSpec(n_rad, n_ang, 0, angular, partition, functional, max_batch_pts, 0, eta, mk_alpha, rho_tol)
+
+
+class XcError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("libxc_b200: %s (%d): %s" % (_lib.xc_strerror(code).decode(), code, msg))
+        self.code = code
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError("libxc_b200.so not built (run `python -m paper_2007_03143_b200.build` or __graft_entry__.build()); "
+                          "there is no CPU fallback")
+    lib = C.CDLL(LIB_PATH)
+    vp, dp, ip, lp = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_int64)
+    lib.xc_strerror.restype = C.c_char_p
+    lib.xc_strerror.argtypes = [C.c_int]
+    lib.xc_last_error.restype = C.c_char_p
+    lib.xc_plan_create.argtypes = [C.POINTER(XcAtom), C.c_int32, C.POINTER(XcShell), C.c_int32, dp, dp, C.c_int32,
+                                   C.POINTER(XcGridSpec), C.c_int32, C.POINTER(vp)]
+    lib.xc_plan_info.argtypes = [vp, lp, lp, ip, lp, dp]
+    lib.xc_plan_stats.argtypes = [vp, dp]
+    lib.xc_plan_export.argtypes = [vp, dp, dp, ip, lp, lp, lp, ip]
+    lib.xc_eval.argtypes = [vp, vp, C.c_int64, vp, C.c_int64, dp, dp, C.c_int32, vp]
+    lib.xc_eval_host.argtypes = [vp, vp, C.c_int64, vp, C.c_int64, dp, dp, C.c_int32]
+    lib.xc_eval_diagnostics.argtypes = [vp, dp, dp, dp, dp, dp]
+    lib.xc_eval_timings.argtypes = [vp, C.POINTER(C.c_float), ip]
+    lib.xc_plan_destroy.argtypes = [vp]
+    lib.xc_integrate.argtypes = [C.POINTER(XcAtom), C.c_int32, C.POINTER(XcShell), C.c_int32, dp, dp, C.c_int32,
+                                 C.POINTER(XcGridSpec), C.c_int32, vp, C.c_int64, vp, C.c_int64, dp, dp, vp]
+    lib.xc_partition_weights.argtypes = [C.POINTER(XcAtom), C.c_int32, C.c_int32, C.c_int64, vp, vp, vp, vp, vp, vp, vp]
+    lib.xc_functional.argtypes = [C.c_int32, C.c_int64, vp, vp, C.c_double, vp, vp, vp, vp]
+    for name in EXPORTED:
+        getattr(lib, name)  # fail loudly if a declared symbol is missing
+    return lib
+
+
+EXPORTED = ["xc_plan_create", "xc_plan_info", "xc_plan_export", "xc_eval", "xc_eval_host", "xc_eval_diagnostics",
+            "xc_eval_timings", "xc_plan_stats", "xc_plan_destroy", "xc_integrate", "xc_partition_weights",
+            "xc_functional", "xc_strerror", "xc_last_error"]
+
+_lib = _load()
+
+
+def _check(rc):
+    if rc != XC_OK:
+        raise XcError(rc, _lib.xc_last_error().decode())
+
+
+def _dp(a):
+    return None if a is None else a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _atoms(xyz, Z):
+    xyz = np.ascontiguousarray(xyz, np.float64)
+    arr = (XcAtom * len(xyz))()
+    for i in range(len(xyz)):
+        arr[i] = XcAtom(xyz[i, 0], xyz[i, 1], xyz[i, 2], int(Z[i]) if Z is not None else 0, 0)
+    return arr
+
+
+def _shells(atom, L, nprim, off):
+    arr = (XcShell * len(atom))()
+    for i in range(len(atom)):
+        arr[i] = XcShell(int(atom[i]), int(L[i]), int(nprim[i]), int(off[i]))
+    return arr
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    return C.c_void_p(int(stream) if isinstance(stream, int) else stream.cuda_stream)
+
+
+@dataclasses.dataclass
+class PlanExport:
+    pts: np.ndarray
+    wq: np.ndarray
+    parent: np.ndarray
+    orig: np.ndarray
+    batch_off: np.ndarray
+    shell_off: np.ndarray
+    shells: np.ndarray
+
+
+class Plan:
+    """xc_plan: grid + batches + screening + device workspaces for one molecule/basis/grid."""
+
+    def __init__(self, atoms_xyz, atoms_Z, shell_atom, shell_L, shell_nprim, shell_prim_off, exps, coefs,
+                 spec: XcGridSpec, device: int = 0):
+        exps = np.ascontiguousarray(exps, np.float64)
+        coefs = np.ascontiguousarray(coefs, np.float64)
+        at = _atoms(atoms_xyz, atoms_Z)
+        sh = _shells(shell_atom, shell_L, shell_nprim, shell_prim_off)
+        h = C.c_void_p()
+        _check(_lib.xc_plan_create(at, len(at), sh, len(sh), _dp(exps), _dp(coefs), len(exps), C.byref(spec), device,
+                                   C.byref(h)))
+        self._h = h
+        self.spec = spec
+        self.device = device
+        npts, nbat, nsh = C.c_int64(), C.c_int64(), C.c_int64()
+        nbas = C.c_int32()
+        fl = C.c_double()
+        _check(_lib.xc_plan_info(h, C.byref(npts), C.byref(nbat), C.byref(nbas), C.byref(nsh), C.byref(fl)))
+        self.n_points, self.n_batches, self.n_basis = npts.value, nbat.value, nbas.value
+        self.n_shell_entries, self.algorithmic_flops = nsh.value, fl.value
+
+    @classmethod
+    def from_workload(cls, w, spec=None, device=0, **kw):
+        if spec is None:
+            spec = grid_spec(w.n_rad, w.n_ang, w.functional, **kw)
+        return cls(w.atoms_xyz, w.atoms_Z, w.shell_atom, w.shell_L, w.shell_nprim, w.shell_prim_off, w.exps, w.coefs,
+                   spec, device)
+
+    def stats(self):
+        s = (C.c_double * 6)()
+        _check(_lib.xc_plan_stats(self._h, s))
+        return dict(sum_nb_nq=s[0], sum_nb2=s[1], flops=s[2], max_nb=int(s[3]), mean_nq=s[4], workspace_bytes=s[5])
+
+    def export(self) -> PlanExport:
+        n, nb = self.n_points, self.n_batches
+        pts = np.empty((n, 3))
+        wq = np.empty(n)
+        parent = np.empty(n, np.int32)
+        orig = np.empty(n, np.int64)
+        boff = np.empty(nb + 1, np.int64)
+        soff = np.empty(nb + 1, np.int64)
+        shells = np.empty(self.n_shell_entries, np.int32)
+        _check(_lib.xc_plan_export(self._h, _dp(pts), _dp(wq), parent.ctypes.data_as(C.POINTER(C.c_int32)),
+                                   orig.ctypes.data_as(C.POINTER(C.c_int64)), boff.ctypes.data_as(C.POINTER(C.c_int64)),
+                                   soff.ctypes.data_as(C.POINTER(C.c_int64)),
+                                   shells.ctypes.data_as(C.POINTER(C.c_int32))))
+        return PlanExport(pts, wq, parent, orig, boff, soff, shells)
+
+    def eval(self, P, V=None, reuse_weights=False, stream=None):
+        """P, V: torch CUDA float64 tensors (n_basis x n_basis). Returns (E_xc, N_el, V)."""
+        import torch
+        assert P.is_cuda and P.dtype == torch.float64 and P.dim() == 2 and P.stride(1) == 1
+        if V is None:
+            V = torch.empty((self.n_basis, self.n_basis), dtype=torch.float64, device=P.device)
+        assert V.is_cuda and V.dtype == torch.float64 and V.stride(1) == 1
+        E, N = C.c_double(), C.c_double()
+        _check(_lib.xc_eval(self._h, C.c_void_p(P.data_ptr()), P.stride(0), C.c_void_p(V.data_ptr()), V.stride(0),
+                            C.byref(E), C.byref(N), 1 if reuse_weights else 0, _stream_ptr(stream)))
+        return E.value, N.value, V
+
+    def eval_host(self, P, V=None, reuse_weights=False):
+        """P, V: host buffers (numpy arrays or pinned torch CPU tensors), float64, row-major."""
+        Pp, ldp = _host_ptr(P)
+        if V is None:
+            V = np.empty((self.n_basis, self.n_basis))
+        Vp, ldv = _host_ptr(V)
+        E, N = C.c_double(), C.c_double()
+        _check(_lib.xc_eval_host(self._h, Pp, ldp, Vp, ldv, C.byref(E), C.byref(N), 1 if reuse_weights else 0))
+        return E.value, N.value, V
+
+    def diagnostics(self, want_points=True):
+        n, nb = self.n_points, self.n_batches
+        w = np.empty(n) if want_points else None
+        rho = np.empty(n) if want_points else None
+        gr = np.empty((n, 3)) if want_points else None
+        Eb, Nb = np.empty(nb), np.empty(nb)
+        _check(_lib.xc_eval_diagnostics(self._h, _dp(w), _dp(rho), _dp(gr), _dp(Eb), _dp(Nb)))
+        return dict(w=w, rho=rho, grad_rho=gr, E_batch=Eb, N_batch=Nb)
+
+    def timings(self):
+        ms = (C.c_float * 5)()
+        n = C.c_int32()
+        _check(_lib.xc_eval_timings(self._h, ms, C.byref(n)))
+        return dict(weights_ms=ms[0], density_ms=ms[1], potential_ms=ms[2], finalize_ms=ms[3], total_ms=ms[4],
+                    launches=n.value)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _lib.xc_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def _host_ptr(a):
+    if isinstance(a, np.ndarray):
+        assert a.dtype == np.float64 and a.ndim == 2 and a.strides[1] == 8
+        return C.c_void_p(a.ctypes.data), a.strides[0] // 8
+    assert (not a.is_cuda) and a.dim() == 2 and a.stride(1) == 1  # torch CPU tensor
+    return C.c_void_p(a.data_ptr()), a.stride(0)
+
+
+def xc_integrate(w, P, spec=None, device=0, stream=None):
+    """One-shot form of BASELINE.json:north_star: (atoms, shells, grid_spec, P) -> (E_xc, V_xc, N_el)."""
+    import torch
+    if spec is None:
+        spec = grid_spec(w.n_rad, w.n_ang, w.functional)
+    exps = np.ascontiguousarray(w.exps, np.float64)
+    coefs = np.ascontiguousarray(w.coefs, np.float64)
+    at = _atoms(w.atoms_xyz, w.atoms_Z)
+    sh = _shells(w.shell_atom, w.shell_L, w.shell_nprim, w.shell_prim_off)
+    V = torch.empty_like(P)
+    E, N = C.c_double(), C.c_double()
+    _check(_lib.xc_integrate(at, len(at), sh, len(sh), _dp(exps), _dp(coefs), len(exps), C.byref(spec), device,
+                             C.c_void_p(P.data_ptr()), P.stride(0), C.c_void_p(V.data_ptr()), V.stride(0), C.byref(E),
+                             C.byref(N), _stream_ptr(stream)))
+    return E.value, V, N.value
+
+
+def partition_weights(atoms_xyz, pts, wq, parent, partition=0, stream=None):
+    """Step (a) alone on torch CUDA tensors; pts (n,3)."""
+    import torch
+    at = _atoms(atoms_xyz, None)
+    x, y, z = (pts[:, k].contiguous() for k in range(3))
+    out = torch.empty_like(wq)
+    _check(_lib.xc_partition_weights(at, len(at), partition, wq.numel(), C.c_void_p(x.data_ptr()),
+                                     C.c_void_p(y.data_ptr()), C.c_void_p(z.data_ptr()), C.c_void_p(wq.data_ptr()),
+                                     C.c_void_p(parent.data_ptr()), C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+    return out
+
+
+def functional(kind, rho, sigma, rho_tol=1e-15, stream=None):
+    """Step (f) point values on torch CUDA tensors: returns f, v_rho, v_sigma."""
+    import torch
+    f, vr, vs = torch.empty_like(rho), torch.empty_like(rho), torch.empty_like(rho)
+    _check(_lib.xc_functional(kind, rho.numel(), C.c_void_p(rho.data_ptr()), C.c_void_p(sigma.data_ptr()), rho_tol,
+                              C.c_void_p(f.data_ptr()), C.c_void_p(vr.data_ptr()), C.c_void_p(vs.data_ptr()),
+                              _stream_ptr(stream)))
+    return f, vr, vs

@@ -1,0 +1,363 @@
+// xc_api.cu -- the C ABI of libxc_b200 (include/xc_b200.h): plan lifetime, uploads, the stream-ordered
+// launch sequence of one E_xc / V_xc / N_el build (Alg. 2 l.2.2-2.9 on one GPU), diagnostics.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "xc_internal.h"
+#include "xc_kernels.h"
+
+using namespace xcb;
+
+namespace {
+thread_local std::string g_err;
+int fail(int code, const std::string& msg) { g_err = msg; return code; }
+int cuda_fail(cudaError_t e, const char* what) {
+  g_err = std::string(what) + ": " + cudaGetErrorString(e);
+  return e == cudaErrorMemoryAllocation ? XC_ENOMEM : XC_ECUDA;
+}
+#define CU(call)                                         \
+  do {                                                   \
+    cudaError_t _e = (call);                             \
+    if (_e != cudaSuccess) return cuda_fail(_e, #call);  \
+  } while (0)
+
+template <class T>
+int upload(T** dptr, const std::vector<T>& h) {
+  *dptr = nullptr;
+  size_t bytes = std::max<size_t>(h.size(), 1) * sizeof(T);
+  CU(cudaMalloc((void**)dptr, bytes));
+  if (!h.empty()) CU(cudaMemcpy(*dptr, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice));
+  return XC_OK;
+}
+}  // namespace
+
+struct xc_plan {
+  int device = 0;
+  HostPlan hp;
+  // device copies
+  double *d_px = nullptr, *d_py = nullptr, *d_pz = nullptr, *d_wq = nullptr, *d_w = nullptr;
+  int32_t* d_parent = nullptr;
+  double *d_atoms = nullptr, *d_invR = nullptr, *d_rnn = nullptr;
+  ShellRec* d_shells = nullptr;
+  double *d_exps = nullptr, *d_coefs = nullptr;
+  BatchRec* d_batches = nullptr;
+  int32_t *d_bshells = nullptr, *d_bsfoff = nullptr, *d_bfidx = nullptr, *d_bfinfo = nullptr;
+  DensityItem *d_items64 = nullptr, *d_items32 = nullptr;
+  PotItem* d_pot = nullptr;
+  double *d_phi = nullptr, *d_z = nullptr;
+  unsigned long long *d_vhi = nullptr, *d_vlo = nullptr;
+  double *d_Epart = nullptr, *d_Npart = nullptr, *d_result = nullptr;
+  double *d_rho = nullptr, *d_grho = nullptr;
+  double* h_result = nullptr;  // pinned
+  double *d_Ptmp = nullptr, *d_Vtmp = nullptr;  // for xc_eval_host
+  bool weights_valid = false;
+  std::vector<cudaEvent_t> ev;
+  float ms[5] = {0, 0, 0, 0, 0};
+  int launches = 0;
+};
+
+static void free_plan(xc_plan* p) {
+  if (!p) return;
+  if (p->device < 0) { delete p; return; }
+  cudaSetDevice(p->device);
+  void* ptrs[] = {p->d_px, p->d_py, p->d_pz, p->d_wq, p->d_w, p->d_parent, p->d_atoms, p->d_invR, p->d_rnn, p->d_shells,
+                  p->d_exps, p->d_coefs, p->d_batches, p->d_bshells, p->d_bsfoff, p->d_bfidx, p->d_bfinfo, p->d_items64,
+                  p->d_items32, p->d_pot, p->d_phi, p->d_z, p->d_vhi, p->d_vlo, p->d_Epart, p->d_Npart, p->d_result,
+                  p->d_rho, p->d_grho, p->d_Ptmp, p->d_Vtmp};
+  for (void* q : ptrs) if (q) cudaFree(q);
+  if (p->h_result) cudaFreeHost(p->h_result);
+  for (cudaEvent_t e : p->ev) cudaEventDestroy(e);
+  delete p;
+}
+
+static void atom_tables(const std::vector<double>& atoms, int natoms, std::vector<double>& invR, std::vector<double>& rnn) {
+  invR.assign((size_t)natoms * natoms, 0.0);
+  rnn.assign(natoms, 1e300);
+  for (int a = 0; a < natoms; ++a)
+    for (int b = 0; b < natoms; ++b) {
+      if (a == b) continue;
+      double dx = atoms[3 * a] - atoms[3 * b], dy = atoms[3 * a + 1] - atoms[3 * b + 1], dz = atoms[3 * a + 2] - atoms[3 * b + 2];
+      double r = std::sqrt(dx * dx + dy * dy + dz * dz);
+      invR[(size_t)a * natoms + b] = 1.0 / r;
+      rnn[a] = std::min(rnn[a], r);
+    }
+}
+
+extern "C" {
+
+const char* xc_strerror(int code) {
+  switch (code) {
+    case XC_OK: return "ok";
+    case XC_EINVAL: return "invalid argument";
+    case XC_EUNSUPPORTED: return "unsupported input";
+    case XC_ENOMEM: return "out of memory";
+    case XC_ECUDA: return "CUDA error";
+    default: return "unknown error";
+  }
+}
+const char* xc_last_error(void) { return g_err.c_str(); }
+
+int xc_plan_create(const xc_atom* atoms, int32_t natoms, const xc_shell* shells, int32_t nshells, const double* exps,
+                   const double* coefs, int32_t nprim_total, const xc_grid_spec* spec, int32_t device, xc_plan** out) {
+  if (!out) return fail(XC_EINVAL, "out is null");
+  *out = nullptr;
+  if (device != -1) {
+    int ndev = 0;
+    cudaError_t ce = cudaGetDeviceCount(&ndev);
+    if (ce != cudaSuccess || ndev == 0) return fail(XC_ECUDA, std::string("no CUDA device: ") + cudaGetErrorString(ce));
+    if (device < 0 || device >= ndev) return fail(XC_EINVAL, "bad device index");
+  }
+  xc_plan* p = new (std::nothrow) xc_plan();
+  if (!p) return fail(XC_ENOMEM, "host allocation failed");
+  p->device = device;
+  std::string err;
+  int rc;
+  try {
+    rc = build_host_plan(atoms, natoms, shells, nshells, exps, coefs, nprim_total, spec, p->hp, err);
+  } catch (const std::bad_alloc&) {
+    rc = XC_ENOMEM; err = "host allocation failed in planner";
+  }
+  if (rc != XC_OK) { free_plan(p); return fail(rc, err); }
+  HostPlan& hp = p->hp;
+  if (device == -1) { *out = p; return XC_OK; }   // host-only plan: info / stats / export only
+  auto bail = [&](int code) { free_plan(p); return code; };
+  if (cudaSetDevice(device) != cudaSuccess) return bail(fail(XC_ECUDA, "cudaSetDevice failed"));
+  std::vector<double> invR, rnn;
+  atom_tables(hp.atoms, hp.natoms, invR, rnn);
+#define UP(d, h) do { int _r = upload(&p->d, h); if (_r != XC_OK) return bail(_r); } while (0)
+  UP(d_px, hp.px); UP(d_py, hp.py); UP(d_pz, hp.pz); UP(d_wq, hp.wq); UP(d_parent, hp.parent);
+  UP(d_atoms, hp.atoms); UP(d_invR, invR); UP(d_rnn, rnn);
+  UP(d_shells, hp.shells); UP(d_exps, hp.exps); UP(d_coefs, hp.coefs);
+  UP(d_batches, hp.batches); UP(d_bshells, hp.bshells); UP(d_bsfoff, hp.bsfoff); UP(d_bfidx, hp.bfidx); UP(d_bfinfo, hp.bfinfo);
+  UP(d_items64, hp.items64); UP(d_items32, hp.items32); UP(d_pot, hp.pot_items);
+#undef UP
+  size_t nitems = hp.items64.size() + hp.items32.size();
+  size_t nb2 = (size_t)hp.nbasis * hp.nbasis;
+#define AL(d, bytes) do { cudaError_t _e = cudaMalloc((void**)&p->d, std::max<size_t>((bytes), 8)); if (_e != cudaSuccess) return bail(cuda_fail(_e, "cudaMalloc " #d)); } while (0)
+  AL(d_w, hp.npts * 8); AL(d_phi, (size_t)hp.scr_cap_doubles * 8); AL(d_z, (size_t)hp.scr_cap_doubles * 8);
+  AL(d_vhi, nb2 * 8); AL(d_vlo, nb2 * 8); AL(d_Epart, nitems * 8); AL(d_Npart, nitems * 8); AL(d_result, 16);
+  AL(d_rho, hp.npts * 8); AL(d_grho, hp.npts * 24);
+#undef AL
+  if (cudaMallocHost((void**)&p->h_result, 16) != cudaSuccess) return bail(fail(XC_ENOMEM, "cudaMallocHost failed"));
+  p->ev.resize(4 + 2 * hp.chunks.size());
+  for (auto& e : p->ev)
+    if (cudaEventCreate(&e) != cudaSuccess) return bail(fail(XC_ECUDA, "cudaEventCreate failed"));
+  *out = p;
+  return XC_OK;
+}
+
+int xc_plan_info(const xc_plan* p, int64_t* n_points, int64_t* n_batches, int32_t* n_basis, int64_t* n_shell_entries,
+                 double* algorithmic_flops) {
+  if (!p) return fail(XC_EINVAL, "plan is null");
+  if (n_points) *n_points = p->hp.npts;
+  if (n_batches) *n_batches = (int64_t)p->hp.batches.size();
+  if (n_basis) *n_basis = p->hp.nbasis;
+  if (n_shell_entries) *n_shell_entries = (int64_t)p->hp.bshells.size();
+  if (algorithmic_flops) *algorithmic_flops = p->hp.flops;
+  return XC_OK;
+}
+
+int xc_plan_stats(const xc_plan* p, double stats[6]) {
+  if (!p || !stats) return fail(XC_EINVAL, "null argument");
+  stats[0] = p->hp.sum_nbnq; stats[1] = p->hp.sum_nb2; stats[2] = p->hp.flops; stats[3] = p->hp.max_nb;
+  stats[4] = p->hp.batches.empty() ? 0.0 : (double)p->hp.npts / (double)p->hp.batches.size();
+  stats[5] = 16.0 * (double)p->hp.scr_doubles;
+  return XC_OK;
+}
+
+int xc_plan_export(const xc_plan* p, double* pts, double* wq, int32_t* parent, int64_t* orig, int64_t* batch_off,
+                   int64_t* shell_off, int32_t* shells) {
+  if (!p) return fail(XC_EINVAL, "plan is null");
+  const HostPlan& hp = p->hp;
+  if (pts) for (int64_t i = 0; i < hp.npts; ++i) { pts[3 * i] = hp.px[i]; pts[3 * i + 1] = hp.py[i]; pts[3 * i + 2] = hp.pz[i]; }
+  if (wq) std::copy(hp.wq.begin(), hp.wq.end(), wq);
+  if (parent) std::copy(hp.parent.begin(), hp.parent.end(), parent);
+  if (orig) std::copy(hp.orig.begin(), hp.orig.end(), orig);
+  size_t nb = hp.batches.size();
+  if (batch_off) { for (size_t j = 0; j < nb; ++j) batch_off[j] = hp.batches[j].pt_off; batch_off[nb] = hp.npts; }
+  if (shell_off) { for (size_t j = 0; j < nb; ++j) shell_off[j] = hp.batches[j].sh_off; shell_off[nb] = (int64_t)hp.bshells.size(); }
+  if (shells) std::copy(hp.bshells.begin(), hp.bshells.end(), shells);
+  return XC_OK;
+}
+
+int xc_eval(xc_plan* p, const double* dP, int64_t ldp, double* dV, int64_t ldv, double* E_xc, double* N_el,
+            int32_t flags, void* cuda_stream) {
+  if (!p || !dP || !dV || !E_xc || !N_el) return fail(XC_EINVAL, "null argument");
+  if (p->device < 0) return fail(XC_ECUDA, "host-only plan (device = -1): no CUDA device bound, and there is no CPU fallback");
+  HostPlan& hp = p->hp;
+  if (ldp < hp.nbasis || ldv < hp.nbasis) return fail(XC_EINVAL, "leading dimension smaller than n_basis");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CU(cudaSetDevice(p->device));
+  const bool gga = hp.spec.functional == 1;
+  int launches = 0;
+  size_t ie = 0;
+  CU(cudaEventRecord(p->ev[ie++], st));
+  if (!(flags & 1) || !p->weights_valid) {
+    CU(launch_weights(hp.spec.partition, hp.natoms, p->d_atoms, p->d_invR, p->d_rnn, hp.npts, p->d_px, p->d_py, p->d_pz,
+                      p->d_wq, p->d_parent, p->d_w, st));
+    ++launches;
+    p->weights_valid = true;
+  }
+  CU(cudaEventRecord(p->ev[ie++], st));
+  size_t nb2 = (size_t)hp.nbasis * hp.nbasis;
+  CU(cudaMemsetAsync(p->d_vhi, 0, nb2 * 8, st));
+  CU(cudaMemsetAsync(p->d_vlo, 0, nb2 * 8, st));
+  CU(cudaMemsetAsync(p->d_rho, 0, hp.npts * 8, st));
+  CU(cudaMemsetAsync(p->d_grho, 0, hp.npts * 24, st));
+  DensityArgs da;
+  da.batches = p->d_batches; da.bshells = p->d_bshells; da.bsfoff = p->d_bsfoff; da.bfidx = p->d_bfidx; da.bfinfo = p->d_bfinfo;
+  da.shells = p->d_shells; da.exps = p->d_exps; da.coefs = p->d_coefs;
+  da.px = p->d_px; da.py = p->d_py; da.pz = p->d_pz; da.w = p->d_w;
+  da.P = dP; da.ldp = ldp; da.phi_scr = p->d_phi; da.z_scr = p->d_z;
+  da.rho_out = p->d_rho; da.grho_out = gga ? p->d_grho : nullptr;
+  da.Epart = p->d_Epart; da.Npart = p->d_Npart; da.rho_tol = hp.spec.rho_tol;
+  PotArgs pa;
+  pa.batches = p->d_batches; pa.bfidx = p->d_bfidx; pa.phi_scr = p->d_phi; pa.z_scr = p->d_z;
+  pa.vhi = p->d_vhi; pa.vlo = p->d_vlo; pa.nbasis = hp.nbasis;
+  const int n64 = (int)hp.items64.size();
+  for (const auto& c : hp.chunks) {
+    if (c.i64_1 > c.i64_0) {
+      CU(launch_density(64, gga, da, p->d_items64 + c.i64_0, (int)(c.i64_1 - c.i64_0), (int)c.i64_0, hp.smem64, st));
+      ++launches;
+    }
+    if (c.i32_1 > c.i32_0) {
+      CU(launch_density(32, gga, da, p->d_items32 + c.i32_0, (int)(c.i32_1 - c.i32_0), n64 + (int)c.i32_0, hp.smem32, st));
+      ++launches;
+    }
+    CU(cudaEventRecord(p->ev[ie++], st));
+    pa.items = p->d_pot + c.p0; pa.nitems = c.p1 - c.p0;
+    if (pa.nitems > 0) { CU(launch_potential(pa, st)); ++launches; }
+    CU(cudaEventRecord(p->ev[ie++], st));
+  }
+  CU(launch_finalize(hp.nbasis, p->d_vhi, p->d_vlo, dV, ldv, st));
+  CU(launch_reduce((int64_t)(hp.items64.size() + hp.items32.size()), p->d_Epart, p->d_Npart, p->d_result, st));
+  launches += 2;
+  CU(cudaMemcpyAsync(p->h_result, p->d_result, 16, cudaMemcpyDeviceToHost, st));
+  CU(cudaEventRecord(p->ev[ie++], st));
+  CU(cudaStreamSynchronize(st));
+  *E_xc = p->h_result[0];
+  *N_el = p->h_result[1];
+  // stage timings
+  float t;
+  p->ms[0] = p->ms[1] = p->ms[2] = p->ms[3] = p->ms[4] = 0.f;
+  CU(cudaEventElapsedTime(&t, p->ev[0], p->ev[1])); p->ms[0] = t;
+  size_t k = 1;
+  for (size_t c = 0; c < hp.chunks.size(); ++c) {
+    CU(cudaEventElapsedTime(&t, p->ev[k], p->ev[k + 1])); p->ms[1] += t;   // includes the memsets on the first chunk
+    CU(cudaEventElapsedTime(&t, p->ev[k + 1], p->ev[k + 2])); p->ms[2] += t;
+    k += 2;
+  }
+  CU(cudaEventElapsedTime(&t, p->ev[k], p->ev[k + 1])); p->ms[3] = t;
+  CU(cudaEventElapsedTime(&t, p->ev[0], p->ev[k + 1])); p->ms[4] = t;
+  p->launches = launches;
+  return XC_OK;
+}
+
+int xc_eval_host(xc_plan* p, const double* hP, int64_t ldp, double* hV, int64_t ldv, double* E_xc, double* N_el, int32_t flags) {
+  if (!p || !hP || !hV) return fail(XC_EINVAL, "null argument");
+  if (p->device < 0) return fail(XC_ECUDA, "host-only plan (device = -1): no CUDA device bound, and there is no CPU fallback");
+  const int n = p->hp.nbasis;
+  if (ldp < n || ldv < n) return fail(XC_EINVAL, "leading dimension smaller than n_basis");
+  CU(cudaSetDevice(p->device));
+  size_t bytes = (size_t)n * n * 8;
+  if (!p->d_Ptmp) CU(cudaMalloc((void**)&p->d_Ptmp, bytes));
+  if (!p->d_Vtmp) CU(cudaMalloc((void**)&p->d_Vtmp, bytes));
+  CU(cudaMemcpy2DAsync(p->d_Ptmp, (size_t)n * 8, hP, (size_t)ldp * 8, (size_t)n * 8, n, cudaMemcpyHostToDevice, 0));
+  int rc = xc_eval(p, p->d_Ptmp, n, p->d_Vtmp, n, E_xc, N_el, flags, nullptr);
+  if (rc != XC_OK) return rc;
+  CU(cudaMemcpy2D(hV, (size_t)ldv * 8, p->d_Vtmp, (size_t)n * 8, (size_t)n * 8, n, cudaMemcpyDeviceToHost));
+  return XC_OK;
+}
+
+int xc_eval_diagnostics(xc_plan* p, double* w, double* rho, double* grad_rho, double* E_batch, double* N_batch) {
+  if (!p) return fail(XC_EINVAL, "plan is null");
+  if (p->device < 0) return fail(XC_ECUDA, "host-only plan (device = -1)");
+  const HostPlan& hp = p->hp;
+  CU(cudaSetDevice(p->device));
+  CU(cudaDeviceSynchronize());
+  if (w) CU(cudaMemcpy(w, p->d_w, hp.npts * 8, cudaMemcpyDeviceToHost));
+  if (rho) CU(cudaMemcpy(rho, p->d_rho, hp.npts * 8, cudaMemcpyDeviceToHost));
+  if (grad_rho) CU(cudaMemcpy(grad_rho, p->d_grho, hp.npts * 24, cudaMemcpyDeviceToHost));
+  if (E_batch || N_batch) {
+    size_t n64 = hp.items64.size(), n32 = hp.items32.size();
+    std::vector<double> ep(n64 + n32), np(n64 + n32);
+    if (n64 + n32) {
+      CU(cudaMemcpy(ep.data(), p->d_Epart, ep.size() * 8, cudaMemcpyDeviceToHost));
+      CU(cudaMemcpy(np.data(), p->d_Npart, np.size() * 8, cudaMemcpyDeviceToHost));
+    }
+    size_t nb = hp.batches.size();
+    if (E_batch) std::fill(E_batch, E_batch + nb, 0.0);
+    if (N_batch) std::fill(N_batch, N_batch + nb, 0.0);
+    for (size_t i = 0; i < n64 + n32; ++i) {
+      int j = i < n64 ? hp.items64[i].batch : hp.items32[i - n64].batch;
+      if (E_batch) E_batch[j] += ep[i];
+      if (N_batch) N_batch[j] += np[i];
+    }
+  }
+  return XC_OK;
+}
+
+int xc_eval_timings(const xc_plan* p, float ms[5], int32_t* launches) {
+  if (!p) return fail(XC_EINVAL, "plan is null");
+  if (ms) std::copy(p->ms, p->ms + 5, ms);
+  if (launches) *launches = p->launches;
+  return XC_OK;
+}
+
+int xc_plan_destroy(xc_plan* p) {
+  free_plan(p);
+  return XC_OK;
+}
+
+int xc_integrate(const xc_atom* atoms, int32_t natoms, const xc_shell* shells, int32_t nshells, const double* exps,
+                 const double* coefs, int32_t nprim_total, const xc_grid_spec* spec, int32_t device, const double* dP,
+                 int64_t ldp, double* dV, int64_t ldv, double* E_xc, double* N_el, void* cuda_stream) {
+  xc_plan* p = nullptr;
+  int rc = xc_plan_create(atoms, natoms, shells, nshells, exps, coefs, nprim_total, spec, device, &p);
+  if (rc != XC_OK) return rc;
+  rc = xc_eval(p, dP, ldp, dV, ldv, E_xc, N_el, 0, cuda_stream);
+  std::string keep = g_err;
+  xc_plan_destroy(p);
+  g_err = keep;
+  return rc;
+}
+
+int xc_partition_weights(const xc_atom* atoms, int32_t natoms, int32_t partition, int64_t npts, const double* dx,
+                         const double* dy, const double* dz, const double* dwq, const int32_t* dparent, double* dw_out,
+                         void* cuda_stream) {
+  if (!atoms || natoms < 1 || npts < 0 || (npts && (!dx || !dy || !dz || !dwq || !dparent || !dw_out)))
+    return fail(XC_EINVAL, "bad argument");
+  if (partition < 0 || partition > 1) return fail(XC_EINVAL, "bad partition enum");
+  std::vector<double> a(3 * (size_t)natoms), invR, rnn;
+  for (int i = 0; i < natoms; ++i) { a[3 * i] = atoms[i].x; a[3 * i + 1] = atoms[i].y; a[3 * i + 2] = atoms[i].z; }
+  atom_tables(a, natoms, invR, rnn);
+  double *da = nullptr, *di = nullptr, *dr = nullptr;
+  int rc = upload(&da, a);
+  if (rc == XC_OK) rc = upload(&di, invR);
+  if (rc == XC_OK) rc = upload(&dr, rnn);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (rc == XC_OK) {
+    cudaError_t e = launch_weights(partition, natoms, da, di, dr, npts, dx, dy, dz, dwq, dparent, dw_out, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) rc = cuda_fail(e, "xc_partition_weights");
+  }
+  cudaFree(da); cudaFree(di); cudaFree(dr);
+  return rc;
+}
+
+int xc_functional(int32_t functional, int64_t n, const double* drho, const double* dsigma, double rho_tol, double* df,
+                  double* dvrho, double* dvsigma, void* cuda_stream) {
+  if (functional < 0 || functional > 1 || n < 0 || (n && (!drho || !df || !dvrho || !dvsigma)) || (functional == 1 && n && !dsigma))
+    return fail(XC_EINVAL, "bad argument");
+  CU(launch_functional(functional, n, drho, dsigma, rho_tol, df, dvrho, dvsigma, (cudaStream_t)cuda_stream));
+  return XC_OK;
+}
+
+}  // extern "C"

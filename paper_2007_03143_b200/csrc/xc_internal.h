@@ -1,0 +1,75 @@
+// xc_internal.h -- structures shared by the host planner and the CUDA kernels of libxc_b200.
+// (Product code.  Shares nothing with oracle/.)
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/xc_b200.h"
+
+namespace xcb {
+
+constexpr int kMaxL = 2;
+constexpr int kMaxPrim = 16;
+constexpr int kKC = 8;          // nu-rows of P staged per pipeline stage in the density kernel
+constexpr int kMuPass = 192;    // mu columns handled per pass of the density kernel
+constexpr int kDensityThreads = 512;
+constexpr int kPotThreads = 256;
+constexpr int kPotKPart = 128;  // points per work item of the potential kernel
+constexpr size_t kSmemLimit = 227 * 1024;
+
+struct ShellRec {      // 48 bytes
+  double x, y, z;      // centre
+  int32_t L, nprim, prim_off, func_off;  // func_off: first GLOBAL function index
+  int32_t atom, _pad;
+};
+
+struct BatchRec {      // one quadrature batch B_j with its shell list S_j
+  int32_t pt_off, nq;          // first point (plan order), N_q^j
+  int32_t nq_pad;              // N_q^j rounded up to 4
+  int32_t sh_off, ns;          // offset into batch shell list, |S_j| in shells
+  int32_t f_off, nb;           // offset into batch function-index list, N_b^j
+  int32_t nb_pad8;             // N_b^j rounded up to 8
+  int64_t scr_off;             // offset (doubles) of this batch's Phi / Z workspace
+};
+
+struct DensityItem { int32_t batch, tile_start; };            // one CTA of the density kernel
+struct PotItem { int32_t batch; int16_t tm, tn; int32_t k0, k1; };  // one warp of the potential kernel
+
+inline int ncart(int L) { return (L + 1) * (L + 2) / 2; }
+inline int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
+
+// shared-memory footprint of the density kernel for a batch (bytes); T = points per tile
+size_t density_smem_bytes(int T, bool gga, int nb, int ns);
+
+struct HostPlan {
+  int natoms = 0, nshells = 0, nbasis = 0, nprim = 0;
+  xc_grid_spec spec{};
+  int64_t npts = 0;
+  std::vector<double> atoms;           // natoms*3
+  std::vector<ShellRec> shells;
+  std::vector<double> exps, coefs, rcut;
+  std::vector<double> px, py, pz, wq;  // plan order
+  std::vector<int32_t> parent;
+  std::vector<int64_t> orig;
+  std::vector<BatchRec> batches;
+  std::vector<int32_t> bshells;        // concatenated S_j (global shell ids, ascending)
+  std::vector<int32_t> bsfoff;         // per entry of bshells: first LOCAL function index of that shell in its batch
+  std::vector<int32_t> bfidx;          // concatenated global function indices of S_j
+  std::vector<int32_t> bfinfo;         // per local function: (local shell slot << 8) | (l<<4 | m<<2 | n)
+  std::vector<DensityItem> items64, items32;  // density-kernel work lists (tile of 64 / 32 points)
+  std::vector<PotItem> pot_items;
+  struct Chunk { int64_t b0, b1, i64_0, i64_1, i32_0, i32_1, p0, p1; int64_t scr; };
+  std::vector<Chunk> chunks;            // batches [b0,b1) share one pass over the Phi/Z workspace
+  int64_t scr_cap_doubles = 0;          // workspace doubles per matrix (max over chunks)
+  int64_t scr_doubles = 0;
+  double sum_nbnq = 0, sum_nb2 = 0, flops = 0;
+  int max_nb = 0, max_ns = 0;
+  size_t smem64 = 0, smem32 = 0;       // max dynamic smem over each density work list
+};
+
+// Builds grid, batches, screening, work lists.  Returns XC_OK or an error code (message in err).
+int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, int nshells, const double* exps,
+                    const double* coefs, int nprim_total, const xc_grid_spec* spec, HostPlan& hp, std::string& err);
+
+}  // namespace xcb

@@ -1,0 +1,358 @@
+// xc_planner.cpp -- host side of libxc_b200: atom-centred grid, spatial batching, shell screening,
+// work lists (step (b) of the hot path; the analogue of Alg. 3 l.3.5-3.7, on one GPU).
+//
+// Batching (free by PAPER.md:L124 "the choice of batching scheme does not effect the methodological
+// details"; reading A8): the WHOLE point cloud (all atoms pooled) is bisected recursively at the median
+// of the longest bounding-box axis until a cuboid holds <= max_batch_pts points; split sizes are rounded
+// to multiples of 64 so that almost every batch is a whole number of 64-point tiles.  Batches come out
+// in depth-first order, i.e. spatially coherent.  Eq. (11) holds by construction.
+// Screening: Alg. 1 (reading A7) on the tight bounding box of the batch's points with
+// the cutoff radius of Eq. (10).
+#include <algorithm>
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <numeric>
+
+#include "xc_internal.h"
+
+namespace xcb {
+
+namespace {
+
+const double kPiH = 3.141592653589793238462643383279502884;
+
+void radial_mura_knowles(int n, double alpha, std::vector<double>& r, std::vector<double>& w) {
+  r.resize(n); w.resize(n);
+  for (int i = 0; i < n; ++i) {
+    double x = double(i + 1) / double(n + 1);
+    double x3 = x * x * x;
+    double om = 1.0 - x3;
+    r[i] = -alpha * std::log(om);
+    double drdx = 3.0 * alpha * x * x / om;
+    w[i] = r[i] * r[i] * drdx / double(n + 1);
+  }
+}
+
+bool angular_rule(int kind, int n, std::vector<double>& u, std::vector<double>& w) {
+  u.resize(3 * (size_t)n); w.resize(n);
+  if (kind == 0) {  // Fibonacci sphere
+    const double ga = kPiH * (3.0 - std::sqrt(5.0));
+    for (int k = 0; k < n; ++k) {
+      double z = 1.0 - (2.0 * k + 1.0) / double(n);
+      double s = std::sqrt(1.0 - z * z), ph = k * ga;
+      u[3 * k] = s * std::cos(ph); u[3 * k + 1] = s * std::sin(ph); u[3 * k + 2] = z;
+      w[k] = 4.0 * kPiH / double(n);
+    }
+    return true;
+  }
+  if (kind == 1) {  // Gauss-Legendre in cos(theta) x trapezoid in phi
+    int nt = (int)std::lround(std::sqrt(n / 2.0));
+    if (nt < 1 || 2 * nt * nt != n) return false;
+    std::vector<double> xs(nt), ws(nt);
+    for (int i = 0; i < nt; ++i) {
+      double x = std::cos(kPiH * (i + 0.75) / (nt + 0.5)), dp = 1.0;
+      for (int it = 0; it < 64; ++it) {
+        double pm = 1.0, p = x;
+        for (int k = 1; k < nt; ++k) { double pn = ((2 * k + 1) * x * p - k * pm) / (k + 1); pm = p; p = pn; }
+        if (nt == 1) { pm = 1.0; p = x; }
+        dp = nt * (pm - x * p) / (1.0 - x * x);
+        double dx = p / dp;
+        x -= dx;
+        if (std::fabs(dx) < 1e-16) break;
+      }
+      double pm = 1.0, p = x;
+      for (int k = 1; k < nt; ++k) { double pn = ((2 * k + 1) * x * p - k * pm) / (k + 1); pm = p; p = pn; }
+      dp = nt * (pm - x * p) / (1.0 - x * x);
+      xs[i] = x; ws[i] = 2.0 / ((1.0 - x * x) * dp * dp);
+    }
+    int k = 0;
+    for (int i = 0; i < nt; ++i)
+      for (int m = 0; m < 2 * nt; ++m, ++k) {
+        double ph = (m + 0.5) * kPiH / nt, s = std::sqrt(1.0 - xs[i] * xs[i]);
+        u[3 * k] = s * std::cos(ph); u[3 * k + 1] = s * std::sin(ph); u[3 * k + 2] = xs[i];
+        w[k] = ws[i] * kPiH / nt;
+      }
+    return true;
+  }
+  return false;
+}
+
+struct Box { double lo[3], hi[3]; };
+
+inline bool sphere_hits_box(const double* c, double r, const Box& b) {
+  double d2 = 0.0;
+  for (int p = 0; p < 3; ++p) {
+    double t = c[p] < b.lo[p] ? b.lo[p] - c[p] : (c[p] > b.hi[p] ? c[p] - b.hi[p] : 0.0);
+    d2 += t * t;
+  }
+  return d2 <= r * r;
+}
+
+struct Leaf { int64_t begin, end; };
+
+}  // namespace
+
+size_t density_smem_bytes(int T, bool gga, int nb, int ns) {
+  // must mirror the shared-memory carve of k_density (xc_kernels.cu)
+  size_t nb4 = round_up(nb, 4);
+  size_t mb = std::min<size_t>(round_up(nb, T == 64 ? 32 : 64), kMuPass);
+  size_t npass = (nb + kMuPass - 1) / kMuPass;
+  size_t b = 0;
+  b += nb4 * (T + 4) * 8;                       // Phi panel
+  if (gga) b += (size_t)ns * T * 2 * 8;          // R0/R1 panel
+  b += 2 * (size_t)kKC * (mb + 4) * 8;           // P stages
+  b += (size_t)T * 8 * 12;                       // x,y,z,w, scratch, a,g0,g1,g2
+  b += 1024 * 8;                                 // cross-warp reduction buffer
+  b += (size_t)ns * sizeof(ShellRec);            // shell records
+  b += npass * kMuPass * 4 + nb4 * 4;            // padded function indices (mu side) + (nu side)
+  b += nb4 * 4;                                  // function info
+  return b + 64;
+}
+
+int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, int nshells, const double* exps,
+                    const double* coefs, int nprim_total, const xc_grid_spec* spec, HostPlan& hp, std::string& err) {
+  if (!atoms || !shells || !exps || !coefs || !spec) { err = "null argument"; return XC_EINVAL; }
+  if (natoms < 1 || nshells < 1 || nprim_total < 1) { err = "empty system"; return XC_EINVAL; }
+  if (spec->n_rad < 1 || spec->n_ang < 1 || spec->max_batch_pts < 1 || spec->max_batch_pts > 512) {
+    err = "bad grid_spec sizes (need n_rad,n_ang >= 1 and 1 <= max_batch_pts <= 512)"; return XC_EINVAL;
+  }
+  if (spec->radial != 0 || spec->angular < 0 || spec->angular > 1 || spec->partition < 0 || spec->partition > 1 ||
+      spec->functional < 0 || spec->functional > 1) { err = "bad grid_spec enum"; return XC_EINVAL; }
+  if (!(spec->eta > 0.0) || !(spec->mk_alpha > 0.0) || !(spec->rho_tol >= 0.0)) { err = "bad grid_spec reals"; return XC_EINVAL; }
+  hp.natoms = natoms; hp.nshells = nshells; hp.nprim = nprim_total; hp.spec = *spec;
+  hp.atoms.resize(3 * (size_t)natoms);
+  for (int a = 0; a < natoms; ++a) { hp.atoms[3 * a] = atoms[a].x; hp.atoms[3 * a + 1] = atoms[a].y; hp.atoms[3 * a + 2] = atoms[a].z; }
+  hp.exps.assign(exps, exps + nprim_total);
+  hp.coefs.assign(coefs, coefs + nprim_total);
+  for (int k = 0; k < nprim_total; ++k)
+    if (!(exps[k] > 0.0) || !std::isfinite(exps[k]) || !std::isfinite(coefs[k])) { err = "non-positive or non-finite exponent/coefficient"; return XC_EINVAL; }
+  hp.shells.resize(nshells); hp.rcut.resize(nshells);
+  int foff = 0;
+  for (int s = 0; s < nshells; ++s) {
+    const xc_shell& sh = shells[s];
+    if (sh.atom < 0 || sh.atom >= natoms || sh.nprim < 1 || sh.prim_off < 0 || sh.prim_off + sh.nprim > nprim_total || sh.L < 0) {
+      err = "bad shell record"; return XC_EINVAL;
+    }
+    if (sh.L > kMaxL) { err = "angular momentum L > 2 is not supported"; return XC_EUNSUPPORTED; }
+    if (sh.nprim > kMaxPrim) { err = "contraction depth > 16 is not supported"; return XC_EUNSUPPORTED; }
+    ShellRec& r = hp.shells[s];
+    r.x = atoms[sh.atom].x; r.y = atoms[sh.atom].y; r.z = atoms[sh.atom].z;
+    r.L = sh.L; r.nprim = sh.nprim; r.prim_off = sh.prim_off; r.func_off = foff; r.atom = sh.atom; r._pad = 0;
+    foff += ncart(sh.L);
+    double m = 0.0;  // Eq. (10)
+    for (int k = 0; k < sh.nprim; ++k) {
+      double al = exps[sh.prim_off + k];
+      double v = (0.5 * std::log(al) - std::log(spec->eta)) / al;
+      if (v > 0.0) m = std::max(m, std::sqrt(v));
+    }
+    hp.rcut[s] = m;
+  }
+  hp.nbasis = foff;
+
+  // ---- grid (canonical order: atom-major, radial, angular) ----
+  std::vector<double> rr, rw, au, aw;
+  radial_mura_knowles(spec->n_rad, spec->mk_alpha, rr, rw);
+  if (!angular_rule(spec->angular, spec->n_ang, au, aw)) { err = "angular rule: n_ang must be 2*n_theta^2 for the product rule"; return XC_EINVAL; }
+  const int64_t per_atom = (int64_t)spec->n_rad * spec->n_ang;
+  const int64_t npts = per_atom * natoms;
+  if (npts >= (int64_t)1 << 31) { err = "more than 2^31 grid points"; return XC_EUNSUPPORTED; }
+  hp.npts = npts;
+  std::vector<double> cx(npts), cy(npts), cz(npts);
+#pragma omp parallel for schedule(static)
+  for (int64_t p = 0; p < npts; ++p) {
+    int a = (int)(p / per_atom);
+    int64_t q = p % per_atom;
+    int i = (int)(q / spec->n_ang), k = (int)(q % spec->n_ang);
+    cx[p] = hp.atoms[3 * a] + rr[i] * au[3 * k];
+    cy[p] = hp.atoms[3 * a + 1] + rr[i] * au[3 * k + 1];
+    cz[p] = hp.atoms[3 * a + 2] + rr[i] * au[3 * k + 2];
+  }
+
+  // ---- recursive median bisection ----
+  std::vector<int64_t> idx(npts);
+  std::iota(idx.begin(), idx.end(), (int64_t)0);
+  const int maxp = spec->max_batch_pts;
+  const double* coord[3] = {cx.data(), cy.data(), cz.data()};
+  std::vector<Leaf> leaves;
+  {
+    std::vector<Leaf> stack;
+    stack.push_back({0, npts});
+    // depth-first, left part first => spatially coherent output order
+    while (!stack.empty()) {
+      Leaf cur = stack.back(); stack.pop_back();
+      int64_t n = cur.end - cur.begin;
+      if (n <= maxp) { leaves.push_back(cur); continue; }
+      double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+      for (int64_t k = cur.begin; k < cur.end; ++k)
+        for (int p = 0; p < 3; ++p) { double v = coord[p][idx[k]]; lo[p] = std::min(lo[p], v); hi[p] = std::max(hi[p], v); }
+      int ax = 0;
+      for (int p = 1; p < 3; ++p) if (hi[p] - lo[p] > hi[ax] - lo[ax]) ax = p;
+      int64_t half = n / 2;
+      if (maxp >= 64 && n >= 128) half = std::max<int64_t>(64, half / 64 * 64);
+      const double* c = coord[ax];
+      std::nth_element(idx.begin() + cur.begin, idx.begin() + cur.begin + half, idx.begin() + cur.end,
+                       [c](int64_t a, int64_t b) { return c[a] < c[b] || (c[a] == c[b] && a < b); });
+      stack.push_back({cur.begin + half, cur.end});
+      stack.push_back({cur.begin, cur.begin + half});
+    }
+  }
+
+  // ---- per-batch shell screening (Alg. 1 on the tight bounding box), with re-splitting of batches whose
+  //      shell list exceeds the density kernel's shared-memory capacity ----
+  std::vector<std::vector<int>> atom_shells(natoms);
+  std::vector<double> atom_rmax(natoms, 0.0);
+  for (int s = 0; s < nshells; ++s) {
+    atom_shells[hp.shells[s].atom].push_back(s);
+    atom_rmax[hp.shells[s].atom] = std::max(atom_rmax[hp.shells[s].atom], hp.rcut[s]);
+  }
+  const bool gga = spec->functional == 1;
+  auto screen = [&](const Leaf& lf, std::vector<int32_t>& out, int& nb) {
+    Box b;
+    for (int p = 0; p < 3; ++p) { b.lo[p] = 1e300; b.hi[p] = -1e300; }
+    for (int64_t k = lf.begin; k < lf.end; ++k)
+      for (int p = 0; p < 3; ++p) { double v = coord[p][idx[k]]; b.lo[p] = std::min(b.lo[p], v); b.hi[p] = std::max(b.hi[p], v); }
+    out.clear(); nb = 0;
+    for (int a = 0; a < natoms; ++a) {
+      if (!sphere_hits_box(&hp.atoms[3 * a], atom_rmax[a], b)) continue;
+      for (int s : atom_shells[a])
+        if (sphere_hits_box(&hp.atoms[3 * a], hp.rcut[s], b)) { out.push_back(s); nb += ncart(hp.shells[s].L); }
+    }
+    std::sort(out.begin(), out.end());
+  };
+  std::vector<std::vector<int32_t>> lists(leaves.size());
+  std::vector<int> nbs(leaves.size());
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t j = 0; j < (int64_t)leaves.size(); ++j) screen(leaves[j], lists[j], nbs[j]);
+  // re-split oversized batches (rare): sequential fix-up pass
+  {
+    std::vector<Leaf> L2; std::vector<std::vector<int32_t>> S2; std::vector<int> N2;
+    bool any = false;
+    for (size_t j = 0; j < leaves.size(); ++j)
+      if (density_smem_bytes(32, gga, nbs[j], (int)lists[j].size()) > kSmemLimit) { any = true; break; }
+    if (any) {
+      for (size_t j = 0; j < leaves.size(); ++j) {
+        std::vector<Leaf> st{leaves[j]};
+        bool first = true;
+        while (!st.empty()) {
+          Leaf cur = st.back(); st.pop_back();
+          std::vector<int32_t> sl; int nb;
+          if (first) { sl = lists[j]; nb = nbs[j]; first = false; } else screen(cur, sl, nb);
+          int64_t n = cur.end - cur.begin;
+          if (density_smem_bytes(32, gga, nb, (int)sl.size()) <= kSmemLimit) { L2.push_back(cur); S2.push_back(sl); N2.push_back(nb); continue; }
+          if (n <= 1) { err = "a single grid point sees more basis functions than the density kernel supports"; return XC_EUNSUPPORTED; }
+          double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+          for (int64_t k = cur.begin; k < cur.end; ++k)
+            for (int p = 0; p < 3; ++p) { double v = coord[p][idx[k]]; lo[p] = std::min(lo[p], v); hi[p] = std::max(hi[p], v); }
+          int ax = 0;
+          for (int p = 1; p < 3; ++p) if (hi[p] - lo[p] > hi[ax] - lo[ax]) ax = p;
+          int64_t half = n / 2;
+          const double* c = coord[ax];
+          std::nth_element(idx.begin() + cur.begin, idx.begin() + cur.begin + half, idx.begin() + cur.end,
+                           [c](int64_t a, int64_t b) { return c[a] < c[b] || (c[a] == c[b] && a < b); });
+          st.push_back({cur.begin + half, cur.end});
+          st.push_back({cur.begin, cur.begin + half});
+        }
+      }
+      leaves.swap(L2); lists.swap(S2); nbs.swap(N2);
+    }
+  }
+
+  // ---- permuted point arrays ----
+  hp.px.resize(npts); hp.py.resize(npts); hp.pz.resize(npts); hp.wq.resize(npts); hp.parent.resize(npts); hp.orig.resize(npts);
+#pragma omp parallel for schedule(static)
+  for (int64_t k = 0; k < npts; ++k) {
+    int64_t p = idx[k];
+    hp.px[k] = cx[p]; hp.py[k] = cy[p]; hp.pz[k] = cz[p];
+    int a = (int)(p / per_atom);
+    int64_t q = p % per_atom;
+    hp.wq[k] = rw[q / spec->n_ang] * aw[q % spec->n_ang];
+    hp.parent[k] = a; hp.orig[k] = p;
+  }
+
+  // ---- batch records, function lists, work items ----
+  const int64_t nbatch = (int64_t)leaves.size();
+  hp.batches.resize(nbatch);
+  int64_t sh_off = 0, f_off = 0, scr = 0, scr_total = 0;
+  // workspace cap per matrix (doubles): batches are processed in chunks that fit (analogue of Alg. 2 l.2.5-2.8)
+  int64_t cap = (int64_t)2 << 30;  // 2 Gi doubles = 16 GiB per matrix
+  if (const char* e = getenv("XC_B200_WORKSPACE_MB")) cap = std::max<int64_t>(1, atoll(e)) * (1 << 20) / 8;
+  hp.chunks.clear();
+  HostPlan::Chunk ch{0, 0, 0, 0, 0, 0, 0, 0, 0};
+  std::vector<int64_t> chunk_of(nbatch);
+  for (int64_t j = 0; j < nbatch; ++j) {
+    BatchRec& b = hp.batches[j];
+    b.pt_off = (int32_t)leaves[j].begin; b.nq = (int32_t)(leaves[j].end - leaves[j].begin);
+    b.nq_pad = (int32_t)round_up(b.nq, 4);
+    b.sh_off = (int32_t)sh_off; b.ns = (int32_t)lists[j].size();
+    b.f_off = (int32_t)f_off; b.nb = nbs[j]; b.nb_pad8 = (int32_t)round_up(b.nb, 8);
+    int64_t need = (int64_t)b.nb_pad8 * b.nq_pad;
+    if (scr + need > cap && scr > 0) {  // close the chunk
+      ch.b1 = j; ch.scr = scr; hp.chunks.push_back(ch);
+      hp.scr_cap_doubles = std::max(hp.scr_cap_doubles, scr);
+      ch = HostPlan::Chunk{j, 0, 0, 0, 0, 0, 0, 0, 0};
+      scr = 0;
+    }
+    chunk_of[j] = (int64_t)hp.chunks.size();
+    b.scr_off = scr;
+    sh_off += b.ns; f_off += b.nb;
+    scr += need; scr_total += need;
+    if (sh_off >= ((int64_t)1 << 31) || f_off >= ((int64_t)1 << 31)) { err = "batch lists exceed 2^31 entries"; return XC_EUNSUPPORTED; }
+  }
+  ch.b1 = nbatch; ch.scr = scr; hp.chunks.push_back(ch);
+  hp.scr_cap_doubles = std::max(hp.scr_cap_doubles, scr);
+  hp.scr_doubles = scr_total;
+  hp.bshells.resize(sh_off); hp.bsfoff.resize(sh_off); hp.bfidx.resize(f_off); hp.bfinfo.resize(f_off);
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t j = 0; j < nbatch; ++j) {
+    const BatchRec& b = hp.batches[j];
+    int f = b.f_off;
+    for (int k = 0; k < b.ns; ++k) {
+      int s = lists[j][k];
+      hp.bshells[b.sh_off + k] = s;
+      hp.bsfoff[b.sh_off + k] = f - b.f_off;
+      int L = hp.shells[s].L, c = 0;
+      for (int l = L; l >= 0; --l)
+        for (int m = L - l; m >= 0; --m, ++c, ++f) {
+          int n = L - l - m;
+          hp.bfidx[f] = hp.shells[s].func_off + c;
+          hp.bfinfo[f] = (k << 8) | (l << 4) | (m << 2) | n;
+        }
+    }
+  }
+  hp.sum_nbnq = hp.sum_nb2 = hp.flops = 0; hp.max_nb = hp.max_ns = 0; hp.smem64 = hp.smem32 = 0;
+  for (int64_t j = 0; j < nbatch; ++j) {
+    const BatchRec& b = hp.batches[j];
+    hp.sum_nbnq += (double)b.nb * b.nq; hp.sum_nb2 += (double)b.nb * b.nb; hp.flops += 4.0 * b.nb * (double)b.nb * b.nq;
+    hp.max_nb = std::max(hp.max_nb, b.nb); hp.max_ns = std::max(hp.max_ns, b.ns);
+    if (b.nb == 0) continue;  // nothing to integrate: rho = 0 on every point
+    size_t s64 = density_smem_bytes(64, gga, b.nb, b.ns);
+    if (s64 <= kSmemLimit) {
+      hp.smem64 = std::max(hp.smem64, s64);
+      for (int t = 0; t < b.nq; t += 64) hp.items64.push_back({(int32_t)j, t});
+    } else {
+      hp.smem32 = std::max(hp.smem32, density_smem_bytes(32, gga, b.nb, b.ns));
+      for (int t = 0; t < b.nq; t += 32) hp.items32.push_back({(int32_t)j, t});
+    }
+    int nt = (b.nb + 31) / 32;
+    int nparts = (b.nq_pad + kPotKPart - 1) / kPotKPart;
+    for (int kp = 0; kp < nparts; ++kp) {
+      // equalised part boundaries, multiples of 4
+      int k0 = (int)((int64_t)b.nq_pad / 4 * kp / nparts) * 4, k1 = (int)((int64_t)b.nq_pad / 4 * (kp + 1) / nparts) * 4;
+      for (int tm = 0; tm < nt; ++tm)
+        for (int tn = 0; tn <= tm; ++tn) hp.pot_items.push_back({(int32_t)j, (int16_t)tm, (int16_t)tn, k0, k1});
+    }
+  }
+  // work-item ranges per chunk (lists are in batch order)
+  {
+    size_t i64 = 0, i32 = 0, ip = 0;
+    for (auto& c : hp.chunks) {
+      c.i64_0 = (int64_t)i64; while (i64 < hp.items64.size() && hp.items64[i64].batch < c.b1) ++i64; c.i64_1 = (int64_t)i64;
+      c.i32_0 = (int64_t)i32; while (i32 < hp.items32.size() && hp.items32[i32].batch < c.b1) ++i32; c.i32_1 = (int64_t)i32;
+      c.p0 = (int64_t)ip; while (ip < hp.pot_items.size() && hp.pot_items[ip].batch < c.b1) ++ip; c.p1 = (int64_t)ip;
+    }
+  }
+  return XC_OK;
+}
+
+}  // namespace xcb
