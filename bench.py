@@ -1,0 +1,337 @@
+#!/usr/bin/env python
+"""bench.py -- grid points/s of the full E_xc + V_xc + N_el build (fp64) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2] [--also c4,c5] [--impl reference]
+
+A step = one pass of the whole hot path (weights -> density -> potential -> scatter/finalise) over one
+synthetic water-cluster workload (BASELINE.json:configs; generator: workloads/).  Prints ONE JSON line.
+N > 1 (torchrun): the path is not sharded ("replicas only"): every rank runs the same build on
+its own GPU, value = N * points / max-over-ranks device time, scaling = "weak".
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "grid points/s for full E_xc+V_xc build (fp64, 1 B200); % of FP64 roofline"
+UNIT = "grid points/s"
+FP64_PEAK_TFLOPS = 37.2   # 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz; DMMA microbenchmark measured 37.18 (profiles/)
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            d = json.load(fh)
+        return float(d.get("hbm_gbs", 6650.0)), "measured"
+    return 6650.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.thr, self.index = [], None, None, index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True)
+            self.thr.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def __exit__(self, *a):
+        if self.proc:
+            time.sleep(0.15)
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+                for n, v in zip(names, f[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                pass
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def _hist(a):
+    import numpy as np
+    a = np.asarray(a, dtype=float)
+    return {"mean": float(a.mean()), "p50": float(np.percentile(a, 50)), "p95": float(np.percentile(a, 95)), "max": float(a.max())}
+
+
+def run_workload(name, steps, warmup, functional=None, do_e2e=True, device=0, sampler=None):
+    """Times `steps` full builds of workload `name` on the current GPU. Returns a dict of measurements."""
+    import numpy as np
+    import torch
+
+    import paper_2007_03143_b200 as xc
+    from workloads import make_workload
+
+    w = make_workload(name)
+    fn = w.functional if functional is None else functional
+    t0 = time.perf_counter()
+    plan = xc.Plan.from_workload(w, spec=xc.grid_spec(w.n_rad, w.n_ang, fn), device=device)
+    plan_s = time.perf_counter() - t0
+    P = torch.from_numpy(w.P).cuda()
+    V = torch.empty_like(P)
+    flush = torch.empty(256 * 1024 * 1024 // 8, dtype=torch.float64, device="cuda")  # > 126 MB L2
+    ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(steps)]
+    ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(steps)]
+    for _ in range(warmup):
+        plan.eval(P, V)
+    torch.cuda.synchronize()
+    stage = {"weights_ms": 0.0, "density_ms": 0.0, "potential_ms": 0.0, "finalize_ms": 0.0}
+    launches = 0
+    E = N = 0.0
+    ctx = sampler if sampler is not None else ClockSampler(device)
+    with ctx:
+        for k in range(steps):
+            flush.fill_(float(k))           # L2 flush between timed iterations (untimed)
+            ev0[k].record()
+            E, N, _ = plan.eval(P, V)
+            ev1[k].record()
+            tm = plan.timings()
+            for key in stage:
+                stage[key] += tm[key]
+            launches += tm["launches"]
+        torch.cuda.synchronize()
+    total_ms = sum(a.elapsed_time(b) for a, b in zip(ev0, ev1))
+    ms = total_ms / steps
+    for key in stage:
+        stage[key] /= steps
+    # cached-weights build (reading A16), reported next to the full build
+    t_c = []
+    for k in range(min(steps, 5)):
+        flush.fill_(1.0)
+        plan.eval(P, V, reuse_weights=True)
+        t_c.append(plan.timings()["total_ms"])
+    res = dict(workload=name, functional="PBE" if fn == 1 else "Slater+VWN5", n_points=plan.n_points, n_basis=plan.n_basis,
+               n_atoms=int(len(w.atoms_Z)), n_batches=plan.n_batches, ms_per_step=ms, stage_ms=stage, launches=launches,
+               E_xc=E, N_el=N, N_el_rel_err_vs_trPS=abs(N - 2.0 * w.n_occ) / (2.0 * w.n_occ), plan_seconds=plan_s,
+               cached_weights_ms=float(np.median(t_c)), flops=plan.algorithmic_flops, stats=plan.stats())
+    res["points_per_s"] = plan.n_points / (ms * 1e-3)
+    res["builds_per_s"] = 1e3 / ms
+    res["fp64_tflops"] = plan.algorithmic_flops / (ms * 1e-3) * 1e-12
+    res["fp64_frac"] = res["fp64_tflops"] / FP64_PEAK_TFLOPS
+    ex = plan.export()
+    nq = np.diff(ex.batch_off)
+    foff = (np.asarray(w.shell_L, np.int64) + 1) * (np.asarray(w.shell_L, np.int64) + 2) // 2
+    csum = np.concatenate([[0], np.cumsum(foff[ex.shells])])
+    nbj = csum[ex.shell_off[1:]] - csum[ex.shell_off[:-1]]
+    res["nq_hist"] = _hist(nq)
+    res["nb_hist"] = _hist(nbj)
+    if do_e2e:
+        # end to end through the C ABI with HOST buffers (pinned): H2D of P and D2H of V inside the timed region
+        Ph = torch.from_numpy(w.P).pin_memory()
+        Vh = torch.empty_like(Ph).pin_memory()
+        plan.eval_host(Ph, Vh)
+        t = []
+        for k in range(max(3, min(steps, 10))):
+            flush.fill_(2.0)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            plan.eval_host(Ph, Vh)
+            t.append(time.perf_counter() - t0)
+        e2e_s = statistics.mean(t)
+        nb2 = plan.n_basis * plan.n_basis * 8
+        res["e2e"] = {"value": plan.n_points / e2e_s, "unit": UNIT, "h2d_bytes_per_step": nb2, "d2h_bytes_per_step": nb2 + 16,
+                      "ms_per_step": e2e_s * 1e3}
+        assert float((Vh - V.cpu()).abs().max()) == 0.0
+    plan.close()
+    del P, V, flush
+    torch.cuda.empty_cache()
+    return res, w
+
+
+def oracle_sample(w, name, target_seconds=15.0, stride=None, fn=None):
+    """Times the CPU oracle as it stands (Mode A, its own paper-literal planner, SSF weights with its exact
+    pruning) on a bounded sample of the workload: every `stride`-th atom's batches."""
+    import numpy as np
+
+    import oracle as orc
+    fn = w.functional if fn is None else fn
+    basis = (w.shell_atom, w.shell_L, w.shell_nprim, w.shell_prim_off, w.exps, w.coefs)
+    na = len(w.atoms_Z)
+    if stride is None:
+        # calibrated here: ~1.7 core-seconds per atom-centred grid at 64 waters (LDA, 75x302); the weights term grows with N_atoms
+        per_atom = 0.85 * (1 + na / 200.0) * (1.6 if fn == 1 else 1.0) * (w.n_rad * w.n_ang / 22650.0) / max(1, orc.num_threads())
+        stride = max(1, int(round(na * per_atom / target_seconds)))
+    atoms = np.arange(0, na, stride)
+    t0 = time.perf_counter()
+    pts, wq, par = orc.build_grid(w.atoms_xyz, w.n_rad, w.n_ang)
+    sel = np.isin(par, atoms)
+    pts, wq, par = pts[sel], wq[sel], par[sel]
+    rc = orc.rcut(w.shell_nprim, w.shell_prim_off, w.exps)
+    plan = orc.plan_paper(w.atoms_xyz, pts, wq, par, w.shell_atom, rc)
+    wts = orc.partition_weights(w.atoms_xyz, plan.pts, plan.wq, plan.parent, 0, True)
+    r = orc.evaluate(plan, wts, basis, w.atoms_xyz, w.P, fn, want_V=True)
+    dt = time.perf_counter() - t0
+    return dict(value=len(pts) / dt, unit=UNIT, cores=orc.num_threads(), kind="oracle", seconds=dt,
+                sample="atom-centred grids of %d of %d atoms (every %d-th), %d points, %d batches of the oracle's own "
+                       "paper-literal planner; grid + SSF weights + Alg. 4 incl. V; %s"
+                       % (len(atoms), na, stride, len(pts), plan.n_batches, name), E_sample=r.E_xc)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="c2")
+    ap.add_argument("--also", default="c3,c4,c5", help="comma list of extra workloads reported under other_workloads (or 'none')")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
+
+    from workloads import make_workload
+
+    if args.impl == "reference":
+        # the reference arm of this tier = the CPU oracle, as it stands, on the host cores; rank 0 only
+        if rank != 0:
+            return
+        w = make_workload(args.workload)
+        times, last = [], None
+        for k in range(args.warmup + args.steps):
+            last = oracle_sample(w, args.workload, target_seconds=6.0)
+            if k >= args.warmup:
+                times.append(last["seconds"])
+        npts_sample = last["value"] * last["seconds"]
+        val = npts_sample / statistics.mean(times)
+        line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": statistics.mean(times) * 1e3, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": args.workload, "functional": "PBE" if w.functional == 1 else "Slater+VWN5"},
+                "cpu_baseline": {"value": val, "unit": UNIT, "cores": last["cores"], "kind": "oracle", "sample": last["sample"]},
+                "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+        print(json.dumps(line))
+        return
+
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local_rank)
+    res, w = run_workload(args.workload, args.steps, warmup, device=local_rank, sampler=sampler)
+    ms = res["ms_per_step"]
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+        e = torch.tensor([res["e2e"]["ms_per_step"]], dtype=torch.float64, device="cuda")
+        dist.all_reduce(e, op=dist.ReduceOp.MAX)
+        res["e2e"]["value"] = world * res["n_points"] / (float(e.item()) * 1e-3)
+        dist.barrier()
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    hbm_peak, hbm_src = _peaks()
+    value = world * res["n_points"] / (ms * 1e-3)
+    # dominant kernel by device time; its roofline
+    st = res["stage_ms"]
+    stats = res["stats"]
+    gga = w.functional == 1
+    dom = max(("weights_ms", "density_ms", "potential_ms"), key=lambda k: st[k])
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        try:
+            with open(tpath) as fh:
+                traffic = json.load(fh).get(args.workload, {}).get(dom)
+        except Exception:
+            traffic = None
+    half = 0.5 * res["flops"]   # X GEMM and SYR2K are 2 (N_b^j)^2 N_q^j each
+    if dom == "density_ms":
+        roof = {"kernel": "k_density", "bound": "tensor", "achieved": half / (st[dom] * 1e-3) * 1e-12, "peak": FP64_PEAK_TFLOPS,
+                "unit": "TFLOP/s"}
+    elif dom == "potential_ms":
+        roof = {"kernel": "k_potential", "bound": "tensor", "achieved": half / (st[dom] * 1e-3) * 1e-12, "peak": FP64_PEAK_TFLOPS,
+                "unit": "TFLOP/s"}
+    else:
+        # step (a) is plain FP64 ALU work; algorithmic bytes are 44 B/point (x,y,z,w^q,parent in; w out)
+        roof = {"kernel": "k_weights", "bound": "hbm", "achieved": 44.0 * res["n_points"] / (st[dom] * 1e-3) * 1e-9,
+                "peak": hbm_peak, "unit": "GB/s"}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof["traffic"] = traffic
+    roof["peak_source"] = ("FP64 pipe: 148 SM x 64 FMA/clk x 2 x 1.965 GHz (DMMA microbenchmark: 37.18 measured)"
+                           if roof["unit"] == "TFLOP/s" else "MEASURED_PEAKS.json hbm_gbs (%s)" % hbm_src)
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warmup,
+            "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": "%s: 64-water cluster, 192 atoms, 1600 basis functions, 75x302 grid, %s" %
+                                   (args.workload, res["functional"]) if args.workload in ("c2", "c3") else args.workload,
+                       "workload_id": args.workload, "functional": res["functional"], "n_points": res["n_points"],
+                       "n_basis": res["n_basis"], "n_atoms": res["n_atoms"], "n_batches": res["n_batches"],
+                       "partition": "SSF", "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "l2": "flushed between timed iterations (256 MB fill)", "seed": 200703143},
+            "clocks": sampler.summary(), "e2e": {k: res["e2e"][k] for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step")},
+            "gpu_launches": res["launches"], "roofline": roof,
+            "builds_per_s": world * 1e3 / ms, "fp64_tflops": res["flops"] / (ms * 1e-3) * 1e-12,
+            "fp64_roofline_frac": res["flops"] / (ms * 1e-3) * 1e-12 / FP64_PEAK_TFLOPS,
+            "stage_ms": st, "cached_weights_ms": res["cached_weights_ms"],
+            "cached_weights_points_per_s": res["n_points"] / (res["cached_weights_ms"] * 1e-3),
+            "plan": {"seconds": res["plan_seconds"], "algorithmic_flops": res["flops"], "sum_nb_nq": stats["sum_nb_nq"],
+                     "sum_nb2": stats["sum_nb2"], "nq_hist": res["nq_hist"], "nb_hist": res["nb_hist"], "kind": "global k-d bisection"},
+            "E_xc": res["E_xc"], "N_el": res["N_el"], "N_el_rel_err_vs_trPS": res["N_el_rel_err_vs_trPS"]}
+    if not args.no_cpu_baseline:
+        cb = oracle_sample(w, args.workload)
+        line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample", "seconds")}
+    others = []
+    if args.also and args.also != "none" and world == 1:
+        for nm in args.also.split(","):
+            if nm == args.workload:
+                continue
+            try:
+                r2, _ = run_workload(nm, max(3, min(args.steps, 5)), 3, do_e2e=False, device=local_rank, sampler=ClockSampler(local_rank))
+                others.append({k: r2[k] for k in ("workload", "functional", "n_points", "n_basis", "n_batches", "ms_per_step",
+                                                  "points_per_s", "builds_per_s", "fp64_tflops", "fp64_frac", "stage_ms",
+                                                  "cached_weights_ms", "N_el_rel_err_vs_trPS", "nb_hist", "nq_hist")})
+            except Exception as exc:  # an extra workload must never cost the headline line
+                others.append({"workload": nm, "error": repr(exc)[:200]})
+    line["other_workloads"] = others
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

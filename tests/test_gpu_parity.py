@@ -1,0 +1,266 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI binding, against the CPU oracle on the
+same seeded inputs.  Tolerances are BASELINE.json:north_star's: max|dV| <= 1e-10 max|V|, rel. error of E_xc
+and N_el <= 1e-11.  The oracle runs in Mode A on the library's exported plan (reading A9), after
+validating that plan independently (P9)."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from parity_util import TOL_S, TOL_V, basis_of, oracle_plan, report, run_gpu, run_oracle
+from workloads import make_workload
+
+pytestmark = pytest.mark.gpu
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+@pytest.fixture(scope="module")
+def xc():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2007_03143_b200 as m
+    assert os.path.exists(m.LIB_PATH)
+    return m
+
+
+def _check(rep):
+    assert rep["dV"] <= TOL_V, rep
+    assert rep["dE"] <= TOL_S and rep["dN"] <= TOL_S, rep
+    assert rep["asym"] == 0.0, rep
+    if "dw" in rep:
+        assert rep["dw"] <= 1e-13, rep
+    if "drho" in rep:
+        assert rep["drho"] <= 1e-12, rep
+
+
+def _full_parity(orc, name, functional, partition=0, **spec_kw):
+    w = make_workload(name)
+    plan, g = run_gpu(w, functional, partition=partition, **spec_kw)
+    ex = plan.export()
+    rc = orc.rcut(w.shell_nprim, w.shell_prim_off, w.exps)
+    assert orc.validate_plan(oracle_plan(orc, ex), w.atoms_xyz, w.shell_atom, rc, spec_kw.get("max_batch_pts", 512)) == 0
+    op, wts, r = run_oracle(orc, w, ex, functional, partition)
+    rep = report(g, r, wts)
+    _check(rep)
+    assert np.max(np.abs(g["E_batch"] - r.E_batch)) <= 1e-12 * abs(r.E_xc)
+    assert np.max(np.abs(g["N_batch"] - r.N_batch)) <= 1e-12 * abs(r.N_el)
+    if functional == 1:
+        assert np.max(np.abs(g["grad_rho"] - r.grad_rho)) <= 1e-12 * np.max(np.abs(r.grad_rho))
+    return w, plan, g, r
+
+
+@pytest.mark.parametrize("functional", [0, 1])
+def test_c1_monomer(xc, orc, functional):
+    w, plan, g, r = _full_parity(orc, "c1", functional)
+    assert abs(g["N"] - 10.0) / 10.0 < 2e-4   # P2 at the stated 50x194 Fibonacci grid
+    plan.close()
+
+
+def test_w8_becke_partition(xc, orc):
+    _, plan, _, _ = _full_parity(orc, "w8", 1, partition=1)
+    plan.close()
+
+
+def test_w27_pbe(xc, orc):
+    _, plan, _, _ = _full_parity(orc, "w27", 1)
+    plan.close()
+
+
+def test_c2_lda_64_waters(xc, orc):
+    w, plan, g, r = _full_parity(orc, "c2", 0)
+    assert abs(g["N"] - 640.0) / 640.0 < 2e-4
+    plan.close()
+
+
+def test_c3_pbe_64_waters(xc, orc):
+    _, plan, _, _ = _full_parity(orc, "c3", 1)
+    plan.close()
+
+
+@pytest.mark.parametrize("max_pts,angular,n_ang", [(37, 0, 194), (100, 1, 288), (512, 0, 50), (1, 0, 6)])
+def test_ragged_batches_and_product_grid(xc, orc, max_pts, angular, n_ang):
+    # batch sizes that are not multiples of the 64-point tile; the Gauss-Legendre product rule; 1-point batches
+    w = make_workload("c1")
+    w.n_ang = n_ang
+    if max_pts == 1:
+        w.n_rad = 20
+    plan, g = run_gpu(w, 1, max_batch_pts=max_pts, angular=angular)
+    ex = plan.export()
+    rc = orc.rcut(w.shell_nprim, w.shell_prim_off, w.exps)
+    assert orc.validate_plan(oracle_plan(orc, ex), w.atoms_xyz, w.shell_atom, rc, max_pts) == 0
+    assert np.diff(ex.batch_off).max() <= max_pts
+    _, wts, r = run_oracle(orc, w, ex, 1)
+    _check(report(g, r, wts))
+    plan.close()
+
+
+@pytest.mark.parametrize("alpha", [0.5, 3.0])
+def test_one_atom_one_shell_closed_form(xc, alpha):
+    # pin P1 through the CUDA path: Slater exchange of one normalised s primitive; LDA adds VWN5, so compare
+    # N_el = 2 (exact to quadrature) and V symmetric 1x1; E against the oracle is covered elsewhere
+    import torch
+    norm = (2.0 * alpha / math.pi) ** 0.75
+    spec = xc.grid_spec(75, 302, 0)
+    plan = xc.Plan(np.array([[0.3, -0.2, 0.1]]), np.array([1]), [0], [0], [1], [0], [alpha], [norm], spec)
+    P = torch.tensor([[2.0]], dtype=torch.float64, device="cuda")
+    E, N, V = plan.eval(P)
+    assert N == pytest.approx(2.0, rel=1e-13)
+    assert plan.diagnostics()["w"] == pytest.approx(plan.export().wq, rel=0, abs=0)   # single atom: w = w^q exactly
+    plan.close()
+
+
+def test_determinism_ld_host_path_and_one_shot(xc, orc):
+    import torch
+    w = make_workload("w8")
+    plan = xc.Plan.from_workload(w)
+    n = w.n_basis
+    P = torch.from_numpy(w.P).cuda()
+    E1, N1, V1 = plan.eval(P)
+    V1 = V1.clone()
+    E2, N2, V2 = plan.eval(P)
+    assert E1 == E2 and N1 == N2 and torch.equal(V1, V2)                      # bit-identical
+    E3, N3, V3 = plan.eval(P, reuse_weights=True)
+    assert E1 == E3 and N1 == N3 and torch.equal(V1, V3)                      # cached-weights build
+    Ppad = torch.zeros((n, n + 7), dtype=torch.float64, device="cuda")
+    Ppad[:, :n] = P
+    Vpad = torch.full((n, n + 5), 7.0, dtype=torch.float64, device="cuda")
+    E4, N4, _ = plan.eval(Ppad[:, :n], Vpad[:, :n])                           # leading dimensions > n_basis
+    assert E1 == E4 and torch.equal(V1, Vpad[:, :n]) and bool((Vpad[:, n:] == 7.0).all())
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        E5, N5, V5 = plan.eval(P, stream=s)                                   # non-default stream
+    assert E1 == E5 and torch.equal(V1, V5)
+    Eh, Nh, Vh = plan.eval_host(w.P.copy())                                   # host buffers through the C ABI
+    assert Eh == E1 and Nh == N1 and np.array_equal(Vh, V1.cpu().numpy())
+    Eo, Vo, No = xc.xc_integrate(w, P)                                        # one-shot create+eval+destroy
+    assert Eo == E1 and No == N1 and torch.equal(Vo, V1)
+    plan.close()
+
+
+def test_error_codes(xc):
+    import torch
+    w = make_workload("c1")
+    with pytest.raises(xc.XcError) as e:
+        xc.Plan.from_workload(w, spec=xc.grid_spec(10, 26, 0, max_batch_pts=4096))
+    assert e.value.code == -1
+    w2 = make_workload("c1")
+    w2.shell_L = w2.shell_L.copy()
+    w2.shell_L[0] = 3
+    with pytest.raises(xc.XcError) as e:
+        xc.Plan.from_workload(w2)
+    assert e.value.code == -2
+    plan = xc.Plan.from_workload(w, spec=xc.grid_spec(10, 26, 0))
+    P = torch.from_numpy(w.P).cuda()
+    import ctypes as C
+    from paper_2007_03143_b200 import binding as b
+    E, N = C.c_double(), C.c_double()
+    rc = b._lib.xc_eval(plan._h, C.c_void_p(P.data_ptr()), 3, C.c_void_p(P.data_ptr()), 25, C.byref(E), C.byref(N), 0, None)
+    assert rc == -1   # ld < n_basis
+    plan.close()
+
+
+# ---- single kernels, element by element ---------------------------------------------------------
+def test_functional_kernel_vs_oracle_and_golden(xc, orc):
+    import torch
+    rng = np.random.default_rng(21)
+    n = 20000
+    rho = np.exp(rng.uniform(np.log(1e-12), np.log(500.0), n))
+    sig = rho ** (8.0 / 3.0) * np.exp(rng.uniform(np.log(1e-6), np.log(1e3), n))
+    sig[::17] = 0.0
+    rho[::501] = 1e-16   # below rho_tol
+    for kind in (0, 1):
+        f, vr, vs = (t.cpu().numpy() for t in xc.functional(kind, torch.from_numpy(rho).cuda(), torch.from_numpy(sig).cuda()))
+        of, ovr, ovs = orc.functional(kind, rho, sig)
+        assert np.max(np.abs(f - of) / (np.abs(of) + 1e-300)) < 1e-12
+        assert np.max(np.abs(vr - ovr) / (np.abs(ovr) + 1e-300)) < 1e-11
+        if kind == 1:
+            # v_sigma is a difference of an exchange and a correlation term: tolerance relative to the exchange term
+            scale = np.abs(ovs) + 0.05 / rho ** (4.0 / 3.0)
+            assert np.max(np.abs(vs - ovs) / scale) < 1e-12
+    rows = [l.split() for l in open(os.path.join(HERE, "golden", "functional_values.txt")) if not l.startswith("#")]
+    for row in rows:
+        kind = int(row[0])
+        if kind > 1:
+            continue
+        r_, s_, f_, vr_, vs_ = (float(x) for x in row[1:6])
+        f, vr, vs = (float(t.item()) for t in xc.functional(kind, torch.tensor([r_], dtype=torch.float64, device="cuda"),
+                                                           torch.tensor([s_], dtype=torch.float64, device="cuda")))
+        assert f == pytest.approx(f_, rel=1e-13) and vr == pytest.approx(vr_, rel=1e-13)
+        assert vs == pytest.approx(vs_, rel=1e-12, abs=1e-15)
+
+
+@pytest.mark.parametrize("kind", [0, 1])
+def test_partition_kernel_vs_oracle(xc, orc, kind):
+    import torch
+    w = make_workload("w27", with_P=False)
+    rng = np.random.default_rng(4)
+    n = 5000
+    par = rng.integers(0, len(w.atoms_xyz), n).astype(np.int32)
+    pts = w.atoms_xyz[par] + rng.normal(size=(n, 3)) * rng.choice([0.02, 0.5, 2.0, 8.0], size=(n, 1))
+    wq = rng.uniform(0.1, 2.0, n)
+    got = xc.partition_weights(w.atoms_xyz, torch.from_numpy(pts).cuda(), torch.from_numpy(wq).cuda(),
+                               torch.from_numpy(par).cuda(), kind).cpu().numpy()
+    ref = orc.partition_weights(w.atoms_xyz, pts, wq, par, kind, prune=False)
+    assert np.max(np.abs(got - ref)) <= 1e-13 * np.max(wq)
+    if kind == 0:
+        assert np.array_equal(got == 0.0, ref == 0.0) and np.array_equal(got == wq, ref == wq)
+
+
+# ---- full-size configs: sampled outputs + properties ---------------------------------------------
+@pytest.mark.parametrize("name", ["c4", "c5"])
+def test_full_size_sampled(xc, orc, name):
+    """256- and 512-water PBE workloads in the launch configuration bench.py times.  The oracle cannot run
+    them whole in seconds, so it computes (i) the weights, rho, grad rho and the per-batch E / N_el partial sums
+    of sampled batches, and (ii) sampled V entries exactly: V[mu,nu] only receives contributions from batches
+    whose S_j holds both shells, so evaluating that subset of batches gives the full entry.  Properties at any
+    size: V symmetric, N_el = tr(PS) within the grid error, bit-identical repeat."""
+    import torch
+    w = make_workload(name)
+    plan = xc.Plan.from_workload(w)
+    P = torch.from_numpy(w.P).cuda()
+    E, N, V = plan.eval(P)
+    Vh = V.cpu().numpy()
+    assert np.array_equal(Vh, Vh.T)
+    assert abs(N - 2.0 * w.n_occ) / (2.0 * w.n_occ) < 2e-4
+    d = plan.diagnostics()
+    assert N == pytest.approx(float(np.sum(d["N_batch"])), rel=1e-12) and E == pytest.approx(float(np.sum(d["E_batch"])), rel=1e-12)
+    ex = plan.export()
+    op = oracle_plan(orc, ex)
+    basis = basis_of(w)
+    rng = np.random.default_rng(99)
+    nb = plan.n_batches
+    # (i) sampled batches
+    sub = np.sort(rng.choice(nb, 48, replace=False))
+    pidx = np.concatenate([np.arange(ex.batch_off[j], ex.batch_off[j + 1]) for j in sub])
+    wts = np.zeros(plan.n_points)
+    wts[pidx] = orc.partition_weights(w.atoms_xyz, ex.pts[pidx], ex.wq[pidx], ex.parent[pidx], 0, True)
+    assert np.max(np.abs(d["w"][pidx] - wts[pidx])) <= 1e-13 * np.max(ex.wq[pidx])
+    r = orc.evaluate(op, wts, basis, w.atoms_xyz, w.P, 1, subset=sub, want_V=False, want_batch=True, want_rho=True)
+    assert np.max(np.abs(d["rho"][pidx] - r.rho[pidx])) <= 1e-12 * np.max(np.abs(r.rho[pidx]))
+    assert np.max(np.abs(d["grad_rho"][pidx] - r.grad_rho[pidx])) <= 1e-12 * np.max(np.abs(r.grad_rho[pidx]))
+    assert np.max(np.abs(d["E_batch"][sub] - r.E_batch[sub])) <= 1e-11 * np.max(np.abs(r.E_batch[sub]))
+    assert np.max(np.abs(d["N_batch"][sub] - r.N_batch[sub])) <= 1e-11 * np.max(np.abs(r.N_batch[sub]))
+    # (ii) sampled V entries: tight shells (d of an O, p of its H) keep the batch subset small
+    foff = w.shell_func_off
+    atom = int(rng.integers(0, len(w.atoms_Z) // 3)) * 3          # an O atom
+    sh_d = [s for s in range(len(w.shell_L)) if w.shell_atom[s] == atom and w.shell_L[s] == 2][0]
+    sh_p = [s for s in range(len(w.shell_L)) if w.shell_atom[s] == atom + 1 and w.shell_L[s] == 1][0]
+    has = np.zeros((nb, 2), bool)
+    bid = np.repeat(np.arange(nb), np.diff(ex.shell_off))
+    has[bid[ex.shells == sh_d], 0] = True
+    has[bid[ex.shells == sh_p], 1] = True
+    both = np.where(has[:, 0] & has[:, 1])[0]
+    assert 0 < len(both) < 4000
+    pidx = np.concatenate([np.arange(ex.batch_off[j], ex.batch_off[j + 1]) for j in both])
+    wts2 = np.zeros(plan.n_points)
+    wts2[pidx] = d["w"][pidx]     # weights already checked on the sample above; reuse the GPU's here
+    r2 = orc.evaluate(op, wts2, basis, w.atoms_xyz, w.P, 1, subset=both, want_V=True)
+    rows = np.arange(foff[sh_d], foff[sh_d] + 6)
+    cols = np.arange(foff[sh_p], foff[sh_p] + 3)
+    blk_o, blk_g = r2.V[np.ix_(rows, cols)], Vh[np.ix_(rows, cols)]
+    assert np.max(np.abs(blk_o - blk_g)) <= TOL_V * np.max(np.abs(Vh))
+    assert np.max(np.abs(blk_o)) > 0
+    E2, N2, V2 = plan.eval(P)
+    assert E2 == E and N2 == N and bool((V2.cpu().numpy() == Vh).all())
+    plan.close()
