@@ -49,6 +49,8 @@ struct xc_plan {
   double *d_exps = nullptr, *d_coefs = nullptr;
   BatchRec* d_batches = nullptr;
   int32_t *d_bshells = nullptr, *d_bsfoff = nullptr, *d_bfidx = nullptr, *d_bfinfo = nullptr;
+  double *d_nbr = nullptr, *d_wbox = nullptr;
+  int32_t *d_watoms = nullptr, *d_wsmall = nullptr, *d_wlarge = nullptr;
   DensityItem *d_items64 = nullptr, *d_items32 = nullptr;
   PotItem* d_pot = nullptr;
   double *d_phi = nullptr, *d_z = nullptr;
@@ -70,7 +72,7 @@ static void free_plan(xc_plan* p) {
   void* ptrs[] = {p->d_px, p->d_py, p->d_pz, p->d_wq, p->d_w, p->d_parent, p->d_atoms, p->d_invR, p->d_rnn, p->d_shells,
                   p->d_exps, p->d_coefs, p->d_batches, p->d_bshells, p->d_bsfoff, p->d_bfidx, p->d_bfinfo, p->d_items64,
                   p->d_items32, p->d_pot, p->d_phi, p->d_z, p->d_vhi, p->d_vlo, p->d_Epart, p->d_Npart, p->d_result,
-                  p->d_rho, p->d_grho, p->d_Ptmp, p->d_Vtmp};
+                  p->d_rho, p->d_grho, p->d_Ptmp, p->d_Vtmp, p->d_watoms, p->d_wsmall, p->d_wlarge, p->d_nbr, p->d_wbox};
   for (void* q : ptrs) if (q) cudaFree(q);
   if (p->h_result) cudaFreeHost(p->h_result);
   for (cudaEvent_t e : p->ev) cudaEventDestroy(e);
@@ -136,6 +138,8 @@ int xc_plan_create(const xc_atom* atoms, int32_t natoms, const xc_shell* shells,
   UP(d_atoms, hp.atoms); UP(d_invR, invR); UP(d_rnn, rnn);
   UP(d_shells, hp.shells); UP(d_exps, hp.exps); UP(d_coefs, hp.coefs);
   UP(d_batches, hp.batches); UP(d_bshells, hp.bshells); UP(d_bsfoff, hp.bsfoff); UP(d_bfidx, hp.bfidx); UP(d_bfinfo, hp.bfinfo);
+  UP(d_wbox, hp.wbox);
+  UP(d_watoms, hp.watoms); UP(d_wsmall, hp.wbatch_small); UP(d_wlarge, hp.wbatch_large);
   UP(d_items64, hp.items64); UP(d_items32, hp.items32); UP(d_pot, hp.pot_items);
 #undef UP
   size_t nitems = hp.items64.size() + hp.items32.size();
@@ -200,9 +204,17 @@ int xc_eval(xc_plan* p, const double* dP, int64_t ldp, double* dV, int64_t ldv, 
   size_t ie = 0;
   CU(cudaEventRecord(p->ev[ie++], st));
   if (!(flags & 1) || !p->weights_valid) {
-    CU(launch_weights(hp.spec.partition, hp.natoms, p->d_atoms, p->d_invR, p->d_rnn, hp.npts, p->d_px, p->d_py, p->d_pz,
-                      p->d_wq, p->d_parent, p->d_w, st));
-    ++launches;
+    WeightArgs wa;
+    wa.batches = p->d_batches; wa.watoms = p->d_watoms; wa.atoms = p->d_atoms; wa.invR = p->d_invR; wa.rnn = p->d_rnn;
+    wa.nbr = nullptr; wa.wbox = p->d_wbox; wa.natoms = hp.natoms; wa.px = p->d_px; wa.py = p->d_py; wa.pz = p->d_pz; wa.wq = p->d_wq; wa.parent = p->d_parent; wa.w = p->d_w;
+    if (!hp.wbatch_large.empty()) {   // long lists first: they are the long pole
+      CU(launch_weights_batched(hp.spec.partition, wa, p->d_wlarge, (int)hp.wbatch_large.size(), hp.w_warps_large, hp.w_max_large, st));
+      ++launches;
+    }
+    if (!hp.wbatch_small.empty()) {
+      CU(launch_weights_batched(hp.spec.partition, wa, p->d_wsmall, (int)hp.wbatch_small.size(), 8, hp.w_max_small, st));
+      ++launches;
+    }
     p->weights_valid = true;
   }
   CU(cudaEventRecord(p->ev[ie++], st));

@@ -17,6 +17,8 @@ constexpr int kDensityThreads = 512;
 constexpr int kPotThreads = 256;
 constexpr int kPotKPart = 128;  // points per work item of the potential kernel
 constexpr size_t kSmemLimit = 227 * 1024;
+constexpr int kWeightSmallList = 192; // atom-list length that separates the two launches of the weights kernel
+constexpr int kWeightThreads = 256;
 
 struct ShellRec {      // 48 bytes
   double x, y, z;      // centre
@@ -31,6 +33,8 @@ struct BatchRec {      // one quadrature batch B_j with its shell list S_j (PAPE
   int32_t f_off, nb;           // offset into batch function-index list, N_b^j
   int32_t nb_pad8;             // N_b^j rounded up to 8
   int64_t scr_off;             // offset (doubles) of this batch's Phi / Z workspace
+  int64_t wa_off;              // offset into the weight-kernel atom lists
+  int32_t wa_nB, wa_nC;        // atoms that can own weight here / atoms that can appear in a cell product
 };
 
 struct DensityItem { int32_t batch, tile_start; };            // one CTA of the density kernel
@@ -41,6 +45,7 @@ inline int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
 
 // shared-memory footprint of the density kernel for a batch (bytes); T = points per tile
 size_t density_smem_bytes(int T, bool gga, int nb, int ns);
+size_t weights_smem_bytes(int nC, int warps);
 
 struct HostPlan {
   int natoms = 0, nshells = 0, nbasis = 0, nprim = 0;
@@ -57,6 +62,10 @@ struct HostPlan {
   std::vector<int32_t> bsfoff;         // per entry of bshells: first LOCAL function index of that shell in its batch
   std::vector<int32_t> bfidx;          // concatenated global function indices of S_j
   std::vector<int32_t> bfinfo;         // per local function: (local shell slot << 8) | (l<<4 | m<<2 | n)
+  std::vector<int32_t> watoms;         // concatenated per-batch atom lists of the weights kernel (sorted by distance to the batch box)
+  std::vector<double> wbox;            // [nbatch][6] tight bounding boxes
+  std::vector<int32_t> wbatch_small, wbatch_large;  // batch ids by list length (two launches)
+  int w_max_small = 0, w_max_large = 0, w_warps_large = 8;
   std::vector<DensityItem> items64, items32;  // density-kernel work lists (tile of 64 / 32 points)
   std::vector<PotItem> pot_items;
   struct Chunk { int64_t b0, b1, i64_0, i64_1, i32_0, i32_1, p0, p1; int64_t scr; };

@@ -11,6 +11,7 @@
 // and epilogue arithmetic; tcgen05 has no f64 kind.  (Product code; shares nothing with oracle/.)
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cstdint>
 
 #include "xc_internal.h"
@@ -231,6 +232,269 @@ __global__ void __launch_bounds__(128) k_weights(int natoms, const double* __res
   }
   if (!done) result = base * PA / sum;
   if (act) w[i] = result;
+}
+
+// ------------------------------------------------------------------------------------------------
+// step (a), hot path: one CTA per batch, one WARP per point.  The batch's atom list (planner: exact SSF support,
+// sorted by distance to the batch box; owners = the first nB, partners = all nC) sits in shared memory; the
+// lanes of a warp split the partners, so there is no divergence between points, and the products are
+// combined with an xor butterfly (same value in every lane, fixed order => deterministic).
+// ------------------------------------------------------------------------------------------------
+template <int PART>
+__global__ void __launch_bounds__(kWeightThreads) k_weights_batched(WeightArgs a, const int32_t* __restrict__ batch_ids, int nwarps) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const unsigned FULL = 0xffffffffu;
+  const BatchRec b = a.batches[batch_ids[blockIdx.x]];
+  const int nC = b.wa_nC, nB = PART == 0 ? b.wa_nB : b.wa_nC;
+  double* sXYZ = (double*)smem_raw;                 // [nC][3]
+  double* sDall = sXYZ + (size_t)3 * nC;            // [nwarps][nC]
+  int* sAt = (int*)(sDall + (size_t)nwarps * nC);   // [nC]
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (warp >= nwarps) return;
+  for (int c = threadIdx.x; c < nC; c += nwarps * 32) {
+    int at = a.watoms[b.wa_off + c];
+    sAt[c] = at;
+    sXYZ[3 * c] = a.atoms[3 * at]; sXYZ[3 * c + 1] = a.atoms[3 * at + 1]; sXYZ[3 * c + 2] = a.atoms[3 * at + 2];
+  }
+  // nwarps*32 threads take part (the others returned): named barrier over the active threads
+  asm volatile("bar.sync 1, %0;" ::"r"(nwarps * 32));
+  double* sD = sDall + (size_t)warp * nC;
+  const double kappa = (1.0 + 0.64) / (1.0 - 0.64);
+  for (int p = warp; p < b.nq; p += nwarps) {
+    const int64_t gi = (int64_t)b.pt_off + p;
+    const double x = a.px[gi], y = a.py[gi], z = a.pz[gi], base = a.wq[gi];
+    const int A = a.parent[gi];
+    double result = base;
+    bool trivial = a.natoms == 1;
+    if (PART == 0 && !trivial) {
+      double dx = x - a.atoms[3 * A], dy = y - a.atoms[3 * A + 1], dz = z - a.atoms[3 * A + 2];
+      trivial = sqrt(dx * dx + dy * dy + dz * dz) < 0.5 * (1.0 - 0.64) * a.rnn[A];
+    }
+    if (!trivial) {
+      double dmin = 1e300;
+      int imin = 0x7fffffff;
+      for (int c = lane; c < nC; c += 32) {
+        double dx = x - sXYZ[3 * c], dy = y - sXYZ[3 * c + 1], dz = z - sXYZ[3 * c + 2];
+        double d = sqrt(dx * dx + dy * dy + dz * dz);
+        sD[c] = d;
+        if (d < dmin) { dmin = d; imin = c; }
+      }
+#pragma unroll
+      for (int o = 16; o >= 1; o >>= 1) {
+        double od = __shfl_xor_sync(FULL, dmin, o);
+        int oi = __shfl_xor_sync(FULL, imin, o);
+        if (od < dmin || (od == dmin && oi < imin)) { dmin = od; imin = oi; }
+      }
+      __syncwarp();
+      double sum = 0.0, PA = 0.0;
+      const int nsteps = (nC + 31) >> 5;
+      for (int bb = 0; bb < nB; ++bb) {
+        const double rB = sD[bb];
+        if (PART == 0 && rB >= kappa * dmin && rB > dmin) continue;           // P_B = 0 exactly
+        const int Bid = sAt[bb];
+        const double* iR = a.invR + (size_t)Bid * a.natoms;
+        double PB = 1.0;
+        if (PART == 0 && bb != imin) {
+          PB = s_ssf((rB - dmin) * __ldg(iR + sAt[imin]));                     // nearest atom first
+          if (PB == 0.0) continue;
+        }
+        double part = 1.0;
+        for (int k = 0; k < nsteps; ++k) {
+          const int c = (k << 5) + lane;
+          if (c < nC && c != bb && (PART == 1 || c != imin)) {
+            const double rC = sD[c];
+            if (PART == 1) part *= s_becke((rB - rC) * __ldg(iR + sAt[c]));
+            else if (rC < kappa * rB) part *= s_ssf((rB - rC) * __ldg(iR + sAt[c]));  // else the factor is exactly 1
+          }
+          if (PART == 0 && (k & 3) == 3 && !__any_sync(FULL, part != 0.0)) break;
+        }
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) part *= __shfl_xor_sync(FULL, part, o);
+        PB *= part;
+        sum += PB;
+        if (Bid == A) PA = PB;
+      }
+      result = base * PA / sum;
+      __syncwarp();
+    }
+    if (lane == 0) a.w[gi] = result;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// step (a), hot path for SSF: one CTA per batch, one WARP per point, partner-outer loops.
+// Exact pruning only; the batch's atom list (planner) is sorted by
+// dmin(atom, batch box) <= r_atom, so every scan stops as soon as dmin reaches its bound:
+//   1. nearest atom m and r_min                        (scan while dmin < r_min)
+//   2. owner candidates B: r_B < kappa r_min, not killed by m or by the 8 box-nearest atoms (mu_BC >= a => P_B = 0);
+//      the parent is evaluated first: P_A = 0 => w = 0 and the point is done
+//   3. for chunks of <= 8 owners: ONE pass over the partners C (scan while dmin < kappa max r_B), the lanes
+//      splitting the C's: r_C costs one sqrt per C for all owners, R_BC = rsqrt from shared-memory coordinates,
+//      s(mu_BC) = 1 exactly when r_C >= kappa r_B.  Lane products are combined by an xor butterfly
+//      (same value in every lane, fixed order => deterministic).
+// ------------------------------------------------------------------------------------------------
+constexpr int kOwnChunk = 8;
+constexpr int kOwnMax = 64;
+
+__global__ void __launch_bounds__(kWeightThreads) k_weights_ssf(WeightArgs a, const int32_t* __restrict__ batch_ids) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const unsigned FULL = 0xffffffffu;
+  const int bid = batch_ids[blockIdx.x];
+  const BatchRec b = a.batches[bid];
+  const int nC = b.wa_nC, nB = b.wa_nB;
+  double* sX = (double*)smem_raw;
+  double* sY = sX + nC;
+  double* sZ = sY + nC;
+  double* sDm = sZ + nC;
+  double* sOwnR = sDm + nC;                              // [8 warps][kOwnMax]
+  int* sId = (int*)(sOwnR + (kWeightThreads / 32) * kOwnMax);
+  int* sOwn = sId + nC;                                  // [8 warps][kOwnMax]
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  {
+    const double* box = a.wbox + (size_t)6 * bid;
+    for (int c = threadIdx.x; c < nC; c += kWeightThreads) {
+      int at = a.watoms[b.wa_off + c];
+      double cx = a.atoms[3 * at], cy = a.atoms[3 * at + 1], cz = a.atoms[3 * at + 2];
+      sId[c] = at; sX[c] = cx; sY[c] = cy; sZ[c] = cz;
+      double tx = cx < box[0] ? box[0] - cx : (cx > box[3] ? cx - box[3] : 0.0);
+      double ty = cy < box[1] ? box[1] - cy : (cy > box[4] ? cy - box[4] : 0.0);
+      double tz = cz < box[2] ? box[2] - cz : (cz > box[5] ? cz - box[5] : 0.0);
+      // a hair below the true distance: the early exits must never cut an atom that matters
+      sDm[c] = sqrt(tx * tx + ty * ty + tz * tz) * (1.0 - 1e-12) - 1e-12;
+    }
+  }
+  __syncthreads();
+  const double aa = 0.64, kappa = (1.0 + aa) / (1.0 - aa);
+  double* myOwnR = sOwnR + warp * kOwnMax;
+  int* myOwn = sOwn + warp * kOwnMax;
+  for (int p = warp; p < b.nq; p += kWeightThreads / 32) {
+    const int64_t gi = (int64_t)b.pt_off + p;
+    const double x = a.px[gi], y = a.py[gi], z = a.pz[gi], base = a.wq[gi];
+    const int A = a.parent[gi];
+    double result = base;
+    bool trivial = a.natoms == 1;
+    double rA = 0.0;
+    if (!trivial) {
+      double dx = x - a.atoms[3 * A], dy = y - a.atoms[3 * A + 1], dz = z - a.atoms[3 * A + 2];
+      rA = sqrt(dx * dx + dy * dy + dz * dz);
+      trivial = rA < 0.5 * (1.0 - aa) * a.rnn[A];
+    }
+    if (!trivial) {
+      // 1. nearest atom
+      double rmin = 1e300;
+      int im = 0x7fffffff;
+      for (int c0 = 0; c0 < nC; c0 += 32) {
+        if (sDm[c0] >= rmin) break;
+        const int c = c0 + lane;
+        double d = 1e300;
+        if (c < nC) { double dx = x - sX[c], dy = y - sY[c], dz = z - sZ[c]; d = sqrt(dx * dx + dy * dy + dz * dz); }
+        int ci = c;
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) {
+          double od = __shfl_xor_sync(FULL, d, o);
+          int oi = __shfl_xor_sync(FULL, ci, o);
+          if (od < d || (od == d && oi < ci)) { d = od; ci = oi; }
+        }
+        if (d < rmin) { rmin = d; im = ci; }
+      }
+      if (rA >= kappa * rmin && rA > rmin) {
+        result = 0.0;                                     // P_A = 0 exactly
+      } else {
+        // distances to the 8 box-nearest atoms (extra exact kill tests)
+        const int nk = min(8, nC);
+        double rk = 1e300;
+        if (lane < nk) { double dx = x - sX[lane], dy = y - sY[lane], dz = z - sZ[lane]; rk = sqrt(dx * dx + dy * dy + dz * dz); }
+        // 2. owner candidates, parent first
+        int nown = 0;
+        const double own_lim = kappa * rmin;
+        bool parent_alive = false;
+        for (int b0 = 0; b0 < nB; b0 += 32) {
+          if (sDm[b0] >= own_lim) break;
+          const int bb = b0 + lane;
+          bool cand = false;
+          double rB = 0.0;
+          if (bb < nB) {
+            const double bx = sX[bb], by = sY[bb], bz = sZ[bb];
+            double dx = x - bx, dy = y - by, dz = z - bz;
+            rB = sqrt(dx * dx + dy * dy + dz * dz);
+            cand = bb == im || rB < own_lim;
+            if (cand && bb != im) {
+              double ex = bx - sX[im], ey = by - sY[im], ez = bz - sZ[im];
+              cand = (rB - rmin) * rsqrt(ex * ex + ey * ey + ez * ez) < aa;
+            }
+          }
+          // kill tests against the 8 box-nearest atoms (shuffles outside the divergent region)
+#pragma unroll
+          for (int c = 0; c < 8; ++c) {
+            const double rc = __shfl_sync(FULL, rk, c);
+            if (cand && c < nk && c != bb) {
+              double ex = sX[bb] - sX[c], ey = sY[bb] - sY[c], ez = sZ[bb] - sZ[c];
+              cand = (rB - rc) * rsqrt(ex * ex + ey * ey + ez * ez) < aa;
+            }
+          }
+          const bool isA = cand && sId[bb] == A;
+          if (__any_sync(FULL, isA)) parent_alive = true;
+          unsigned mask = __ballot_sync(FULL, cand && !isA);
+          // parent goes to slot 0; the others are appended in list order
+          int pos = nown + __popc(mask & ((1u << lane) - 1u)) + 1;   // slot 0 reserved for the parent
+          if (cand && !isA && pos < kOwnMax) { myOwn[pos] = bb; myOwnR[pos] = rB; }
+          if (isA) { myOwn[0] = bb; myOwnR[0] = rB; }
+          nown += __popc(mask);
+        }
+        __syncwarp();
+        if (!parent_alive) {
+          result = 0.0;                                   // the parent was killed: P_A = 0 exactly
+        } else {
+          nown = min(nown + 1, kOwnMax);                  // + parent in slot 0
+          double sum = 0.0, PA = 0.0;
+          for (int o0 = 0; o0 < nown; o0 += kOwnChunk) {
+            const int K = min(kOwnChunk, nown - o0);
+            double part[kOwnChunk], rBk[kOwnChunk];
+            int ok[kOwnChunk];
+            double rBmax = 0.0;
+#pragma unroll
+            for (int k = 0; k < kOwnChunk; ++k) {
+              part[k] = 1.0;
+              ok[k] = k < K ? myOwn[o0 + k] : -1;
+              rBk[k] = k < K ? myOwnR[o0 + k] : 0.0;
+              rBmax = fmax(rBmax, rBk[k]);
+            }
+            const double clim = kappa * rBmax;
+            for (int c0 = 0; c0 < nC; c0 += 32) {
+              if (sDm[c0] >= clim) break;
+              const int c = c0 + lane;
+              if (c < nC) {
+                const double cx = sX[c], cy = sY[c], cz = sZ[c];
+                double dx = x - cx, dy = y - cy, dz = z - cz;
+                const double rC = sqrt(dx * dx + dy * dy + dz * dz);
+#pragma unroll
+                for (int k = 0; k < kOwnChunk; ++k) {
+                  if (k < K && c != ok[k] && rC < kappa * rBk[k]) {   // else: not an owner slot / B itself / factor exactly 1
+                    double ex = cx - sX[ok[k]], ey = cy - sY[ok[k]], ez = cz - sZ[ok[k]];
+                    part[k] *= s_ssf((rBk[k] - rC) * rsqrt(ex * ex + ey * ey + ez * ez));
+                  }
+                }
+              }
+            }
+#pragma unroll
+            for (int k = 0; k < kOwnChunk; ++k) {
+              double v = part[k];
+#pragma unroll
+              for (int o = 16; o >= 1; o >>= 1) v *= __shfl_xor_sync(FULL, v, o);
+              if (k < K) {
+                sum += v;
+                if (o0 == 0 && k == 0) PA = v;
+              }
+            }
+            if (o0 == 0 && PA == 0.0) break;              // P_A = 0 => w = 0, whatever the others are
+          }
+          result = PA == 0.0 ? 0.0 : base * PA / sum;
+        }
+        __syncwarp();
+      }
+    }
+    if (lane == 0) a.w[gi] = result;
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -659,6 +923,24 @@ cudaError_t launch_weights(int partition, int natoms, const double* atoms, const
   unsigned grid = (unsigned)((npts + 127) / 128);
   if (partition == 0) k_weights<0><<<grid, 128, 0, st>>>(natoms, atoms, invR, rnn, npts, px, py, pz, wq, parent, w);
   else k_weights<1><<<grid, 128, 0, st>>>(natoms, atoms, invR, rnn, npts, px, py, pz, wq, parent, w);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_weights_batched(int partition, const WeightArgs& a, const int32_t* batch_ids, int nbatches, int nwarps,
+                                   int max_list, cudaStream_t st) {
+  if (nbatches <= 0) return cudaSuccess;
+  size_t smem = weights_smem_bytes(max_list, nwarps);
+  cudaError_t e;
+  if (partition == 0) {
+    smem = (size_t)max_list * 36 + (size_t)(kWeightThreads / 32) * kOwnMax * 12 + 64;   // list: x,y,z,dmin,id; per-warp owner slots
+    e = cudaFuncSetAttribute(k_weights_ssf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(smem, 1024));
+    if (e != cudaSuccess) return e;
+    k_weights_ssf<<<nbatches, kWeightThreads, smem, st>>>(a, batch_ids);
+  } else {
+    e = cudaFuncSetAttribute(k_weights_batched<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(smem, 1024));
+    if (e != cudaSuccess) return e;
+    k_weights_batched<1><<<nbatches, kWeightThreads, smem, st>>>(a, batch_ids, nwarps);
+  }
   return cudaGetLastError();
 }
 

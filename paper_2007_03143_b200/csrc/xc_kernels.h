@@ -23,6 +23,17 @@ struct DensityArgs {
   double rho_tol;
 };
 
+struct WeightArgs {
+  const BatchRec* batches;
+  const int32_t* watoms;
+  const double* atoms; const double* invR; const double* rnn;
+  const double* nbr;    // [natoms][natoms-1][5]: x,y,z of the k-th nearest neighbour atom, a*R, 1/(a*R)
+  const double* wbox;   // [nbatch][6] tight bounding boxes (lo xyz, hi xyz)
+  int natoms;
+  const double* px; const double* py; const double* pz; const double* wq; const int32_t* parent;
+  double* w;
+};
+
 struct PotArgs {
   const PotItem* items; int64_t nitems;
   const BatchRec* batches;
@@ -35,6 +46,8 @@ struct PotArgs {
 cudaError_t launch_weights(int partition, int natoms, const double* atoms, const double* invR, const double* rnn,
                            int64_t npts, const double* px, const double* py, const double* pz, const double* wq,
                            const int32_t* parent, double* w, cudaStream_t st);
+cudaError_t launch_weights_batched(int partition, const WeightArgs& a, const int32_t* batch_ids, int nbatches, int nwarps,
+                                   int max_list, cudaStream_t st);
 cudaError_t launch_functional(int kind, int64_t n, const double* rho, const double* sigma, double rho_tol, double* f,
                               double* vr, double* vs, cudaStream_t st);
 cudaError_t launch_density(int T, bool gga, const DensityArgs& a, const DensityItem* items, int nitems, int item0,

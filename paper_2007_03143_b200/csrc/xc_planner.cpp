@@ -110,6 +110,8 @@ size_t density_smem_bytes(int T, bool gga, int nb, int ns) {
   return b + 64;
 }
 
+size_t weights_smem_bytes(int nC, int warps) { return (size_t)nC * (24 + 4) + (size_t)warps * nC * 8 + 64; }
+
 int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, int nshells, const double* exps,
                     const double* coefs, int nprim_total, const xc_grid_spec* spec, HostPlan& hp, std::string& err) {
   if (!atoms || !shells || !exps || !coefs || !spec) { err = "null argument"; return XC_EINVAL; }
@@ -207,11 +209,12 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     atom_rmax[hp.shells[s].atom] = std::max(atom_rmax[hp.shells[s].atom], hp.rcut[s]);
   }
   const bool gga = spec->functional == 1;
-  auto screen = [&](const Leaf& lf, std::vector<int32_t>& out, int& nb) {
+  auto screen = [&](const Leaf& lf, std::vector<int32_t>& out, int& nb, Box* box_out = nullptr) {
     Box b;
     for (int p = 0; p < 3; ++p) { b.lo[p] = 1e300; b.hi[p] = -1e300; }
     for (int64_t k = lf.begin; k < lf.end; ++k)
       for (int p = 0; p < 3; ++p) { double v = coord[p][idx[k]]; b.lo[p] = std::min(b.lo[p], v); b.hi[p] = std::max(b.hi[p], v); }
+    if (box_out) *box_out = b;
     out.clear(); nb = 0;
     for (int a = 0; a < natoms; ++a) {
       if (!sphere_hits_box(&hp.atoms[3 * a], atom_rmax[a], b)) continue;
@@ -258,6 +261,83 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     }
   }
 
+  // ---- order the points inside each batch along a Morton curve: neighbouring threads of the weights kernel then
+  //      see nearly the same atoms (warp-coherent loop bounds); the batch as a set is unchanged ----
+  {
+    auto spread = [](uint32_t v) { uint64_t x = v & 0x1fffff; x = (x | x << 32) & 0x1f00000000ffffULL; x = (x | x << 16) & 0x1f0000ff0000ffULL;
+                                   x = (x | x << 8) & 0x100f00f00f00f00fULL; x = (x | x << 4) & 0x10c30c30c30c30c3ULL; x = (x | x << 2) & 0x1249249249249249ULL; return x; };
+#pragma omp parallel
+    {
+      std::vector<std::pair<uint64_t, int64_t>> keyed;
+#pragma omp for schedule(dynamic, 64)
+      for (int64_t j = 0; j < (int64_t)leaves.size(); ++j) {
+        double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+        for (int64_t k = leaves[j].begin; k < leaves[j].end; ++k)
+          for (int p = 0; p < 3; ++p) { double v = coord[p][idx[k]]; lo[p] = std::min(lo[p], v); hi[p] = std::max(hi[p], v); }
+        double ext = std::max({hi[0] - lo[0], hi[1] - lo[1], hi[2] - lo[2], 1e-300});
+        keyed.clear();
+        for (int64_t k = leaves[j].begin; k < leaves[j].end; ++k) {
+          uint64_t key = 0;
+          for (int p = 0; p < 3; ++p) {
+            uint32_t q = (uint32_t)std::min(1048575.0, std::floor((coord[p][idx[k]] - lo[p]) / ext * 1048576.0));
+            key |= spread(q) << p;
+          }
+          keyed.push_back({key, idx[k]});
+        }
+        std::sort(keyed.begin(), keyed.end());
+        for (size_t k = 0; k < keyed.size(); ++k) idx[leaves[j].begin + k] = keyed[k].second;
+      }
+    }
+  }
+
+  // ---- atom lists of the weights kernel (step (a)), exact SSF compact support ----
+  // U = min_C dmax(C, box) bounds r_min of every point of the batch from above.  An atom B can own weight at some
+  // point only if r_B < kappa r_min <= kappa U, and a factor s(mu_BC) differs from 1 only if r_C < kappa r_B < kappa^2 U.
+  // With dmin(.,box) <= r_. the lists {dmin < kappa U} (owners) and {dmin < kappa^2 U} (partners) are supersets.
+  hp.wbox.assign(6 * leaves.size(), 0.0);
+  std::vector<std::vector<int32_t>> wlists(leaves.size());
+  std::vector<int> wnB(leaves.size(), 0);
+  {
+    const double a_ssf = 0.64, kappa = (1.0 + a_ssf) / (1.0 - a_ssf);
+    const bool ssf = spec->partition == 0;
+#pragma omp parallel
+    {
+      std::vector<std::pair<double, int32_t>> cand;
+#pragma omp for schedule(dynamic, 64)
+      for (int64_t j = 0; j < (int64_t)leaves.size(); ++j) {
+        if (!ssf) continue;  // Becke-88 has no compact support: one shared list of all atoms (below)
+        Box b;
+        for (int p = 0; p < 3; ++p) { b.lo[p] = 1e300; b.hi[p] = -1e300; }
+        for (int64_t k = leaves[j].begin; k < leaves[j].end; ++k)
+          for (int p = 0; p < 3; ++p) { double v = coord[p][idx[k]]; b.lo[p] = std::min(b.lo[p], v); b.hi[p] = std::max(b.hi[p], v); }
+        double U = 1e300;
+        for (int a = 0; a < natoms; ++a) {
+          double d2 = 0.0;
+          for (int p = 0; p < 3; ++p) { double t = std::max(std::fabs(hp.atoms[3 * a + p] - b.lo[p]), std::fabs(hp.atoms[3 * a + p] - b.hi[p])); d2 += t * t; }
+          U = std::min(U, std::sqrt(d2));
+        }
+        for (int p = 0; p < 3; ++p) { hp.wbox[6 * j + p] = b.lo[p]; hp.wbox[6 * j + 3 + p] = b.hi[p]; }
+        const double rB = kappa * U * (1.0 + 1e-12) + 1e-12, rC = kappa * rB * (1.0 + 1e-12) + 1e-12;
+        cand.clear();
+        for (int a = 0; a < natoms; ++a) {
+          double d2 = 0.0;
+          for (int p = 0; p < 3; ++p) {
+            double c = hp.atoms[3 * a + p];
+            double t = c < b.lo[p] ? b.lo[p] - c : (c > b.hi[p] ? c - b.hi[p] : 0.0);
+            d2 += t * t;
+          }
+          double d = std::sqrt(d2);
+          if (d <= rC) cand.push_back({d, a});
+        }
+        std::sort(cand.begin(), cand.end());
+        wlists[j].resize(cand.size());
+        int nB = 0;
+        for (size_t k = 0; k < cand.size(); ++k) { wlists[j][k] = cand[k].second; if (cand[k].first <= rB) nB = (int)k + 1; }
+        wnB[j] = nB;
+      }
+    }
+  }
+
   // ---- permuted point arrays ----
   hp.px.resize(npts); hp.py.resize(npts); hp.pz.resize(npts); hp.wq.resize(npts); hp.parent.resize(npts); hp.orig.resize(npts);
 #pragma omp parallel for schedule(static)
@@ -278,6 +358,8 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
   int64_t cap = (int64_t)2 << 30;  // 2 Gi doubles = 16 GiB per matrix
   if (const char* e = getenv("XC_B200_WORKSPACE_MB")) cap = std::max<int64_t>(1, atoll(e)) * (1 << 20) / 8;
   hp.chunks.clear();
+  hp.watoms.clear(); hp.wbatch_small.clear(); hp.wbatch_large.clear(); hp.w_max_small = hp.w_max_large = 0;
+  if (spec->partition != 0) { hp.watoms.resize(natoms); std::iota(hp.watoms.begin(), hp.watoms.end(), 0); }
   HostPlan::Chunk ch{0, 0, 0, 0, 0, 0, 0, 0, 0};
   std::vector<int64_t> chunk_of(nbatch);
   for (int64_t j = 0; j < nbatch; ++j) {
@@ -295,6 +377,17 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     }
     chunk_of[j] = (int64_t)hp.chunks.size();
     b.scr_off = scr;
+    if (spec->partition == 0) {
+      b.wa_off = (int64_t)hp.watoms.size(); b.wa_nB = wnB[j]; b.wa_nC = (int32_t)wlists[j].size();
+      hp.watoms.insert(hp.watoms.end(), wlists[j].begin(), wlists[j].end());
+    } else {
+      b.wa_off = 0; b.wa_nB = natoms; b.wa_nC = natoms;
+    }
+    {
+      int len = b.wa_nC;
+      if (len <= kWeightSmallList) { hp.wbatch_small.push_back((int32_t)j); hp.w_max_small = std::max(hp.w_max_small, len); }
+      else { hp.wbatch_large.push_back((int32_t)j); hp.w_max_large = std::max(hp.w_max_large, len); }
+    }
     sh_off += b.ns; f_off += b.nb;
     scr += need; scr_total += need;
     if (sh_off >= ((int64_t)1 << 31) || f_off >= ((int64_t)1 << 31)) { err = "batch lists exceed 2^31 entries"; return XC_EUNSUPPORTED; }
@@ -342,6 +435,15 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
       for (int tm = 0; tm < nt; ++tm)
         for (int tn = 0; tn <= tm; ++tn) hp.pot_items.push_back({(int32_t)j, (int16_t)tm, (int16_t)tn, k0, k1});
     }
+  }
+  // warps per CTA of the large-list weights launch: per-warp distance rows must fit in shared memory
+  hp.w_warps_large = 8;
+  if (spec->partition == 0 && (size_t)hp.w_max_large * 36 + 8 * 64 * 12 + 64 > kSmemLimit) {
+    err = "too many atoms inside the SSF support of one batch for the weights kernel"; return XC_EUNSUPPORTED;
+  }
+  while (spec->partition != 0 && hp.w_warps_large > 1 && weights_smem_bytes(hp.w_max_large, hp.w_warps_large) > kSmemLimit) hp.w_warps_large >>= 1;
+  if (spec->partition != 0 && weights_smem_bytes(hp.w_max_large, hp.w_warps_large) > kSmemLimit) {
+    err = "too many atoms inside the SSF support of one batch for the weights kernel"; return XC_EUNSUPPORTED;
   }
   // work-item ranges per chunk (lists are in batch order)
   {
