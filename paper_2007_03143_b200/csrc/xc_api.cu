@@ -49,7 +49,8 @@ struct xc_plan {
   double *d_exps = nullptr, *d_coefs = nullptr;
   BatchRec* d_batches = nullptr;
   int32_t *d_bshells = nullptr, *d_bsfoff = nullptr, *d_bfidx = nullptr, *d_bfinfo = nullptr;
-  double *d_nbr = nullptr, *d_wbox = nullptr;
+  double *d_wbox = nullptr;
+  double2* d_pairtab = nullptr;
   int32_t *d_watoms = nullptr, *d_wsmall = nullptr, *d_wlarge = nullptr;
   DensityItem *d_items64 = nullptr, *d_items32 = nullptr;
   PotItem* d_pot = nullptr;
@@ -72,7 +73,7 @@ static void free_plan(xc_plan* p) {
   void* ptrs[] = {p->d_px, p->d_py, p->d_pz, p->d_wq, p->d_w, p->d_parent, p->d_atoms, p->d_invR, p->d_rnn, p->d_shells,
                   p->d_exps, p->d_coefs, p->d_batches, p->d_bshells, p->d_bsfoff, p->d_bfidx, p->d_bfinfo, p->d_items64,
                   p->d_items32, p->d_pot, p->d_phi, p->d_z, p->d_vhi, p->d_vlo, p->d_Epart, p->d_Npart, p->d_result,
-                  p->d_rho, p->d_grho, p->d_Ptmp, p->d_Vtmp, p->d_watoms, p->d_wsmall, p->d_wlarge, p->d_nbr, p->d_wbox};
+                  p->d_rho, p->d_grho, p->d_Ptmp, p->d_Vtmp, p->d_watoms, p->d_wsmall, p->d_wlarge, p->d_pairtab, p->d_wbox};
   for (void* q : ptrs) if (q) cudaFree(q);
   if (p->h_result) cudaFreeHost(p->h_result);
   for (cudaEvent_t e : p->ev) cudaEventDestroy(e);
@@ -136,6 +137,11 @@ int xc_plan_create(const xc_atom* atoms, int32_t natoms, const xc_shell* shells,
 #define UP(d, h) do { int _r = upload(&p->d, h); if (_r != XC_OK) return bail(_r); } while (0)
   UP(d_px, hp.px); UP(d_py, hp.py); UP(d_pz, hp.pz); UP(d_wq, hp.wq); UP(d_parent, hp.parent);
   UP(d_atoms, hp.atoms); UP(d_invR, invR); UP(d_rnn, rnn);
+  if (hp.spec.partition == 0) {   // SSF pair table: a R_BC, 1 / (a R_BC)
+    std::vector<double2> tab(invR.size());
+    for (size_t k = 0; k < invR.size(); ++k) tab[k] = invR[k] > 0.0 ? make_double2(0.64 / invR[k], invR[k] / 0.64) : make_double2(0.0, 0.0);
+    UP(d_pairtab, tab);
+  }
   UP(d_shells, hp.shells); UP(d_exps, hp.exps); UP(d_coefs, hp.coefs);
   UP(d_batches, hp.batches); UP(d_bshells, hp.bshells); UP(d_bsfoff, hp.bsfoff); UP(d_bfidx, hp.bfidx); UP(d_bfinfo, hp.bfinfo);
   UP(d_wbox, hp.wbox);
@@ -206,7 +212,7 @@ int xc_eval(xc_plan* p, const double* dP, int64_t ldp, double* dV, int64_t ldv, 
   if (!(flags & 1) || !p->weights_valid) {
     WeightArgs wa;
     wa.batches = p->d_batches; wa.watoms = p->d_watoms; wa.atoms = p->d_atoms; wa.invR = p->d_invR; wa.rnn = p->d_rnn;
-    wa.nbr = nullptr; wa.wbox = p->d_wbox; wa.natoms = hp.natoms; wa.px = p->d_px; wa.py = p->d_py; wa.pz = p->d_pz; wa.wq = p->d_wq; wa.parent = p->d_parent; wa.w = p->d_w;
+    wa.pairtab = p->d_pairtab; wa.wbox = p->d_wbox; wa.natoms = hp.natoms; wa.px = p->d_px; wa.py = p->d_py; wa.pz = p->d_pz; wa.wq = p->d_wq; wa.parent = p->d_parent; wa.w = p->d_w;
     if (!hp.wbatch_large.empty()) {   // long lists first: they are the long pole
       CU(launch_weights_batched(hp.spec.partition, wa, p->d_wlarge, (int)hp.wbatch_large.size(), hp.w_warps_large, hp.w_max_large, st));
       ++launches;

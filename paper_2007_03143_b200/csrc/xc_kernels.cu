@@ -322,176 +322,186 @@ __global__ void __launch_bounds__(kWeightThreads) k_weights_batched(WeightArgs a
 }
 
 // ------------------------------------------------------------------------------------------------
-// step (a), hot path for SSF: one CTA per batch, one WARP per point, partner-outer loops.
+// step (a), hot path for SSF: one CTA per batch, one WARP per point, the lanes split the atom list.
 // Exact pruning only; the batch's atom list (planner) is sorted by
-// dmin(atom, batch box) <= r_atom, so every scan stops as soon as dmin reaches its bound:
-//   1. nearest atom m and r_min                        (scan while dmin < r_min)
-//   2. owner candidates B: r_B < kappa r_min, not killed by m or by the 8 box-nearest atoms (mu_BC >= a => P_B = 0);
-//      the parent is evaluated first: P_A = 0 => w = 0 and the point is done
-//   3. for chunks of <= 8 owners: ONE pass over the partners C (scan while dmin < kappa max r_B), the lanes
-//      splitting the C's: r_C costs one sqrt per C for all owners, R_BC = rsqrt from shared-memory coordinates,
-//      s(mu_BC) = 1 exactly when r_C >= kappa r_B.  Lane products are combined by an xor butterfly
-//      (same value in every lane, fixed order => deterministic).
+// dmin(atom, batch box) <= r_atom, so every scan stops as soon as dmin reaches its bound, and all control
+// flow is warp-uniform:
+//   0. r_A < (1-a)/2 R_nn(A)  =>  w = w^q.  The other points of the batch are compacted (in order); a batch
+//      of core points never touches the atom list.
+//   1. nearest atom m, r_min                 (32 atoms per step, scan while dmin < r_min)
+//   2. P_A first: P_A = 0 => w = 0 and the point is done.
+//   3. owner candidates B, 32 per step (scan while dmin < kappa r_min): r_B < kappa r_min and mu_Bm < a;
+//      each surviving candidate's cell product P_B is then evaluated by the whole warp.
+//   A cell product scans the partners C, 32 per step (while dmin < kappa r_B): s(mu_BC) = 1 exactly when
+//   r_C >= r_B + a R_BC (tested on squares, no sqrt), and the scan stops as soon as one mu_BC >= a (P_B = 0).
+//   Lane products are combined by an xor butterfly (same value in every lane) and the owners are summed in
+//   list order, so w is bit-identical from run to run.
 // ------------------------------------------------------------------------------------------------
-constexpr int kOwnChunk = 8;
-constexpr int kOwnMax = 64;
+__device__ __forceinline__ double ssf_cell_product(const double4* __restrict__ sAt, const int* __restrict__ sId, int nC, int lane,
+                                                   double x, double y, double z, double Bx, double By, double Bz, int Bid,
+                                                   double rB, double rB2) {
+  const unsigned FULL = 0xffffffffu;
+  const double kappa = (1.0 + 0.64) / (1.0 - 0.64);
+  const double krB = kappa * rB, f4 = (4.0 * 0.64 * 0.64) * rB2;
+  double part = 1.0;
+  for (int c0 = 0; c0 < nC; c0 += 32) {
+    if (sAt[c0].w >= krB) break;                          // every later C has r_C >= kappa r_B: factor 1
+    const int c = c0 + lane;
+    bool dead = false;
+    if (c < nC) {
+      const double4 at = sAt[c];
+      if (at.w < krB && sId[c] != Bid) {
+        const double dx = x - at.x, dy = y - at.y, dz = z - at.z;
+        const double d2 = dx * dx + dy * dy + dz * dz;                 // r_C^2
+        const double ex = Bx - at.x, ey = By - at.y, ez = Bz - at.z;
+        const double R2 = ex * ex + ey * ey + ez * ez;                 // R_BC^2
+        // s(mu_BC) = 1 exactly  <=>  r_C >= r_B + a R_BC  <=>  t >= 0 and t^2 >= 4 a^2 r_B^2 R_BC^2,
+        // t = r_C^2 - r_B^2 - a^2 R_BC^2   (no square root)
+        const double t = d2 - rB2 - (0.64 * 0.64) * R2;
+        if (!(t >= 0.0 && t * t >= f4 * R2)) {
+          const double zz = (rB - sqrt(d2)) * rsqrt(R2) * (1.0 / 0.64);   // mu_BC / a
+          if (zz >= 1.0) {
+            dead = true;                                               // s = 0: P_B = 0
+          } else if (zz > -1.0) {
+            const double z2 = zz * zz;
+            part *= 0.5 - zz * (35.0 + z2 * (-35.0 + z2 * (21.0 - 5.0 * z2))) * (1.0 / 32.0);
+          }
+        }
+      }
+    }
+    if (__any_sync(FULL, dead)) return 0.0;
+  }
+#pragma unroll
+  for (int o = 16; o >= 1; o >>= 1) part *= __shfl_xor_sync(FULL, part, o);
+  return part;
+}
 
-__global__ void __launch_bounds__(kWeightThreads) k_weights_ssf(WeightArgs a, const int32_t* __restrict__ batch_ids) {
+__global__ void __launch_bounds__(kWeightThreads, 4) k_weights_ssf(WeightArgs a, const int32_t* __restrict__ batch_ids) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ int sCnt[2 * (kWeightThreads / 32)];
   const unsigned FULL = 0xffffffffu;
   const int bid = batch_ids[blockIdx.x];
   const BatchRec b = a.batches[bid];
   const int nC = b.wa_nC, nB = b.wa_nB;
-  double* sX = (double*)smem_raw;
-  double* sY = sX + nC;
-  double* sZ = sY + nC;
-  double* sDm = sZ + nC;
-  double* sOwnR = sDm + nC;                              // [8 warps][kOwnMax]
-  int* sId = (int*)(sOwnR + (kWeightThreads / 32) * kOwnMax);
-  int* sOwn = sId + nC;                                  // [8 warps][kOwnMax]
+  double4* sAt = (double4*)smem_raw;                     // x, y, z, dmin
+  int* sId = (int*)(sAt + nC);
+  short* sList = (short*)(sId + nC);                     // compacted non-trivial points of the batch (<= 512)
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const double aa = 0.64, kappa = (1.0 + aa) / (1.0 - aa);
+
+  // ---- 0. trivial points, ordered compaction of the others ----
+  int rank[2];
+  bool live[2];
+#pragma unroll
+  for (int r = 0; r < 2; ++r) {
+    const int p = r * kWeightThreads + threadIdx.x;
+    live[r] = false;
+    if (p < b.nq) {
+      const int64_t gi = (int64_t)b.pt_off + p;
+      const int A = a.parent[gi];
+      bool trivial = a.natoms == 1;
+      if (!trivial) {
+        double dx = a.px[gi] - a.atoms[3 * A], dy = a.py[gi] - a.atoms[3 * A + 1], dz = a.pz[gi] - a.atoms[3 * A + 2];
+        trivial = sqrt(dx * dx + dy * dy + dz * dz) < 0.5 * (1.0 - aa) * a.rnn[A];
+      }
+      if (trivial) a.w[gi] = a.wq[gi];
+      live[r] = !trivial;
+    }
+    const unsigned mask = __ballot_sync(FULL, live[r]);
+    rank[r] = __popc(mask & ((1u << lane) - 1u));
+    if (lane == 0) sCnt[r * (kWeightThreads / 32) + warp] = __popc(mask);
+  }
+  __syncthreads();
+  int total = 0;
+#pragma unroll
+  for (int r = 0; r < 2; ++r) {
+    int off = 0;
+    for (int k = 0; k < 2 * (kWeightThreads / 32); ++k) {
+      if (k < r * (kWeightThreads / 32) + warp) off += sCnt[k];
+      if (r == 0) total += sCnt[k];
+    }
+    if (live[r]) sList[off + rank[r]] = (short)(r * kWeightThreads + threadIdx.x);
+  }
+  if (total == 0) return;
   {
     const double* box = a.wbox + (size_t)6 * bid;
     for (int c = threadIdx.x; c < nC; c += kWeightThreads) {
       int at = a.watoms[b.wa_off + c];
       double cx = a.atoms[3 * at], cy = a.atoms[3 * at + 1], cz = a.atoms[3 * at + 2];
-      sId[c] = at; sX[c] = cx; sY[c] = cy; sZ[c] = cz;
       double tx = cx < box[0] ? box[0] - cx : (cx > box[3] ? cx - box[3] : 0.0);
       double ty = cy < box[1] ? box[1] - cy : (cy > box[4] ? cy - box[4] : 0.0);
       double tz = cz < box[2] ? box[2] - cz : (cz > box[5] ? cz - box[5] : 0.0);
       // a hair below the true distance: the early exits must never cut an atom that matters
-      sDm[c] = sqrt(tx * tx + ty * ty + tz * tz) * (1.0 - 1e-12) - 1e-12;
+      sAt[c] = make_double4(cx, cy, cz, sqrt(tx * tx + ty * ty + tz * tz) * (1.0 - 1e-12) - 1e-12);
+      sId[c] = at;
     }
   }
   __syncthreads();
-  const double aa = 0.64, kappa = (1.0 + aa) / (1.0 - aa);
-  double* myOwnR = sOwnR + warp * kOwnMax;
-  int* myOwn = sOwn + warp * kOwnMax;
-  for (int p = warp; p < b.nq; p += kWeightThreads / 32) {
-    const int64_t gi = (int64_t)b.pt_off + p;
-    const double x = a.px[gi], y = a.py[gi], z = a.pz[gi], base = a.wq[gi];
+
+  for (int n = warp; n < total; n += kWeightThreads / 32) {
+    const int64_t gi = (int64_t)b.pt_off + sList[n];
+    const double x = a.px[gi], y = a.py[gi], z = a.pz[gi];
     const int A = a.parent[gi];
-    double result = base;
-    bool trivial = a.natoms == 1;
-    double rA = 0.0;
-    if (!trivial) {
-      double dx = x - a.atoms[3 * A], dy = y - a.atoms[3 * A + 1], dz = z - a.atoms[3 * A + 2];
-      rA = sqrt(dx * dx + dy * dy + dz * dz);
-      trivial = rA < 0.5 * (1.0 - aa) * a.rnn[A];
+    // ---- 1. nearest atom ----
+    double rmin2 = 1e300;
+    int im = 0;
+    for (int c0 = 0; c0 < nC; c0 += 32) {
+      const double dm = sAt[c0].w;
+      if (dm > 0.0 && dm * dm >= rmin2) break;
+      const int c = c0 + lane;
+      double d2 = 1e300;
+      if (c < nC) { const double4 at = sAt[c]; const double dx = x - at.x, dy = y - at.y, dz = z - at.z; d2 = dx * dx + dy * dy + dz * dz; }
+      int ci = c;
+#pragma unroll
+      for (int o = 16; o >= 1; o >>= 1) {
+        const double od = __shfl_xor_sync(FULL, d2, o);
+        const int oi = __shfl_xor_sync(FULL, ci, o);
+        if (od < d2 || (od == d2 && oi < ci)) { d2 = od; ci = oi; }
+      }
+      if (d2 < rmin2) { rmin2 = d2; im = ci; }
     }
-    if (!trivial) {
-      // 1. nearest atom
-      double rmin = 1e300;
-      int im = 0x7fffffff;
-      for (int c0 = 0; c0 < nC; c0 += 32) {
-        if (sDm[c0] >= rmin) break;
-        const int c = c0 + lane;
-        double d = 1e300;
-        if (c < nC) { double dx = x - sX[c], dy = y - sY[c], dz = z - sZ[c]; d = sqrt(dx * dx + dy * dy + dz * dz); }
-        int ci = c;
-#pragma unroll
-        for (int o = 16; o >= 1; o >>= 1) {
-          double od = __shfl_xor_sync(FULL, d, o);
-          int oi = __shfl_xor_sync(FULL, ci, o);
-          if (od < d || (od == d && oi < ci)) { d = od; ci = oi; }
+    const double rmin = sqrt(rmin2), own_lim = kappa * rmin, own_lim2 = own_lim * own_lim;
+    const double4 atm = sAt[im];
+    const int mid = sId[im];
+    // ---- 2. the parent's cell product ----
+    const double Ax = a.atoms[3 * A], Ay = a.atoms[3 * A + 1], Az = a.atoms[3 * A + 2];
+    double rA2;
+    { const double dx = x - Ax, dy = y - Ay, dz = z - Az; rA2 = dx * dx + dy * dy + dz * dz; }
+    const double rA = sqrt(rA2);
+    double PA = 0.0;
+    if (!(rA >= own_lim && rA > rmin)) PA = ssf_cell_product(sAt, sId, nC, lane, x, y, z, Ax, Ay, Az, A, rA, rA2);
+    double result = 0.0;
+    if (PA != 0.0) {
+      // ---- 3. the other owners ----
+      double sum = PA;
+      for (int b0 = 0; b0 < nB; b0 += 32) {
+        if (sAt[b0].w >= own_lim) break;
+        const int bb = b0 + lane;
+        bool cand = false;
+        double4 at = make_double4(0.0, 0.0, 0.0, 0.0);
+        double d2 = 0.0;
+        int cid = -1;
+        if (bb < nB) {
+          at = sAt[bb]; cid = sId[bb];
+          const double dx = x - at.x, dy = y - at.y, dz = z - at.z;
+          d2 = dx * dx + dy * dy + dz * dz;
+          cand = at.w < own_lim && cid != A && d2 < own_lim2;          // else r_B >= kappa r_min: P_B = 0 exactly
+          if (cand && cid != mid) {                                    // mu_Bm >= a  =>  P_B = 0
+            const double ex = at.x - atm.x, ey = at.y - atm.y, ez = at.z - atm.z;
+            cand = (sqrt(d2) - rmin) * rsqrt(ex * ex + ey * ey + ez * ez) < aa;
+          }
         }
-        if (d < rmin) { rmin = d; im = ci; }
+        unsigned mask = __ballot_sync(FULL, cand);
+        while (mask) {
+          const int src = __ffs(mask) - 1;
+          mask &= mask - 1;
+          const double Bx = __shfl_sync(FULL, at.x, src), By = __shfl_sync(FULL, at.y, src), Bz = __shfl_sync(FULL, at.z, src);
+          const double rB2 = __shfl_sync(FULL, d2, src);
+          const int Bid = __shfl_sync(FULL, cid, src);
+          sum += ssf_cell_product(sAt, sId, nC, lane, x, y, z, Bx, By, Bz, Bid, sqrt(rB2), rB2);
+        }
       }
-      if (rA >= kappa * rmin && rA > rmin) {
-        result = 0.0;                                     // P_A = 0 exactly
-      } else {
-        // distances to the 8 box-nearest atoms (extra exact kill tests)
-        const int nk = min(8, nC);
-        double rk = 1e300;
-        if (lane < nk) { double dx = x - sX[lane], dy = y - sY[lane], dz = z - sZ[lane]; rk = sqrt(dx * dx + dy * dy + dz * dz); }
-        // 2. owner candidates, parent first
-        int nown = 0;
-        const double own_lim = kappa * rmin;
-        bool parent_alive = false;
-        for (int b0 = 0; b0 < nB; b0 += 32) {
-          if (sDm[b0] >= own_lim) break;
-          const int bb = b0 + lane;
-          bool cand = false;
-          double rB = 0.0;
-          if (bb < nB) {
-            const double bx = sX[bb], by = sY[bb], bz = sZ[bb];
-            double dx = x - bx, dy = y - by, dz = z - bz;
-            rB = sqrt(dx * dx + dy * dy + dz * dz);
-            cand = bb == im || rB < own_lim;
-            if (cand && bb != im) {
-              double ex = bx - sX[im], ey = by - sY[im], ez = bz - sZ[im];
-              cand = (rB - rmin) * rsqrt(ex * ex + ey * ey + ez * ez) < aa;
-            }
-          }
-          // kill tests against the 8 box-nearest atoms (shuffles outside the divergent region)
-#pragma unroll
-          for (int c = 0; c < 8; ++c) {
-            const double rc = __shfl_sync(FULL, rk, c);
-            if (cand && c < nk && c != bb) {
-              double ex = sX[bb] - sX[c], ey = sY[bb] - sY[c], ez = sZ[bb] - sZ[c];
-              cand = (rB - rc) * rsqrt(ex * ex + ey * ey + ez * ez) < aa;
-            }
-          }
-          const bool isA = cand && sId[bb] == A;
-          if (__any_sync(FULL, isA)) parent_alive = true;
-          unsigned mask = __ballot_sync(FULL, cand && !isA);
-          // parent goes to slot 0; the others are appended in list order
-          int pos = nown + __popc(mask & ((1u << lane) - 1u)) + 1;   // slot 0 reserved for the parent
-          if (cand && !isA && pos < kOwnMax) { myOwn[pos] = bb; myOwnR[pos] = rB; }
-          if (isA) { myOwn[0] = bb; myOwnR[0] = rB; }
-          nown += __popc(mask);
-        }
-        __syncwarp();
-        if (!parent_alive) {
-          result = 0.0;                                   // the parent was killed: P_A = 0 exactly
-        } else {
-          nown = min(nown + 1, kOwnMax);                  // + parent in slot 0
-          double sum = 0.0, PA = 0.0;
-          for (int o0 = 0; o0 < nown; o0 += kOwnChunk) {
-            const int K = min(kOwnChunk, nown - o0);
-            double part[kOwnChunk], rBk[kOwnChunk];
-            int ok[kOwnChunk];
-            double rBmax = 0.0;
-#pragma unroll
-            for (int k = 0; k < kOwnChunk; ++k) {
-              part[k] = 1.0;
-              ok[k] = k < K ? myOwn[o0 + k] : -1;
-              rBk[k] = k < K ? myOwnR[o0 + k] : 0.0;
-              rBmax = fmax(rBmax, rBk[k]);
-            }
-            const double clim = kappa * rBmax;
-            for (int c0 = 0; c0 < nC; c0 += 32) {
-              if (sDm[c0] >= clim) break;
-              const int c = c0 + lane;
-              if (c < nC) {
-                const double cx = sX[c], cy = sY[c], cz = sZ[c];
-                double dx = x - cx, dy = y - cy, dz = z - cz;
-                const double rC = sqrt(dx * dx + dy * dy + dz * dz);
-#pragma unroll
-                for (int k = 0; k < kOwnChunk; ++k) {
-                  if (k < K && c != ok[k] && rC < kappa * rBk[k]) {   // else: not an owner slot / B itself / factor exactly 1
-                    double ex = cx - sX[ok[k]], ey = cy - sY[ok[k]], ez = cz - sZ[ok[k]];
-                    part[k] *= s_ssf((rBk[k] - rC) * rsqrt(ex * ex + ey * ey + ez * ez));
-                  }
-                }
-              }
-            }
-#pragma unroll
-            for (int k = 0; k < kOwnChunk; ++k) {
-              double v = part[k];
-#pragma unroll
-              for (int o = 16; o >= 1; o >>= 1) v *= __shfl_xor_sync(FULL, v, o);
-              if (k < K) {
-                sum += v;
-                if (o0 == 0 && k == 0) PA = v;
-              }
-            }
-            if (o0 == 0 && PA == 0.0) break;              // P_A = 0 => w = 0, whatever the others are
-          }
-          result = PA == 0.0 ? 0.0 : base * PA / sum;
-        }
-        __syncwarp();
-      }
+      result = a.wq[gi] * PA / sum;
     }
     if (lane == 0) a.w[gi] = result;
   }
@@ -932,7 +942,7 @@ cudaError_t launch_weights_batched(int partition, const WeightArgs& a, const int
   size_t smem = weights_smem_bytes(max_list, nwarps);
   cudaError_t e;
   if (partition == 0) {
-    smem = (size_t)max_list * 36 + (size_t)(kWeightThreads / 32) * kOwnMax * 12 + 64;   // list: x,y,z,dmin,id; per-warp owner slots
+    smem = (size_t)max_list * 36 + 1024 + 64;   // list: x,y,z,dmin,id; compacted point list
     e = cudaFuncSetAttribute(k_weights_ssf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(smem, 1024));
     if (e != cudaSuccess) return e;
     k_weights_ssf<<<nbatches, kWeightThreads, smem, st>>>(a, batch_ids);

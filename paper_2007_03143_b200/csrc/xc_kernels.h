@@ -27,7 +27,7 @@ struct WeightArgs {
   const BatchRec* batches;
   const int32_t* watoms;
   const double* atoms; const double* invR; const double* rnn;
-  const double* nbr;    // [natoms][natoms-1][5]: x,y,z of the k-th nearest neighbour atom, a*R, 1/(a*R)
+  const double2* pairtab;  // [natoms][natoms]: a R_BC, 1 / (a R_BC)  (a = 0.64, SSF)
   const double* wbox;   // [nbatch][6] tight bounding boxes (lo xyz, hi xyz)
   int natoms;
   const double* px; const double* py; const double* pz; const double* wq; const int32_t* parent;

@@ -438,7 +438,7 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
   }
   // warps per CTA of the large-list weights launch: per-warp distance rows must fit in shared memory
   hp.w_warps_large = 8;
-  if (spec->partition == 0 && (size_t)hp.w_max_large * 36 + 8 * 64 * 12 + 64 > kSmemLimit) {
+  if (spec->partition == 0 && (size_t)hp.w_max_large * 36 + 512 * 30 + 2048 * 4 + 64 > kSmemLimit) {
     err = "too many atoms inside the SSF support of one batch for the weights kernel"; return XC_EUNSUPPORTED;
   }
   while (spec->partition != 0 && hp.w_warps_large > 1 && weights_smem_bytes(hp.w_max_large, hp.w_warps_large) > kSmemLimit) hp.w_warps_large >>= 1;
