@@ -110,7 +110,7 @@ def run_workload(name, steps, warmup, functional=None, do_e2e=True, device=0, sa
     for _ in range(warmup):
         plan.eval(P, V)
     torch.cuda.synchronize()
-    stage = {"weights_ms": 0.0, "density_ms": 0.0, "potential_ms": 0.0, "finalize_ms": 0.0}
+    stage = {"weights_ms": 0.0, "pack_ms": 0.0, "batch_ms": 0.0, "finalize_ms": 0.0}
     launches = 0
     E = N = 0.0
     ctx = sampler if sampler is not None else ClockSampler(device)
@@ -270,7 +270,7 @@ def main():
     st = res["stage_ms"]
     stats = res["stats"]
     gga = w.functional == 1
-    dom = max(("weights_ms", "density_ms", "potential_ms"), key=lambda k: st[k])
+    dom = max(("weights_ms", "batch_ms"), key=lambda k: st[k])
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
@@ -279,13 +279,13 @@ def main():
                 traffic = json.load(fh).get(args.workload, {}).get(dom)
         except Exception:
             traffic = None
-    half = 0.5 * res["flops"]   # X GEMM and SYR2K are 2 (N_b^j)^2 N_q^j each
-    if dom == "density_ms":
-        roof = {"kernel": "k_density", "bound": "tensor", "achieved": half / (st[dom] * 1e-3) * 1e-12, "peak": FP64_PEAK_TFLOPS,
-                "unit": "TFLOP/s"}
-    elif dom == "potential_ms":
-        roof = {"kernel": "k_potential", "bound": "tensor", "achieved": half / (st[dom] * 1e-3) * 1e-12, "peak": FP64_PEAK_TFLOPS,
-                "unit": "TFLOP/s"}
+    # algorithmic flops of the dense contractions: X GEMM 2 (N_b^j)^2 N_q^j, V^j 2 (N_b^j)^2 N_q^j (GGA, SYR2K triangle)
+    # or (N_b^j)^2 N_q^j (LDA, SYRK triangle): "count what the method needs"
+    contraction_flops = res["flops"] * (1.0 if gga else 0.75)
+    batch_roof = {"kernel": "k_xc_batch", "bound": "tensor", "achieved": contraction_flops / (st["batch_ms"] * 1e-3) * 1e-12,
+                  "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s"}
+    if dom == "batch_ms":
+        roof = batch_roof
     else:
         # step (a) is plain FP64 ALU work; algorithmic bytes are 44 B/point (x,y,z,w^q,parent in; w out)
         roof = {"kernel": "k_weights", "bound": "hbm", "achieved": 44.0 * res["n_points"] / (st[dom] * 1e-3) * 1e-9,

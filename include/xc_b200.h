@@ -106,12 +106,13 @@ int xc_eval_host(xc_plan* plan, const double* hP, int64_t ldp, double* hV, int64
 int xc_eval_diagnostics(xc_plan* plan, double* w, double* rho, double* grad_rho, double* E_batch, double* N_batch);
 
 /* Device time in milliseconds of each stage of the last xc_eval (CUDA events on the eval stream):
- * ms[0] weights (a), ms[1] density kernel (c,d1,e,f,Z), ms[2] potential kernel (d2 + scatter g), ms[3] finalise, ms[4] total.
+ * ms[0] weights (a), ms[1] P^j pack (d1 gather; includes zeroing the accumulators), ms[2] fused batch kernel (c,d1,e,f,d2,g),
+ * ms[3] finalise, ms[4] total.
  * launches: number of kernel launches of that xc_eval. */
 int xc_eval_timings(const xc_plan* plan, float ms[5], int32_t* launches);
 
 /* Algorithmic sizes of the plan used by the roofline report: [0] sum_j N_b^j N_q^j (function-points),
- * [1] sum_j (N_b^j)^2, [2] sum_j 4 (N_b^j)^2 N_q^j, [3] max N_b^j, [4] mean N_q^j, [5] bytes of Phi/Z workspace. */
+ * [1] sum_j (N_b^j)^2, [2] sum_j 4 (N_b^j)^2 N_q^j, [3] max N_b^j, [4] mean N_q^j, [5] bytes of the packed-P^j buffer. */
 int xc_plan_stats(const xc_plan* plan, double stats[6]);
 
 int xc_plan_destroy(xc_plan* plan);

@@ -201,7 +201,7 @@ class Plan:
         ms = (C.c_float * 5)()
         n = C.c_int32()
         _check(_lib.xc_eval_timings(self._h, ms, C.byref(n)))
-        return dict(weights_ms=ms[0], density_ms=ms[1], potential_ms=ms[2], finalize_ms=ms[3], total_ms=ms[4],
+        return dict(weights_ms=ms[0], pack_ms=ms[1], batch_ms=ms[2], finalize_ms=ms[3], total_ms=ms[4],
                     launches=n.value)
 
     def close(self):

@@ -52,9 +52,8 @@ struct xc_plan {
   double *d_wbox = nullptr;
   double2* d_pairtab = nullptr;
   int32_t *d_watoms = nullptr, *d_wsmall = nullptr, *d_wlarge = nullptr;
-  DensityItem *d_items64 = nullptr, *d_items32 = nullptr;
-  PotItem* d_pot = nullptr;
-  double *d_phi = nullptr, *d_z = nullptr;
+  int32_t *d_ids_small = nullptr, *d_ids_large = nullptr;
+  double* d_ppk = nullptr;
   unsigned long long *d_vhi = nullptr, *d_vlo = nullptr;
   double *d_Epart = nullptr, *d_Npart = nullptr, *d_result = nullptr;
   double *d_rho = nullptr, *d_grho = nullptr;
@@ -71,8 +70,8 @@ static void free_plan(xc_plan* p) {
   if (p->device < 0) { delete p; return; }
   cudaSetDevice(p->device);
   void* ptrs[] = {p->d_px, p->d_py, p->d_pz, p->d_wq, p->d_w, p->d_parent, p->d_atoms, p->d_invR, p->d_rnn, p->d_shells,
-                  p->d_exps, p->d_coefs, p->d_batches, p->d_bshells, p->d_bsfoff, p->d_bfidx, p->d_bfinfo, p->d_items64,
-                  p->d_items32, p->d_pot, p->d_phi, p->d_z, p->d_vhi, p->d_vlo, p->d_Epart, p->d_Npart, p->d_result,
+                  p->d_exps, p->d_coefs, p->d_batches, p->d_bshells, p->d_bsfoff, p->d_bfidx, p->d_bfinfo, p->d_ids_small,
+                  p->d_ids_large, p->d_ppk, p->d_vhi, p->d_vlo, p->d_Epart, p->d_Npart, p->d_result,
                   p->d_rho, p->d_grho, p->d_Ptmp, p->d_Vtmp, p->d_watoms, p->d_wsmall, p->d_wlarge, p->d_pairtab, p->d_wbox};
   for (void* q : ptrs) if (q) cudaFree(q);
   if (p->h_result) cudaFreeHost(p->h_result);
@@ -146,17 +145,19 @@ int xc_plan_create(const xc_atom* atoms, int32_t natoms, const xc_shell* shells,
   UP(d_batches, hp.batches); UP(d_bshells, hp.bshells); UP(d_bsfoff, hp.bsfoff); UP(d_bfidx, hp.bfidx); UP(d_bfinfo, hp.bfinfo);
   UP(d_wbox, hp.wbox);
   UP(d_watoms, hp.watoms); UP(d_wsmall, hp.wbatch_small); UP(d_wlarge, hp.wbatch_large);
-  UP(d_items64, hp.items64); UP(d_items32, hp.items32); UP(d_pot, hp.pot_items);
+  UP(d_ids_small, hp.ids_small); UP(d_ids_large, hp.ids_large);
 #undef UP
-  size_t nitems = hp.items64.size() + hp.items32.size();
+  size_t nitems = hp.batches.size();
   size_t nb2 = (size_t)hp.nbasis * hp.nbasis;
 #define AL(d, bytes) do { cudaError_t _e = cudaMalloc((void**)&p->d, std::max<size_t>((bytes), 8)); if (_e != cudaSuccess) return bail(cuda_fail(_e, "cudaMalloc " #d)); } while (0)
-  AL(d_w, hp.npts * 8); AL(d_phi, (size_t)hp.scr_cap_doubles * 8); AL(d_z, (size_t)hp.scr_cap_doubles * 8);
+  AL(d_w, hp.npts * 8); AL(d_ppk, (size_t)hp.ppk_doubles * 8);
   AL(d_vhi, nb2 * 8); AL(d_vlo, nb2 * 8); AL(d_Epart, nitems * 8); AL(d_Npart, nitems * 8); AL(d_result, 16);
   AL(d_rho, hp.npts * 8); AL(d_grho, hp.npts * 24);
 #undef AL
+  if (cudaMemset(p->d_Epart, 0, std::max<size_t>(nitems * 8, 8)) != cudaSuccess || cudaMemset(p->d_Npart, 0, std::max<size_t>(nitems * 8, 8)) != cudaSuccess)
+    return bail(fail(XC_ECUDA, "cudaMemset failed"));   // batches without functions never write their partials
   if (cudaMallocHost((void**)&p->h_result, 16) != cudaSuccess) return bail(fail(XC_ENOMEM, "cudaMallocHost failed"));
-  p->ev.resize(4 + 2 * hp.chunks.size());
+  p->ev.resize(5);
   for (auto& e : p->ev)
     if (cudaEventCreate(&e) != cudaSuccess) return bail(fail(XC_ECUDA, "cudaEventCreate failed"));
   *out = p;
@@ -178,7 +179,7 @@ int xc_plan_stats(const xc_plan* p, double stats[6]) {
   if (!p || !stats) return fail(XC_EINVAL, "null argument");
   stats[0] = p->hp.sum_nbnq; stats[1] = p->hp.sum_nb2; stats[2] = p->hp.flops; stats[3] = p->hp.max_nb;
   stats[4] = p->hp.batches.empty() ? 0.0 : (double)p->hp.npts / (double)p->hp.batches.size();
-  stats[5] = 16.0 * (double)p->hp.scr_doubles;
+  stats[5] = 8.0 * (double)p->hp.ppk_doubles;
   return XC_OK;
 }
 
@@ -229,33 +230,23 @@ int xc_eval(xc_plan* p, const double* dP, int64_t ldp, double* dV, int64_t ldv, 
   CU(cudaMemsetAsync(p->d_vlo, 0, nb2 * 8, st));
   CU(cudaMemsetAsync(p->d_rho, 0, hp.npts * 8, st));
   CU(cudaMemsetAsync(p->d_grho, 0, hp.npts * 24, st));
-  DensityArgs da;
-  da.batches = p->d_batches; da.bshells = p->d_bshells; da.bsfoff = p->d_bsfoff; da.bfidx = p->d_bfidx; da.bfinfo = p->d_bfinfo;
-  da.shells = p->d_shells; da.exps = p->d_exps; da.coefs = p->d_coefs;
-  da.px = p->d_px; da.py = p->d_py; da.pz = p->d_pz; da.w = p->d_w;
-  da.P = dP; da.ldp = ldp; da.phi_scr = p->d_phi; da.z_scr = p->d_z;
-  da.rho_out = p->d_rho; da.grho_out = gga ? p->d_grho : nullptr;
-  da.Epart = p->d_Epart; da.Npart = p->d_Npart; da.rho_tol = hp.spec.rho_tol;
-  PotArgs pa;
-  pa.batches = p->d_batches; pa.bfidx = p->d_bfidx; pa.phi_scr = p->d_phi; pa.z_scr = p->d_z;
-  pa.vhi = p->d_vhi; pa.vlo = p->d_vlo; pa.nbasis = hp.nbasis;
-  const int n64 = (int)hp.items64.size();
-  for (const auto& c : hp.chunks) {
-    if (c.i64_1 > c.i64_0) {
-      CU(launch_density(64, gga, da, p->d_items64 + c.i64_0, (int)(c.i64_1 - c.i64_0), (int)c.i64_0, hp.smem64, st));
-      ++launches;
-    }
-    if (c.i32_1 > c.i32_0) {
-      CU(launch_density(32, gga, da, p->d_items32 + c.i32_0, (int)(c.i32_1 - c.i32_0), n64 + (int)c.i32_0, hp.smem32, st));
-      ++launches;
-    }
-    CU(cudaEventRecord(p->ev[ie++], st));
-    pa.items = p->d_pot + c.p0; pa.nitems = c.p1 - c.p0;
-    if (pa.nitems > 0) { CU(launch_potential(pa, st)); ++launches; }
-    CU(cudaEventRecord(p->ev[ie++], st));
-  }
+  BatchArgs ba;
+  ba.batches = p->d_batches; ba.bshells = p->d_bshells; ba.bsfoff = p->d_bsfoff; ba.bfidx = p->d_bfidx; ba.bfinfo = p->d_bfinfo;
+  ba.shells = p->d_shells; ba.exps = p->d_exps; ba.coefs = p->d_coefs;
+  ba.px = p->d_px; ba.py = p->d_py; ba.pz = p->d_pz; ba.w = p->d_w;
+  ba.P = dP; ba.ldp = ldp; ba.ppk = p->d_ppk;
+  ba.rho_out = p->d_rho; ba.grho_out = gga ? p->d_grho : nullptr;
+  ba.Epart = p->d_Epart; ba.Npart = p->d_Npart; ba.vhi = p->d_vhi; ba.vlo = p->d_vlo; ba.nbasis = hp.nbasis;
+  ba.rho_tol = hp.spec.rho_tol;
+  // P^j pack (Alg. 4 l.4.2), then the fused batch kernel (l.4.3-4.10); large N_b^j first
+  if (!hp.ids_large.empty()) { CU(launch_pack(ba, p->d_ids_large, (int)hp.ids_large.size(), st)); ++launches; }
+  if (!hp.ids_small.empty()) { CU(launch_pack(ba, p->d_ids_small, (int)hp.ids_small.size(), st)); ++launches; }
+  CU(cudaEventRecord(p->ev[ie++], st));
+  if (!hp.ids_large.empty()) { CU(launch_batch(1, gga, ba, p->d_ids_large, (int)hp.ids_large.size(), hp.smem_large, st)); ++launches; }
+  if (!hp.ids_small.empty()) { CU(launch_batch(0, gga, ba, p->d_ids_small, (int)hp.ids_small.size(), hp.smem_small, st)); ++launches; }
+  CU(cudaEventRecord(p->ev[ie++], st));
   CU(launch_finalize(hp.nbasis, p->d_vhi, p->d_vlo, dV, ldv, st));
-  CU(launch_reduce((int64_t)(hp.items64.size() + hp.items32.size()), p->d_Epart, p->d_Npart, p->d_result, st));
+  CU(launch_reduce((int64_t)hp.batches.size(), p->d_Epart, p->d_Npart, p->d_result, st));
   launches += 2;
   CU(cudaMemcpyAsync(p->h_result, p->d_result, 16, cudaMemcpyDeviceToHost, st));
   CU(cudaEventRecord(p->ev[ie++], st));
@@ -266,14 +257,10 @@ int xc_eval(xc_plan* p, const double* dP, int64_t ldp, double* dV, int64_t ldv, 
   float t;
   p->ms[0] = p->ms[1] = p->ms[2] = p->ms[3] = p->ms[4] = 0.f;
   CU(cudaEventElapsedTime(&t, p->ev[0], p->ev[1])); p->ms[0] = t;
-  size_t k = 1;
-  for (size_t c = 0; c < hp.chunks.size(); ++c) {
-    CU(cudaEventElapsedTime(&t, p->ev[k], p->ev[k + 1])); p->ms[1] += t;   // includes the memsets on the first chunk
-    CU(cudaEventElapsedTime(&t, p->ev[k + 1], p->ev[k + 2])); p->ms[2] += t;
-    k += 2;
-  }
-  CU(cudaEventElapsedTime(&t, p->ev[k], p->ev[k + 1])); p->ms[3] = t;
-  CU(cudaEventElapsedTime(&t, p->ev[0], p->ev[k + 1])); p->ms[4] = t;
+  CU(cudaEventElapsedTime(&t, p->ev[1], p->ev[2])); p->ms[1] = t;   // includes the memsets
+  CU(cudaEventElapsedTime(&t, p->ev[2], p->ev[3])); p->ms[2] = t;
+  CU(cudaEventElapsedTime(&t, p->ev[3], p->ev[4])); p->ms[3] = t;
+  CU(cudaEventElapsedTime(&t, p->ev[0], p->ev[4])); p->ms[4] = t;
   p->launches = launches;
   return XC_OK;
 }
@@ -303,22 +290,8 @@ int xc_eval_diagnostics(xc_plan* p, double* w, double* rho, double* grad_rho, do
   if (w) CU(cudaMemcpy(w, p->d_w, hp.npts * 8, cudaMemcpyDeviceToHost));
   if (rho) CU(cudaMemcpy(rho, p->d_rho, hp.npts * 8, cudaMemcpyDeviceToHost));
   if (grad_rho) CU(cudaMemcpy(grad_rho, p->d_grho, hp.npts * 24, cudaMemcpyDeviceToHost));
-  if (E_batch || N_batch) {
-    size_t n64 = hp.items64.size(), n32 = hp.items32.size();
-    std::vector<double> ep(n64 + n32), np(n64 + n32);
-    if (n64 + n32) {
-      CU(cudaMemcpy(ep.data(), p->d_Epart, ep.size() * 8, cudaMemcpyDeviceToHost));
-      CU(cudaMemcpy(np.data(), p->d_Npart, np.size() * 8, cudaMemcpyDeviceToHost));
-    }
-    size_t nb = hp.batches.size();
-    if (E_batch) std::fill(E_batch, E_batch + nb, 0.0);
-    if (N_batch) std::fill(N_batch, N_batch + nb, 0.0);
-    for (size_t i = 0; i < n64 + n32; ++i) {
-      int j = i < n64 ? hp.items64[i].batch : hp.items32[i - n64].batch;
-      if (E_batch) E_batch[j] += ep[i];
-      if (N_batch) N_batch[j] += np[i];
-    }
-  }
+  if (E_batch && !hp.batches.empty()) CU(cudaMemcpy(E_batch, p->d_Epart, hp.batches.size() * 8, cudaMemcpyDeviceToHost));
+  if (N_batch && !hp.batches.empty()) CU(cudaMemcpy(N_batch, p->d_Npart, hp.batches.size() * 8, cudaMemcpyDeviceToHost));
   return XC_OK;
 }
 

@@ -11,11 +11,9 @@ namespace xcb {
 
 constexpr int kMaxL = 2;
 constexpr int kMaxPrim = 16;
-constexpr int kKC = 8;          // nu-rows of P staged per pipeline stage in the density kernel
-constexpr int kMuPass = 192;    // mu columns handled per pass of the density kernel
-constexpr int kDensityThreads = 512;
-constexpr int kPotThreads = 256;
-constexpr int kPotKPart = 128;  // points per work item of the potential kernel
+constexpr int kBatchThreads = 512;  // 16 warps per batch CTA
+constexpr int kSmallNb = 112;   // N_b^j limit of the 64-point-tile instantiation (<= 28 lower-triangle 16x16 blocks = 2 per warp)
+constexpr int kMaxNb = 192;     // N_b^j limit of the batch kernel (<= 78 blocks = 5 per warp); the planner splits larger batches
 constexpr size_t kSmemLimit = 227 * 1024;
 constexpr int kWeightSmallList = 192; // atom-list length that separates the two launches of the weights kernel
 constexpr int kWeightThreads = 256;
@@ -28,23 +26,18 @@ struct ShellRec {      // 48 bytes
 
 struct BatchRec {      // one quadrature batch B_j with its shell list S_j
   int32_t pt_off, nq;          // first point (plan order), N_q^j
-  int32_t nq_pad;              // N_q^j rounded up to 4
   int32_t sh_off, ns;          // offset into batch shell list, |S_j| in shells
   int32_t f_off, nb;           // offset into batch function-index list, N_b^j
-  int32_t nb_pad8;             // N_b^j rounded up to 8
-  int64_t scr_off;             // offset (doubles) of this batch's Phi / Z workspace
+  int64_t ppk_off;             // offset (doubles) of this batch's packed P^j (nb4 x nb8, DMMA fragment order)
   int64_t wa_off;              // offset into the weight-kernel atom lists
   int32_t wa_nB, wa_nC;        // atoms that can own weight here / atoms that can appear in a cell product
 };
 
-struct DensityItem { int32_t batch, tile_start; };            // one CTA of the density kernel
-struct PotItem { int32_t batch; int16_t tm, tn; int32_t k0, k1; };  // one warp of the potential kernel
-
 inline int ncart(int L) { return (L + 1) * (L + 2) / 2; }
 inline int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
 
-// shared-memory footprint of the density kernel for a batch (bytes); T = points per tile
-size_t density_smem_bytes(int T, bool gga, int nb, int ns);
+// shared-memory footprint of the batch kernel for a batch (bytes); T = points per tile
+size_t batch_smem_bytes(int T, bool gga, int nb, int ns);
 size_t weights_smem_bytes(int nC, int warps);
 
 struct HostPlan {
@@ -66,15 +59,11 @@ struct HostPlan {
   std::vector<double> wbox;            // [nbatch][6] tight bounding boxes
   std::vector<int32_t> wbatch_small, wbatch_large;  // batch ids by list length (two launches)
   int w_max_small = 0, w_max_large = 0, w_warps_large = 8;
-  std::vector<DensityItem> items64, items32;  // density-kernel work lists (tile of 64 / 32 points)
-  std::vector<PotItem> pot_items;
-  struct Chunk { int64_t b0, b1, i64_0, i64_1, i32_0, i32_1, p0, p1; int64_t scr; };
-  std::vector<Chunk> chunks;            // batches [b0,b1) share one pass over the Phi/Z workspace
-  int64_t scr_cap_doubles = 0;          // workspace doubles per matrix (max over chunks)
-  int64_t scr_doubles = 0;
+  std::vector<int32_t> ids_small, ids_large;  // batch-kernel work lists (N_b^j <= kSmallNb / the others), heaviest first
+  int64_t ppk_doubles = 0;              // size of the packed-P^j buffer
   double sum_nbnq = 0, sum_nb2 = 0, flops = 0;
   int max_nb = 0, max_ns = 0;
-  size_t smem64 = 0, smem32 = 0;       // max dynamic smem over each density work list
+  size_t smem_small = 0, smem_large = 0;  // max dynamic smem over each work list
 };
 
 // Builds grid, batches, screening, work lists.  Returns XC_OK or an error code (message in err).

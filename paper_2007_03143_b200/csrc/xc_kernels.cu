@@ -1,9 +1,10 @@
 // xc_kernels.cu -- CUDA kernels (sm_100a) of libxc_b200: the hot path of Alg. 4.
 //
 //   k_weights   step (a)   partition weights, Eq. (9), Alg. 4 l.4.1
-//   k_density   steps (c),(d1),(e),(f) + Z of (d2): collocation Eq. (7)/(12a), X = P^j Phi^j Eq. (15),
-//               rho / grad rho Eqs. (13),(14), functional Eq. (19), E/N Eq. (16), Z Eq. (20)
-//   k_potential step (d2),(g): V^j = Z Phi^T + Phi Z^T Eq. (18) and the increment Eq. (17)
+//   k_pack_P    step (d1) gather: P^j Eq. (12b), packed once per batch in DMMA fragment order
+//   k_xc_batch  steps (c)-(g) fused, one CTA per batch: collocation Eq. (7)/(12a), X = P^j Phi^j Eq. (15),
+//               rho / grad rho Eqs. (13),(14), functional Eq. (19), E/N Eq. (16), Z Eq. (20),
+//               V^j = Z Phi^T + Phi Z^T Eq. (18) in registers, increment Eq. (17)
 //   k_finalize  fixed point -> fp64, mirror to the full symmetric V
 //
 // The dense contractions run on the FP64 tensor path (mma.sync m8n8k4 f64 -> DMMA.8x8x4 SASS), which on
@@ -27,14 +28,6 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
                : "+d"(c0), "+d"(c1)
                : "d"(a), "d"(b));
 }
-__device__ __forceinline__ void cp_async8(void* smem, const void* gmem) {
-  unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(s), "l"(gmem));
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
-
 __device__ __forceinline__ double pw012(double v, int n) { return n == 0 ? 1.0 : (n == 1 ? v : v * v); }
 __device__ __forceinline__ double dpw012(double v, int n) { return n == 0 ? 0.0 : (n == 1 ? 1.0 : 2.0 * v); }
 
@@ -508,282 +501,30 @@ __global__ void __launch_bounds__(kWeightThreads, 4) k_weights_ssf(WeightArgs a,
 }
 
 // ------------------------------------------------------------------------------------------------
-// density kernel.  One CTA (512 threads) = one tile of T points of one batch.
-//   phase 0  metadata -> smem
-//   phase 1  collocation: radial sums R0,R1 per (shell, point) -> sR; Phi -> sPhi[nu][i]
-//   phase 2  X^T = Phi^T P  on DMMA (M = points, N = mu, K = nu): A from sPhi, B = P gathered through a
-//            cp.async double buffer; epilogue: rho_i += Phi X, grad rho_i += grad Phi X
-//   phase 3  functional at the T points, E / N_el partials
-//   phase 4  Z = 1/2 a Phi + g . grad Phi; Phi and Z stored fragment-blocked for k_potential
+// P^j pack (Eq. (12b), Alg. 4 l.4.2): gathers the batch's block of P ONCE per build into the
+// DMMA B-fragment order the batch kernel consumes: for k-step ks (4 nu) and column tile nt (8 mu), 32
+// contiguous doubles, lane (g4 = lane >> 2, t4 = lane & 3) holding P[nu = 4 ks + t4][mu = 8 nt + g4];
+// zero padded to nb4 x nb8.  One warp-wide 256-byte load per fragment in the batch kernel, no index math there.
 // ------------------------------------------------------------------------------------------------
-template <int T>
-struct DensityCfg {
-  static constexpr int WP = T / 16;            // warps along points
-  static constexpr int WM = 16 / WP;           // warps along mu
-  static constexpr int NTMAX = kMuPass / (8 * WM);
-  static constexpr int LD = T + 4;             // == 4 (mod 16): conflict-free A-fragment reads
-};
-
-template <int T, bool GGA>
-__global__ void __launch_bounds__(kDensityThreads, 1) k_density(DensityArgs a, const DensityItem* __restrict__ items, int item0) {
-  using Cfg = DensityCfg<T>;
-  constexpr int LD = Cfg::LD;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const DensityItem it = items[blockIdx.x];
-  const BatchRec b = a.batches[it.batch];
-  const int nb = b.nb, ns = b.ns, nb4 = (nb + 3) & ~3;
-  const int npass = (nb + kMuPass - 1) / kMuPass;
-  const int mbmax = min((nb + 8 * Cfg::WM - 1) / (8 * Cfg::WM) * (8 * Cfg::WM), kMuPass);
-  const int LDP = mbmax + 4;
-
-  // ---- carve shared memory ----
-  unsigned char* sp = smem_raw;
-  double* sPhi = (double*)sp; sp += (size_t)nb4 * LD * 8;
-  double* sR = (double*)sp; if (GGA) sp += (size_t)ns * T * 16;
-  double* sP = (double*)sp; sp += (size_t)2 * kKC * LDP * 8;
-  double* sPt = (double*)sp; sp += (size_t)12 * T * 8;
-  double* sRed = (double*)sp; sp += (size_t)1024 * 8;   // [WM][4][T], WM*4*T == 1024
-  ShellRec* sSh = (ShellRec*)sp; sp += (size_t)ns * sizeof(ShellRec);
-  int* sIdxMu = (int*)sp; sp += (size_t)npass * kMuPass * 4;
-  int* sIdxNu = (int*)sp; sp += (size_t)nb4 * 4;
-  int* sInfo = (int*)sp;
-  double *sx = sPt, *sy = sPt + T, *sz = sPt + 2 * T, *sw = sPt + 3 * T;
-  double *sRho = sPt + 4 * T, *sGx = sPt + 5 * T, *sGy = sPt + 6 * T, *sGz = sPt + 7 * T;
-  double *sA = sPt + 8 * T, *sG0 = sPt + 9 * T, *sG1 = sPt + 10 * T, *sG2 = sPt + 11 * T;
-
-  // ---- phase 0 ----
+__global__ void __launch_bounds__(256) k_pack_P(BatchArgs a, const int32_t* __restrict__ batch_ids) {
+  const BatchRec b = a.batches[batch_ids[blockIdx.x]];
+  const int nb = b.nb, ntile = (nb + 7) >> 3, nks = (nb + 3) >> 2;
   const int32_t* fidx = a.bfidx + b.f_off;
-  const int32_t* finfo = a.bfinfo + b.f_off;
-  for (int k = tid; k < ns; k += kDensityThreads) {
-    ShellRec r = a.shells[a.bshells[b.sh_off + k]];
-    r._pad = a.bsfoff[b.sh_off + k];
-    sSh[k] = r;
-  }
-  const int idx0 = fidx[0];
-  for (int f = tid; f < nb4; f += kDensityThreads) {
-    sIdxNu[f] = f < nb ? fidx[f] : idx0;
-    sInfo[f] = f < nb ? finfo[f] : 0;
-  }
-  for (int f = tid; f < npass * kMuPass; f += kDensityThreads) sIdxMu[f] = f < nb ? fidx[f] : idx0;
-  const int npt = min(T, b.nq - it.tile_start);  // valid points in this tile
-  if (tid < T) {
-    int li = min(tid, npt - 1);
-    int64_t gi = (int64_t)b.pt_off + it.tile_start + li;
-    sx[tid] = a.px[gi]; sy[tid] = a.py[gi]; sz[tid] = a.pz[gi];
-    sw[tid] = tid < npt ? a.w[gi] : 0.0;
-  }
-  __syncthreads();
-
-  // ---- phase 1: collocation (Eq. (7); same shell across a warp) ----
-  for (int e = tid; e < ns * T; e += kDensityThreads) {
-    int slot = e / T, i = e - slot * T;
-    const ShellRec sh = sSh[slot];
-    double dx = sx[i] - sh.x, dy = sy[i] - sh.y, dz = sz[i] - sh.z;
-    double r2 = dx * dx + dy * dy + dz * dz;
-    double R0 = 0.0, R1 = 0.0;
-    for (int k = 0; k < sh.nprim; ++k) {
-      double al = __ldg(a.exps + sh.prim_off + k), c = __ldg(a.coefs + sh.prim_off + k);
-      double ev = c * exp(-al * r2);
-      R0 += ev;
-      R1 = fma(-2.0 * al, ev, R1);
-    }
-    if (GGA) *reinterpret_cast<double2*>(sR + ((size_t)slot * T + i) * 2) = make_double2(R0, R1);
-    double* dst = sPhi + (size_t)sh._pad * LD + i;
-    if (sh.L == 0) {
-      dst[0] = R0;
-    } else if (sh.L == 1) {
-      dst[0] = dx * R0; dst[LD] = dy * R0; dst[2 * LD] = dz * R0;
-    } else {
-      double xr = dx * R0, yr = dy * R0;
-      dst[0] = dx * xr; dst[LD] = dy * xr; dst[2 * LD] = dz * xr;
-      dst[3 * LD] = dy * yr; dst[4 * LD] = dz * yr; dst[5 * LD] = dz * dz * R0;
-    }
-  }
-  for (int e = tid; e < (nb4 - nb) * T; e += kDensityThreads) sPhi[(size_t)(nb + e / T) * LD + (e % T)] = 0.0;
-  __syncthreads();
-
-  // ---- phase 2: X^T = Phi^T P and the density reductions ----
-  const int wp = warp % Cfg::WP, wm = warp / Cfg::WP;
-  const int g4 = lane >> 2, t4 = lane & 3;
-  double rho_acc[2] = {0.0, 0.0}, gx_acc[2] = {0.0, 0.0}, gy_acc[2] = {0.0, 0.0}, gz_acc[2] = {0.0, 0.0};
-  const int nchunk = (nb4 + kKC - 1) / kKC;
-  for (int pass = 0; pass < npass; ++pass) {
-    const int mu0 = pass * kMuPass;
-    const int mb = min((nb - mu0 + 8 * Cfg::WM - 1) / (8 * Cfg::WM) * (8 * Cfg::WM), kMuPass);
-    const int mbw = mb / Cfg::WM;     // mu columns per warp (multiple of 8)
-    const int nt = mbw >> 3;
-    double C[2][Cfg::NTMAX][2];
-#pragma unroll
-    for (int u = 0; u < 2; ++u)
-#pragma unroll
-      for (int v = 0; v < Cfg::NTMAX; ++v) C[u][v][0] = C[u][v][1] = 0.0;
-
-    auto stage_load = [&](int chunk, int stage) {
-      double* dstS = sP + (size_t)stage * kKC * LDP;
-      const int rows = min(kKC, nb4 - chunk * kKC);
-      for (int e = tid; e < rows * mb; e += kDensityThreads) {
-        int k = e / mb, mcol = e - k * mb;
-        const double* src = a.P + (size_t)sIdxNu[chunk * kKC + k] * a.ldp + sIdxMu[mu0 + mcol];
-        cp_async8(dstS + (size_t)k * LDP + mcol, src);
-      }
-      cp_async_commit();
-    };
-    stage_load(0, 0);
-    for (int chunk = 0; chunk < nchunk; ++chunk) {
-      const int stage = chunk & 1;
-      if (chunk + 1 < nchunk) { stage_load(chunk + 1, stage ^ 1); cp_async_wait<1>(); }
-      else cp_async_wait<0>();
-      __syncthreads();
-      const double* Ps = sP + (size_t)stage * kKC * LDP + wm * mbw + g4;
-      const int steps = min(kKC, nb4 - chunk * kKC) >> 2;
-      for (int ks = 0; ks < steps; ++ks) {
-        const int kk = chunk * kKC + ks * 4 + t4;
-        const double* Ap = sPhi + (size_t)kk * LD + wp * 16 + g4;
-        double A0 = Ap[0], A1 = Ap[8];
-        const double* Bp = Ps + (size_t)(ks * 4 + t4) * LDP;
-#pragma unroll
-        for (int v = 0; v < Cfg::NTMAX; ++v) {
-          if (v < nt) {
-            double Bv = Bp[v * 8];
-            dmma884(C[0][v][0], C[0][v][1], A0, Bv);
-            dmma884(C[1][v][0], C[1][v][1], A1, Bv);
-          }
-        }
-      }
-      __syncthreads();
-    }
-    // epilogue of this pass: Eqs. (13),(14)
-#pragma unroll
-    for (int u = 0; u < 2; ++u) {
-      const int i = wp * 16 + u * 8 + g4;
-      const double xi = sx[i], yi = sy[i], zi = sz[i];
-#pragma unroll
-      for (int v = 0; v < Cfg::NTMAX; ++v) {
-        if (v < nt) {
-#pragma unroll
-          for (int h = 0; h < 2; ++h) {
-            const int mu = mu0 + wm * mbw + v * 8 + t4 * 2 + h;
-            if (mu < nb) {
-              const double X = C[u][v][h];
-              rho_acc[u] = fma(sPhi[(size_t)mu * LD + i], X, rho_acc[u]);
-              if (GGA) {
-                const int info = sInfo[mu];
-                const int slot = info >> 8;
-                const double2 R = *reinterpret_cast<const double2*>(sR + ((size_t)slot * T + i) * 2);
-                double gx, gy, gz;
-                grad_cart(info, xi - sSh[slot].x, yi - sSh[slot].y, zi - sSh[slot].z, R.x, R.y, gx, gy, gz);
-                gx_acc[u] = fma(gx, X, gx_acc[u]);
-                gy_acc[u] = fma(gy, X, gy_acc[u]);
-                gz_acc[u] = fma(gz, X, gz_acc[u]);
-              }
-            }
-          }
-        }
-      }
-    }
-  }
-  // reduce over the 4 lanes sharing a point, then over the WM warps (fixed order => deterministic)
-#pragma unroll
-  for (int u = 0; u < 2; ++u) {
-#pragma unroll
-    for (int o = 1; o <= 2; o <<= 1) {
-      rho_acc[u] += __shfl_xor_sync(0xffffffffu, rho_acc[u], o);
-      if (GGA) {
-        gx_acc[u] += __shfl_xor_sync(0xffffffffu, gx_acc[u], o);
-        gy_acc[u] += __shfl_xor_sync(0xffffffffu, gy_acc[u], o);
-        gz_acc[u] += __shfl_xor_sync(0xffffffffu, gz_acc[u], o);
-      }
-    }
-    if (t4 == 0) {
-      const int i = wp * 16 + u * 8 + g4;
-      sRed[(size_t)(wm * 4 + 0) * T + i] = rho_acc[u];
-      if (GGA) {
-        sRed[(size_t)(wm * 4 + 1) * T + i] = gx_acc[u];
-        sRed[(size_t)(wm * 4 + 2) * T + i] = gy_acc[u];
-        sRed[(size_t)(wm * 4 + 3) * T + i] = gz_acc[u];
-      }
-    }
-  }
-  __syncthreads();
-
-  // ---- phase 3: functional (Eq. (19)), E and N_el partials (Eq. (16)) ----
-  if (tid < T) {
-    double rho = 0.0, gx = 0.0, gy = 0.0, gz = 0.0;
-    for (int q = 0; q < Cfg::WM; ++q) {
-      rho += sRed[(size_t)(q * 4 + 0) * T + tid];
-      if (GGA) {
-        gx += sRed[(size_t)(q * 4 + 1) * T + tid];
-        gy += sRed[(size_t)(q * 4 + 2) * T + tid];
-        gz += sRed[(size_t)(q * 4 + 3) * T + tid];
-      }
-    }
-    gx *= 2.0; gy *= 2.0; gz *= 2.0;
-    const double sigma = gx * gx + gy * gy + gz * gz;
-    const double wi = sw[tid];
-    double f, vr, vs;
-    xc_point<GGA>(rho, sigma, a.rho_tol, f, vr, vs);
-    sA[tid] = 0.5 * wi * vr;
-    const double gs = 2.0 * wi * vs;
-    sG0[tid] = gs * gx; sG1[tid] = gs * gy; sG2[tid] = gs * gz;
-    if (tid < npt && a.rho_out) {
-      int64_t gi = (int64_t)b.pt_off + it.tile_start + tid;
-      a.rho_out[gi] = rho;
-      if (a.grho_out) { a.grho_out[3 * gi] = gx; a.grho_out[3 * gi + 1] = gy; a.grho_out[3 * gi + 2] = gz; }
-    }
-    double e = wi * f, n = wi * rho;
-#pragma unroll
-    for (int o = 16; o >= 1; o >>= 1) {
-      e += __shfl_xor_sync(0xffffffffu, e, o);
-      n += __shfl_xor_sync(0xffffffffu, n, o);
-    }
-    if (lane == 0) { sRho[warp] = e; sGx[warp] = n; }
-  }
-  __syncthreads();
-  if (tid == 0) {
-    double e = 0.0, n = 0.0;
-    for (int q = 0; q < T / 32; ++q) { e += sRho[q]; n += sGx[q]; }
-    a.Epart[item0 + blockIdx.x] = e;
-    a.Npart[item0 + blockIdx.x] = n;
-  }
-
-  // ---- phase 4: Z (Eq. (20)); store Phi and Z in 8x4 fragment blocks ----
-  {
-    const int nkq = b.nq_pad >> 2;             // 4-point chunks per row tile of the batch
-    const int q0 = it.tile_start >> 2;
-    const int nq4 = min(T / 4, nkq - q0);      // chunks of this tile that exist in the workspace
-    const int nmt = b.nb_pad8 >> 3;
-    double* phi_out = a.phi_scr + b.scr_off;
-    double* z_out = a.z_scr + b.scr_off;
-    for (int blk = warp; blk < nmt * nq4; blk += kDensityThreads / 32) {
-      const int mt = blk / nq4, q = blk - mt * nq4;
-      const int mu = mt * 8 + g4, i = q * 4 + t4;
-      double phi = 0.0, zv = 0.0;
-      if (mu < nb && i < npt) {
-        phi = sPhi[(size_t)mu * LD + i];
-        zv = sA[i] * phi;
-        if (GGA) {
-          const int info = sInfo[mu];
-          const int slot = info >> 8;
-          const double2 R = *reinterpret_cast<const double2*>(sR + ((size_t)slot * T + i) * 2);
-          double gx, gy, gz;
-          grad_cart(info, sx[i] - sSh[slot].x, sy[i] - sSh[slot].y, sz[i] - sSh[slot].z, R.x, R.y, gx, gy, gz);
-          zv = fma(sG0[i], gx, fma(sG1[i], gy, fma(sG2[i], gz, zv)));
-        }
-      }
-      const size_t o = ((size_t)mt * nkq + q0 + q) * 32 + lane;
-      phi_out[o] = phi;
-      z_out[o] = zv;
-    }
+  double* out = a.ppk + b.ppk_off;
+  const int total = nks * ntile * 32;
+  for (int e = threadIdx.x; e < total; e += 256) {
+    const int lane = e & 31, frag = e >> 5;
+    const int ks = frag / ntile, nt = frag - ks * ntile;
+    const int nu = 4 * ks + (lane & 3), mu = 8 * nt + (lane >> 2);
+    double v = 0.0;
+    if (nu < nb && mu < nb) v = __ldg(a.P + (size_t)fidx[mu] * a.ldp + fidx[nu]);   // P symmetric: row mu is read along nu
+    out[e] = v;
   }
 }
 
 // ------------------------------------------------------------------------------------------------
-// potential kernel.  One WARP = one work item: a 32x32 lower-triangle tile of V^j over a range of points.
-// Fragments are read straight from the fragment-blocked workspace (one coalesced 256-byte line per
-// fragment); tiles of the same batch run in the same CTA so the panels are shared through L1.
-// The increment Eq. (17) is done in exact 96-bit fixed point (two 64-bit integer atomics), which is
-// associative: V is bit-identical from run to run whatever the order of arrival.
+// exact, order-independent accumulation: 96-bit fixed point (two 64-bit integer atomics) => V is
+// bit-identical from run to run whatever the order in which the batches arrive.
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void fixed_add(unsigned long long* hi, unsigned long long* lo, double v) {
   // x = round(v * 2^64) as a signed 128-bit integer; lo = low 32 bits, hi = x >> 32
@@ -805,74 +546,316 @@ __device__ __forceinline__ void fixed_add(unsigned long long* hi, unsigned long 
   }
 }
 
-__global__ void __launch_bounds__(kPotThreads, 2) k_potential(PotArgs a) {
-  const int lane = threadIdx.x & 31;
-  const int64_t item = (int64_t)blockIdx.x * (kPotThreads / 32) + (threadIdx.x >> 5);
-  if (item >= a.nitems) return;
-  const PotItem it = a.items[item];
-  const BatchRec b = a.batches[it.batch];
-  const int nkq = b.nq_pad >> 2;
-  const int nmt = b.nb_pad8 >> 3;
-  const double* phi = a.phi_scr + b.scr_off;
-  const double* zz = a.z_scr + b.scr_off;
-  const bool diag = it.tm == it.tn;
-  double C[4][4][2];
-#pragma unroll
-  for (int u = 0; u < 4; ++u)
-#pragma unroll
-    for (int v = 0; v < 4; ++v) C[u][v][0] = C[u][v][1] = 0.0;
-  bool vm[4], vn[4];
-  size_t om[4], on[4];
-#pragma unroll
-  for (int u = 0; u < 4; ++u) {
-    vm[u] = it.tm * 4 + u < nmt;
-    vn[u] = it.tn * 4 + u < nmt;
-    om[u] = (size_t)(it.tm * 4 + u) * nkq * 32 + lane;
-    on[u] = (size_t)(it.tn * 4 + u) * nkq * 32 + lane;
-  }
-  for (int kc = it.k0 >> 2; kc < (it.k1 >> 2); ++kc) {
-    double Zm[4], Pm[4], Zn[4], Pn[4];
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      Zm[u] = vm[u] ? __ldg(zz + om[u] + (size_t)kc * 32) : 0.0;
-      Pm[u] = vm[u] ? __ldg(phi + om[u] + (size_t)kc * 32) : 0.0;
-    }
-    if (diag) {
-#pragma unroll
-      for (int u = 0; u < 4; ++u) { Zn[u] = Zm[u]; Pn[u] = Pm[u]; }
-    } else {
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        Zn[u] = vn[u] ? __ldg(zz + on[u] + (size_t)kc * 32) : 0.0;
-        Pn[u] = vn[u] ? __ldg(phi + on[u] + (size_t)kc * 32) : 0.0;
-      }
-    }
-#pragma unroll
-    for (int u = 0; u < 4; ++u)
-#pragma unroll
-      for (int v = 0; v < 4; ++v) {
-        dmma884(C[u][v][0], C[u][v][1], Zm[u], Pn[v]);
-        dmma884(C[u][v][0], C[u][v][1], Pm[u], Zn[v]);
-      }
-  }
-  // scatter: lower triangle (mu >= nu) only; global indices ascend with local ones
-  const int32_t* fidx = a.bfidx + b.f_off;
+// ------------------------------------------------------------------------------------------------
+// batch kernel: ONE CTA (512 threads, 16 warps) = one batch B_j, Alg. 4 l.4.3-4.10 fused.  The CTA walks
+// over the batch's points in tiles of T; nothing but the packed P^j is read from and nothing but the final
+// V^j increment is written to global memory:
+//   per tile   1  collocation: R0, R1 per (shell, point) -> sR (GGA); Phi -> sPhi[nu][i]            Eq. (7)
+//              2  X^T = Phi^T P^j on DMMA (M = points, N = mu, K = nu): A from sPhi, B = packed P^j    Eq. (15)
+//                 epilogue in registers: rho_i += Phi X, grad rho_i += grad Phi X                    Eqs. (13),(14)
+//              3  functional at the T points; E / N_el partials                                     Eqs. (19),(16)
+//              4  GGA: Z = 1/2 a Phi + g . grad Phi -> sZ                                            Eq. (20)
+//              5  V^j += Z Phi^T + Phi Z^T on DMMA, lower-triangle 16x16 blocks, accumulators in     Eq. (18)
+//                 REGISTERS over all tiles of the batch.  LDA: Z = 1/2 a Phi, so V^j = (a Phi) Phi^T is one
+//                 symmetric product (half the flops); the scaling by a_i is applied to the A fragment.
+//   per batch  6  increment of V (Eq. (17)): one fixed-point add per lower-triangle element.
+// ------------------------------------------------------------------------------------------------
+template <int T>
+struct BatchCfg {
+  static constexpr int WP = T / 16;            // warps along points in the X GEMM
+  static constexpr int WM = 16 / WP;           // warps along mu
+  static constexpr int LD = T + 4;             // == 4 (mod 16) doubles: conflict-free fragment reads
+};
+
+template <int T, bool GGA, int NTW, int ROUNDS>
+__global__ void __launch_bounds__(kBatchThreads, 1) k_xc_batch(BatchArgs a, const int32_t* __restrict__ batch_ids) {
+  using Cfg = BatchCfg<T>;
+  constexpr int LD = Cfg::LD;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int g4 = lane >> 2, t4 = lane & 3;
+  const int bidx = batch_ids[blockIdx.x];
+  const BatchRec b = a.batches[bidx];
+  const int nb = b.nb, ns = b.ns;
+  const int nb16 = (nb + 15) & ~15, ntile = (nb + 7) >> 3, nks = (nb + 3) >> 2;
+  const int nbk = nb16 >> 4, nblocks = nbk * (nbk + 1) / 2;
+
+  // ---- carve shared memory (mirrored by batch_smem_bytes in the planner) ----
+  unsigned char* sp = smem_raw;
+  double* sPhi = (double*)sp; sp += (size_t)nb16 * LD * 8;
+  double* sZ = (double*)sp; if (GGA) sp += (size_t)nb16 * LD * 8;
+  double* sR = (double*)sp; if (GGA) sp += (size_t)ns * T * 16;
+  double* sPt = (double*)sp; sp += (size_t)12 * T * 8;
+  double* sRed = (double*)sp; sp += (size_t)1024 * 8;   // [WM][4][T], WM*4*T == 1024
+  ShellRec* sSh = (ShellRec*)sp; sp += (size_t)ns * sizeof(ShellRec);
+  int* sInfo = (int*)sp; sp += (size_t)nb16 * 4;
+  int* sIdx = (int*)sp;
+  double *sx = sPt, *sy = sPt + T, *sz = sPt + 2 * T, *sw = sPt + 3 * T;
+  double *sE = sPt + 4 * T, *sN = sPt + 5 * T;
+  double *sA = sPt + 8 * T, *sG0 = sPt + 9 * T, *sG1 = sPt + 10 * T, *sG2 = sPt + 11 * T;
+
+  // ---- per batch: metadata, zero padding rows, V^j block assignment ----
+  {
+    const int32_t* fidx = a.bfidx + b.f_off;
+    const int32_t* finfo = a.bfinfo + b.f_off;
+    for (int k = tid; k < ns; k += kBatchThreads) {
+      ShellRec r = a.shells[a.bshells[b.sh_off + k]];
+      r._pad = a.bsfoff[b.sh_off + k];
+      sSh[k] = r;
+    }
+    for (int f = tid; f < nb16; f += kBatchThreads) {
+      sIdx[f] = f < nb ? fidx[f] : 0;
+      sInfo[f] = f < nb ? finfo[f] : 0;
+    }
+    for (int e = tid; e < (nb16 - nb) * LD; e += kBatchThreads) {
+      sPhi[(size_t)nb * LD + e] = 0.0;
+      if (GGA) sZ[(size_t)nb * LD + e] = 0.0;
+    }
+  }
+  int blk_m[ROUNDS], blk_n[ROUNDS];
+  double V[ROUNDS][2][2][2];
 #pragma unroll
-  for (int u = 0; u < 4; ++u) {
-    const int mu = it.tm * 32 + u * 8 + g4;
-    if (mu >= b.nb) continue;
-    const size_t row = (size_t)fidx[mu] * a.nbasis;
+  for (int r = 0; r < ROUNDS; ++r) {
+    const int q = warp + 16 * r;
+    int bm = (int)((sqrtf(8.0f * q + 1.0f) - 1.0f) * 0.5f);
+    while ((bm + 1) * (bm + 2) / 2 <= q) ++bm;
+    while (bm * (bm + 1) / 2 > q) --bm;
+    blk_m[r] = q < nblocks ? bm : -1;
+    blk_n[r] = q - bm * (bm + 1) / 2;
 #pragma unroll
-    for (int v = 0; v < 4; ++v)
+    for (int u = 0; u < 2; ++u)
 #pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        const int nu = it.tn * 32 + v * 8 + t4 * 2 + h;
-        if (nu <= mu && nu < b.nb) {
-          const size_t o = row + fidx[nu];
-          fixed_add(a.vhi + o, a.vlo + o, C[u][v][h]);
+      for (int v = 0; v < 2; ++v) V[r][u][v][0] = V[r][u][v][1] = 0.0;
+  }
+  const double* __restrict__ ppk = a.ppk + b.ppk_off;
+  const int wp = warp % Cfg::WP, wm = warp / Cfg::WP;
+  double Eacc = 0.0, Nacc = 0.0;
+
+  for (int t0 = 0; t0 < b.nq; t0 += T) {
+    const int npt = min(T, b.nq - t0);         // valid points in this tile
+    __syncthreads();                           // previous tile's readers of sPhi / sZ / sPt are done
+    if (tid < T) {
+      const int li = min(tid, npt - 1);
+      const int64_t gi = (int64_t)b.pt_off + t0 + li;
+      sx[tid] = a.px[gi]; sy[tid] = a.py[gi]; sz[tid] = a.pz[gi];
+      sw[tid] = tid < npt ? a.w[gi] : 0.0;
+    }
+    __syncthreads();
+
+    // ---- 1. collocation (Eq. (7); same shell across a warp) ----
+    for (int e = tid; e < ns * T; e += kBatchThreads) {
+      const int slot = e / T, i = e - slot * T;
+      const ShellRec sh = sSh[slot];
+      const double dx = sx[i] - sh.x, dy = sy[i] - sh.y, dz = sz[i] - sh.z;
+      const double r2 = dx * dx + dy * dy + dz * dz;
+      double R0 = 0.0, R1 = 0.0;
+      for (int k = 0; k < sh.nprim; ++k) {
+        const double al = __ldg(a.exps + sh.prim_off + k);
+        const double arg = al * r2;
+        if (arg < 746.0) {                     // beyond, exp() underflows to exactly 0: skipping is bit-identical
+          const double ev = __ldg(a.coefs + sh.prim_off + k) * exp(-arg);
+          R0 += ev;
+          R1 = fma(-2.0 * al, ev, R1);
         }
       }
+      if (GGA) *reinterpret_cast<double2*>(sR + ((size_t)slot * T + i) * 2) = make_double2(R0, R1);
+      double* dst = sPhi + (size_t)sh._pad * LD + i;
+      if (sh.L == 0) {
+        dst[0] = R0;
+      } else if (sh.L == 1) {
+        dst[0] = dx * R0; dst[LD] = dy * R0; dst[2 * LD] = dz * R0;
+      } else {
+        const double xr = dx * R0, yr = dy * R0;
+        dst[0] = dx * xr; dst[LD] = dy * xr; dst[2 * LD] = dz * xr;
+        dst[3 * LD] = dy * yr; dst[4 * LD] = dz * yr; dst[5 * LD] = dz * dz * R0;
+      }
+    }
+    __syncthreads();
+
+    // ---- 2. X^T = Phi^T P^j and the density reductions ----
+    {
+      double C[2][NTW][2];
+#pragma unroll
+      for (int u = 0; u < 2; ++u)
+#pragma unroll
+        for (int v = 0; v < NTW; ++v) C[u][v][0] = C[u][v][1] = 0.0;
+      const double* Ap = sPhi + (size_t)t4 * LD + wp * 16 + g4;
+      const double* Bp = ppk + (size_t)wm * 32 + lane;
+#pragma unroll 2
+      for (int ks = 0; ks < nks; ++ks) {
+        const double A0 = Ap[0], A1 = Ap[8];
+#pragma unroll
+        for (int v = 0; v < NTW; ++v) {
+          if (wm + v * Cfg::WM < ntile) {
+            const double Bv = __ldg(Bp + (size_t)v * Cfg::WM * 32);
+            dmma884(C[0][v][0], C[0][v][1], A0, Bv);
+            dmma884(C[1][v][0], C[1][v][1], A1, Bv);
+          }
+        }
+        Ap += 4 * LD;
+        Bp += (size_t)ntile * 32;
+      }
+      // epilogue: Eqs. (13),(14)
+      double rho_acc[2] = {0.0, 0.0}, gx_acc[2] = {0.0, 0.0}, gy_acc[2] = {0.0, 0.0}, gz_acc[2] = {0.0, 0.0};
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const int i = wp * 16 + u * 8 + g4;
+        const double xi = sx[i], yi = sy[i], zi = sz[i];
+#pragma unroll
+        for (int v = 0; v < NTW; ++v) {
+          if (wm + v * Cfg::WM < ntile) {
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+              const int mu = (wm + v * Cfg::WM) * 8 + t4 * 2 + h;
+              if (mu < nb) {
+                const double X = C[u][v][h];
+                rho_acc[u] = fma(sPhi[(size_t)mu * LD + i], X, rho_acc[u]);
+                if (GGA) {
+                  const int info = sInfo[mu];
+                  const int slot = info >> 8;
+                  const double2 R = *reinterpret_cast<const double2*>(sR + ((size_t)slot * T + i) * 2);
+                  double gx, gy, gz;
+                  grad_cart(info, xi - sSh[slot].x, yi - sSh[slot].y, zi - sSh[slot].z, R.x, R.y, gx, gy, gz);
+                  gx_acc[u] = fma(gx, X, gx_acc[u]);
+                  gy_acc[u] = fma(gy, X, gy_acc[u]);
+                  gz_acc[u] = fma(gz, X, gz_acc[u]);
+                }
+              }
+            }
+          }
+        }
+      }
+      // reduce over the 4 lanes sharing a point, then over the WM warps (fixed order => deterministic)
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+#pragma unroll
+        for (int o = 1; o <= 2; o <<= 1) {
+          rho_acc[u] += __shfl_xor_sync(0xffffffffu, rho_acc[u], o);
+          if (GGA) {
+            gx_acc[u] += __shfl_xor_sync(0xffffffffu, gx_acc[u], o);
+            gy_acc[u] += __shfl_xor_sync(0xffffffffu, gy_acc[u], o);
+            gz_acc[u] += __shfl_xor_sync(0xffffffffu, gz_acc[u], o);
+          }
+        }
+        if (t4 == 0) {
+          const int i = wp * 16 + u * 8 + g4;
+          sRed[(size_t)(wm * 4 + 0) * T + i] = rho_acc[u];
+          if (GGA) {
+            sRed[(size_t)(wm * 4 + 1) * T + i] = gx_acc[u];
+            sRed[(size_t)(wm * 4 + 2) * T + i] = gy_acc[u];
+            sRed[(size_t)(wm * 4 + 3) * T + i] = gz_acc[u];
+          }
+        }
+      }
+    }
+    __syncthreads();
+
+    // ---- 3. functional (Eq. (19)), E and N_el partials (Eq. (16)) ----
+    if (tid < T) {
+      double rho = 0.0, gx = 0.0, gy = 0.0, gz = 0.0;
+      for (int q = 0; q < Cfg::WM; ++q) {
+        rho += sRed[(size_t)(q * 4 + 0) * T + tid];
+        if (GGA) {
+          gx += sRed[(size_t)(q * 4 + 1) * T + tid];
+          gy += sRed[(size_t)(q * 4 + 2) * T + tid];
+          gz += sRed[(size_t)(q * 4 + 3) * T + tid];
+        }
+      }
+      gx *= 2.0; gy *= 2.0; gz *= 2.0;
+      const double sigma = gx * gx + gy * gy + gz * gz;
+      const double wi = sw[tid];
+      double f, vr, vs;
+      xc_point<GGA>(rho, sigma, a.rho_tol, f, vr, vs);
+      sA[tid] = GGA ? 0.5 * wi * vr : wi * vr;   // LDA: V^j = sum_i (w v_rho)_i Phi_mu,i Phi_nu,i
+      const double gs = 2.0 * wi * vs;
+      sG0[tid] = gs * gx; sG1[tid] = gs * gy; sG2[tid] = gs * gz;
+      if (tid < npt && a.rho_out) {
+        const int64_t gi = (int64_t)b.pt_off + t0 + tid;
+        a.rho_out[gi] = rho;
+        if (a.grho_out) { a.grho_out[3 * gi] = gx; a.grho_out[3 * gi + 1] = gy; a.grho_out[3 * gi + 2] = gz; }
+      }
+      double e = wi * f, n = wi * rho;
+#pragma unroll
+      for (int o = 16; o >= 1; o >>= 1) {
+        e += __shfl_xor_sync(0xffffffffu, e, o);
+        n += __shfl_xor_sync(0xffffffffu, n, o);
+      }
+      if (lane == 0) { sE[warp] = e; sN[warp] = n; }
+    }
+    __syncthreads();
+    if (tid == 0) {
+      for (int q = 0; q < T / 32; ++q) { Eacc += sE[q]; Nacc += sN[q]; }
+    }
+
+    // ---- 4. GGA: Z (Eq. (20)) ----
+    if (GGA) {
+      for (int e = tid; e < nb * T; e += kBatchThreads) {
+        const int mu = e / T, i = e - mu * T;
+        const int info = sInfo[mu];
+        const int slot = info >> 8;
+        const double2 R = *reinterpret_cast<const double2*>(sR + ((size_t)slot * T + i) * 2);
+        double gx, gy, gz;
+        grad_cart(info, sx[i] - sSh[slot].x, sy[i] - sSh[slot].y, sz[i] - sSh[slot].z, R.x, R.y, gx, gy, gz);
+        sZ[(size_t)mu * LD + i] = fma(sG0[i], gx, fma(sG1[i], gy, fma(sG2[i], gz, sA[i] * sPhi[(size_t)mu * LD + i])));
+      }
+      __syncthreads();
+    }
+
+    // ---- 5. V^j += Z Phi^T + Phi Z^T (lower-triangle 16x16 blocks; Eq. (18)) ----
+#pragma unroll 2
+    for (int kk = 0; kk < T / 4; ++kk) {
+      const int i = kk * 4 + t4;
+      const double ai = GGA ? 0.0 : sA[i];
+#pragma unroll
+      for (int r = 0; r < ROUNDS; ++r) {
+        if (blk_m[r] >= 0) {
+          const double* pm = sPhi + (size_t)(blk_m[r] * 16 + g4) * LD + i;
+          const double* pn = sPhi + (size_t)(blk_n[r] * 16 + g4) * LD + i;
+          const bool diag = blk_m[r] == blk_n[r];
+          if (GGA) {
+            const double* zm = sZ + (size_t)(blk_m[r] * 16 + g4) * LD + i;
+            const double* zn = sZ + (size_t)(blk_n[r] * 16 + g4) * LD + i;
+            const double Pm0 = pm[0], Pm1 = pm[8 * LD], Zm0 = zm[0], Zm1 = zm[8 * LD];
+            const double Pn0 = pn[0], Pn1 = pn[8 * LD], Zn0 = zn[0], Zn1 = zn[8 * LD];
+            dmma884(V[r][0][0][0], V[r][0][0][1], Zm0, Pn0); dmma884(V[r][0][0][0], V[r][0][0][1], Pm0, Zn0);
+            dmma884(V[r][1][0][0], V[r][1][0][1], Zm1, Pn0); dmma884(V[r][1][0][0], V[r][1][0][1], Pm1, Zn0);
+            dmma884(V[r][1][1][0], V[r][1][1][1], Zm1, Pn1); dmma884(V[r][1][1][0], V[r][1][1][1], Pm1, Zn1);
+            if (!diag) { dmma884(V[r][0][1][0], V[r][0][1][1], Zm0, Pn1); dmma884(V[r][0][1][0], V[r][0][1][1], Pm0, Zn1); }
+          } else {
+            const double Pm0 = pm[0], Pm1 = pm[8 * LD];
+            const double Pn0 = pn[0], Pn1 = pn[8 * LD];
+            const double Zm0 = ai * Pm0, Zm1 = ai * Pm1;
+            dmma884(V[r][0][0][0], V[r][0][0][1], Zm0, Pn0);
+            dmma884(V[r][1][0][0], V[r][1][0][1], Zm1, Pn0);
+            dmma884(V[r][1][1][0], V[r][1][1][1], Zm1, Pn1);
+            if (!diag) dmma884(V[r][0][1][0], V[r][0][1][1], Zm0, Pn1);
+          }
+        }
+      }
+    }
+  }
+
+  // ---- 6. increment of V (Eq. (17)), lower triangle; global indices ascend with local ones ----
+  if (tid == 0) { a.Epart[bidx] = Eacc; a.Npart[bidx] = Nacc; }
+#pragma unroll
+  for (int r = 0; r < ROUNDS; ++r) {
+    if (blk_m[r] < 0) continue;
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+      const int mu = blk_m[r] * 16 + u * 8 + g4;
+      if (mu >= nb) continue;
+      const size_t row = (size_t)sIdx[mu] * a.nbasis;
+#pragma unroll
+      for (int v = 0; v < 2; ++v)
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          const int nu = blk_n[r] * 16 + v * 8 + t4 * 2 + h;
+          if (nu <= mu) {
+            const size_t o = row + sIdx[nu];
+            fixed_add(a.vhi + o, a.vlo + o, V[r][u][v][h]);
+          }
+        }
+    }
   }
 }
 
@@ -961,29 +944,28 @@ cudaError_t launch_functional(int kind, int64_t n, const double* rho, const doub
   return cudaGetLastError();
 }
 
-template <int T, bool GGA>
-static cudaError_t launch_density_t(const DensityArgs& a, const DensityItem* items, int nitems, int item0, size_t smem,
-                                    cudaStream_t st) {
-  if (nitems <= 0) return cudaSuccess;
-  cudaError_t e = cudaFuncSetAttribute(k_density<T, GGA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+cudaError_t launch_pack(const BatchArgs& a, const int32_t* batch_ids, int nbatches, cudaStream_t st) {
+  if (nbatches <= 0) return cudaSuccess;
+  k_pack_P<<<nbatches, 256, 0, st>>>(a, batch_ids);
+  return cudaGetLastError();
+}
+
+template <int T, bool GGA, int NTW, int ROUNDS>
+static cudaError_t launch_batch_t(const BatchArgs& a, const int32_t* batch_ids, int nbatches, size_t smem, cudaStream_t st) {
+  cudaError_t e = cudaFuncSetAttribute(k_xc_batch<T, GGA, NTW, ROUNDS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  k_density<T, GGA><<<nitems, kDensityThreads, smem, st>>>(a, items, item0);
+  k_xc_batch<T, GGA, NTW, ROUNDS><<<nbatches, kBatchThreads, smem, st>>>(a, batch_ids);
   return cudaGetLastError();
 }
 
-cudaError_t launch_density(int T, bool gga, const DensityArgs& a, const DensityItem* items, int nitems, int item0,
-                           size_t smem, cudaStream_t st) {
-  if (T == 64) return gga ? launch_density_t<64, true>(a, items, nitems, item0, smem, st)
-                          : launch_density_t<64, false>(a, items, nitems, item0, smem, st);
-  return gga ? launch_density_t<32, true>(a, items, nitems, item0, smem, st)
-             : launch_density_t<32, false>(a, items, nitems, item0, smem, st);
-}
-
-cudaError_t launch_potential(const PotArgs& a, cudaStream_t st) {
-  if (a.nitems <= 0) return cudaSuccess;
-  int wpb = kPotThreads / 32;
-  k_potential<<<(unsigned)((a.nitems + wpb - 1) / wpb), kPotThreads, 0, st>>>(a);
-  return cudaGetLastError();
+// cls 0: N_b^j <= kSmallNb, tiles of 64 points; cls 1: N_b^j <= kMaxNb, tiles of 32 points
+cudaError_t launch_batch(int cls, bool gga, const BatchArgs& a, const int32_t* batch_ids, int nbatches, size_t smem,
+                         cudaStream_t st) {
+  if (nbatches <= 0) return cudaSuccess;
+  if (cls == 0) return gga ? launch_batch_t<64, true, 4, 2>(a, batch_ids, nbatches, smem, st)
+                           : launch_batch_t<64, false, 4, 2>(a, batch_ids, nbatches, smem, st);
+  return gga ? launch_batch_t<32, true, 3, 5>(a, batch_ids, nbatches, smem, st)
+             : launch_batch_t<32, false, 3, 5>(a, batch_ids, nbatches, smem, st);
 }
 
 cudaError_t launch_finalize(int nbasis, const unsigned long long* vhi, const unsigned long long* vlo, double* V,

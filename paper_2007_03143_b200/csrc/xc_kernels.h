@@ -6,7 +6,7 @@
 
 namespace xcb {
 
-struct DensityArgs {
+struct BatchArgs {
   const BatchRec* batches;
   const int32_t* bshells;
   const int32_t* bsfoff;
@@ -17,9 +17,11 @@ struct DensityArgs {
   const double* coefs;
   const double* px; const double* py; const double* pz; const double* w;
   const double* P; int64_t ldp;
-  double* phi_scr; double* z_scr;
+  double* ppk;                         // packed P^j of every batch (DMMA B-fragment order)
   double* rho_out; double* grho_out;   // optional diagnostics (may be null)
-  double* Epart; double* Npart;        // one partial per work item
+  double* Epart; double* Npart;        // one partial per batch
+  unsigned long long* vhi; unsigned long long* vlo;   // fixed-point V accumulator (lower triangle)
+  int nbasis;
   double rho_tol;
 };
 
@@ -34,15 +36,6 @@ struct WeightArgs {
   double* w;
 };
 
-struct PotArgs {
-  const PotItem* items; int64_t nitems;
-  const BatchRec* batches;
-  const int32_t* bfidx;
-  const double* phi_scr; const double* z_scr;
-  unsigned long long* vhi; unsigned long long* vlo;
-  int nbasis;
-};
-
 cudaError_t launch_weights(int partition, int natoms, const double* atoms, const double* invR, const double* rnn,
                            int64_t npts, const double* px, const double* py, const double* pz, const double* wq,
                            const int32_t* parent, double* w, cudaStream_t st);
@@ -50,9 +43,9 @@ cudaError_t launch_weights_batched(int partition, const WeightArgs& a, const int
                                    int max_list, cudaStream_t st);
 cudaError_t launch_functional(int kind, int64_t n, const double* rho, const double* sigma, double rho_tol, double* f,
                               double* vr, double* vs, cudaStream_t st);
-cudaError_t launch_density(int T, bool gga, const DensityArgs& a, const DensityItem* items, int nitems, int item0,
-                           size_t smem, cudaStream_t st);
-cudaError_t launch_potential(const PotArgs& a, cudaStream_t st);
+cudaError_t launch_pack(const BatchArgs& a, const int32_t* batch_ids, int nbatches, cudaStream_t st);
+cudaError_t launch_batch(int cls, bool gga, const BatchArgs& a, const int32_t* batch_ids, int nbatches, size_t smem,
+                         cudaStream_t st);
 cudaError_t launch_finalize(int nbasis, const unsigned long long* vhi, const unsigned long long* vlo, double* V,
                             int64_t ldv, cudaStream_t st);
 cudaError_t launch_reduce(int64_t n, const double* ep, const double* np, double* out, cudaStream_t st);

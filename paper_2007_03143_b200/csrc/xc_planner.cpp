@@ -93,20 +93,17 @@ struct Leaf { int64_t begin, end; };
 
 }  // namespace
 
-size_t density_smem_bytes(int T, bool gga, int nb, int ns) {
-  // must mirror the shared-memory carve of k_density (xc_kernels.cu)
-  size_t nb4 = round_up(nb, 4);
-  size_t mb = std::min<size_t>(round_up(nb, T == 64 ? 32 : 64), kMuPass);
-  size_t npass = (nb + kMuPass - 1) / kMuPass;
+size_t batch_smem_bytes(int T, bool gga, int nb, int ns) {
+  // must mirror the shared-memory carve of k_xc_batch (xc_kernels.cu)
+  size_t nb16 = round_up(nb, 16);
   size_t b = 0;
-  b += nb4 * (T + 4) * 8;                       // Phi panel
+  b += nb16 * (T + 4) * 8;                       // Phi tile
+  if (gga) b += nb16 * (T + 4) * 8;              // Z tile
   if (gga) b += (size_t)ns * T * 2 * 8;          // R0/R1 panel
-  b += 2 * (size_t)kKC * (mb + 4) * 8;           // P stages
   b += (size_t)T * 8 * 12;                       // x,y,z,w, scratch, a,g0,g1,g2
   b += 1024 * 8;                                 // cross-warp reduction buffer
   b += (size_t)ns * sizeof(ShellRec);            // shell records
-  b += npass * kMuPass * 4 + nb4 * 4;            // padded function indices (mu side) + (nu side)
-  b += nb4 * 4;                                  // function info
+  b += nb16 * 4 * 2;                             // function info + global function index
   return b + 64;
 }
 
@@ -201,7 +198,7 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
   }
 
   // ---- per-batch shell screening (Alg. 1 on the tight bounding box), with re-splitting of batches whose
-  //      shell list exceeds the density kernel's shared-memory capacity ----
+  //      shell list exceeds the batch kernel's capacity (N_b^j <= kMaxNb, shared memory) ----
   std::vector<std::vector<int>> atom_shells(natoms);
   std::vector<double> atom_rmax(natoms, 0.0);
   for (int s = 0; s < nshells; ++s) {
@@ -232,7 +229,7 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     std::vector<Leaf> L2; std::vector<std::vector<int32_t>> S2; std::vector<int> N2;
     bool any = false;
     for (size_t j = 0; j < leaves.size(); ++j)
-      if (density_smem_bytes(32, gga, nbs[j], (int)lists[j].size()) > kSmemLimit) { any = true; break; }
+      if (nbs[j] > kMaxNb || batch_smem_bytes(32, gga, nbs[j], (int)lists[j].size()) > kSmemLimit) { any = true; break; }
     if (any) {
       for (size_t j = 0; j < leaves.size(); ++j) {
         std::vector<Leaf> st{leaves[j]};
@@ -242,8 +239,8 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
           std::vector<int32_t> sl; int nb;
           if (first) { sl = lists[j]; nb = nbs[j]; first = false; } else screen(cur, sl, nb);
           int64_t n = cur.end - cur.begin;
-          if (density_smem_bytes(32, gga, nb, (int)sl.size()) <= kSmemLimit) { L2.push_back(cur); S2.push_back(sl); N2.push_back(nb); continue; }
-          if (n <= 1) { err = "a single grid point sees more basis functions than the density kernel supports"; return XC_EUNSUPPORTED; }
+          if (nb <= kMaxNb && batch_smem_bytes(32, gga, nb, (int)sl.size()) <= kSmemLimit) { L2.push_back(cur); S2.push_back(sl); N2.push_back(nb); continue; }
+          if (n <= 1) { err = "a single grid point sees more basis functions than the batch kernel supports"; return XC_EUNSUPPORTED; }
           double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
           for (int64_t k = cur.begin; k < cur.end; ++k)
             for (int p = 0; p < 3; ++p) { double v = coord[p][idx[k]]; lo[p] = std::min(lo[p], v); hi[p] = std::max(hi[p], v); }
@@ -353,30 +350,16 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
   // ---- batch records, function lists, work items ----
   const int64_t nbatch = (int64_t)leaves.size();
   hp.batches.resize(nbatch);
-  int64_t sh_off = 0, f_off = 0, scr = 0, scr_total = 0;
-  // workspace cap per matrix (doubles): batches are processed in chunks that fit (analogue of Alg. 2 l.2.5-2.8)
-  int64_t cap = (int64_t)2 << 30;  // 2 Gi doubles = 16 GiB per matrix
-  if (const char* e = getenv("XC_B200_WORKSPACE_MB")) cap = std::max<int64_t>(1, atoll(e)) * (1 << 20) / 8;
-  hp.chunks.clear();
+  int64_t sh_off = 0, f_off = 0, ppk = 0;
   hp.watoms.clear(); hp.wbatch_small.clear(); hp.wbatch_large.clear(); hp.w_max_small = hp.w_max_large = 0;
   if (spec->partition != 0) { hp.watoms.resize(natoms); std::iota(hp.watoms.begin(), hp.watoms.end(), 0); }
-  HostPlan::Chunk ch{0, 0, 0, 0, 0, 0, 0, 0, 0};
-  std::vector<int64_t> chunk_of(nbatch);
   for (int64_t j = 0; j < nbatch; ++j) {
     BatchRec& b = hp.batches[j];
     b.pt_off = (int32_t)leaves[j].begin; b.nq = (int32_t)(leaves[j].end - leaves[j].begin);
-    b.nq_pad = (int32_t)round_up(b.nq, 4);
     b.sh_off = (int32_t)sh_off; b.ns = (int32_t)lists[j].size();
-    b.f_off = (int32_t)f_off; b.nb = nbs[j]; b.nb_pad8 = (int32_t)round_up(b.nb, 8);
-    int64_t need = (int64_t)b.nb_pad8 * b.nq_pad;
-    if (scr + need > cap && scr > 0) {  // close the chunk
-      ch.b1 = j; ch.scr = scr; hp.chunks.push_back(ch);
-      hp.scr_cap_doubles = std::max(hp.scr_cap_doubles, scr);
-      ch = HostPlan::Chunk{j, 0, 0, 0, 0, 0, 0, 0, 0};
-      scr = 0;
-    }
-    chunk_of[j] = (int64_t)hp.chunks.size();
-    b.scr_off = scr;
+    b.f_off = (int32_t)f_off; b.nb = nbs[j];
+    b.ppk_off = ppk;
+    ppk += round_up(b.nb, 4) * round_up(b.nb, 8);
     if (spec->partition == 0) {
       b.wa_off = (int64_t)hp.watoms.size(); b.wa_nB = wnB[j]; b.wa_nC = (int32_t)wlists[j].size();
       hp.watoms.insert(hp.watoms.end(), wlists[j].begin(), wlists[j].end());
@@ -389,12 +372,9 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
       else { hp.wbatch_large.push_back((int32_t)j); hp.w_max_large = std::max(hp.w_max_large, len); }
     }
     sh_off += b.ns; f_off += b.nb;
-    scr += need; scr_total += need;
     if (sh_off >= ((int64_t)1 << 31) || f_off >= ((int64_t)1 << 31)) { err = "batch lists exceed 2^31 entries"; return XC_EUNSUPPORTED; }
   }
-  ch.b1 = nbatch; ch.scr = scr; hp.chunks.push_back(ch);
-  hp.scr_cap_doubles = std::max(hp.scr_cap_doubles, scr);
-  hp.scr_doubles = scr_total;
+  hp.ppk_doubles = ppk;
   hp.bshells.resize(sh_off); hp.bsfoff.resize(sh_off); hp.bfidx.resize(f_off); hp.bfinfo.resize(f_off);
 #pragma omp parallel for schedule(dynamic, 64)
   for (int64_t j = 0; j < nbatch; ++j) {
@@ -413,29 +393,26 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
         }
     }
   }
-  hp.sum_nbnq = hp.sum_nb2 = hp.flops = 0; hp.max_nb = hp.max_ns = 0; hp.smem64 = hp.smem32 = 0;
+  hp.sum_nbnq = hp.sum_nb2 = hp.flops = 0; hp.max_nb = hp.max_ns = 0; hp.smem_small = hp.smem_large = 0;
+  hp.ids_small.clear(); hp.ids_large.clear();
   for (int64_t j = 0; j < nbatch; ++j) {
     const BatchRec& b = hp.batches[j];
     hp.sum_nbnq += (double)b.nb * b.nq; hp.sum_nb2 += (double)b.nb * b.nb; hp.flops += 4.0 * b.nb * (double)b.nb * b.nq;
     hp.max_nb = std::max(hp.max_nb, b.nb); hp.max_ns = std::max(hp.max_ns, b.ns);
     if (b.nb == 0) continue;  // nothing to integrate: rho = 0 on every point
-    size_t s64 = density_smem_bytes(64, gga, b.nb, b.ns);
-    if (s64 <= kSmemLimit) {
-      hp.smem64 = std::max(hp.smem64, s64);
-      for (int t = 0; t < b.nq; t += 64) hp.items64.push_back({(int32_t)j, t});
+    size_t s64 = batch_smem_bytes(64, gga, b.nb, b.ns);
+    if (b.nb <= kSmallNb && s64 <= kSmemLimit) {
+      hp.smem_small = std::max(hp.smem_small, s64);
+      hp.ids_small.push_back((int32_t)j);
     } else {
-      hp.smem32 = std::max(hp.smem32, density_smem_bytes(32, gga, b.nb, b.ns));
-      for (int t = 0; t < b.nq; t += 32) hp.items32.push_back({(int32_t)j, t});
-    }
-    int nt = (b.nb + 31) / 32;
-    int nparts = (b.nq_pad + kPotKPart - 1) / kPotKPart;
-    for (int kp = 0; kp < nparts; ++kp) {
-      // equalised part boundaries, multiples of 4
-      int k0 = (int)((int64_t)b.nq_pad / 4 * kp / nparts) * 4, k1 = (int)((int64_t)b.nq_pad / 4 * (kp + 1) / nparts) * 4;
-      for (int tm = 0; tm < nt; ++tm)
-        for (int tn = 0; tn <= tm; ++tn) hp.pot_items.push_back({(int32_t)j, (int16_t)tm, (int16_t)tn, k0, k1});
+      hp.smem_large = std::max(hp.smem_large, batch_smem_bytes(32, gga, b.nb, b.ns));
+      hp.ids_large.push_back((int32_t)j);
     }
   }
+  // heaviest batches first: the tail of each launch is made of cheap CTAs
+  auto cost = [&](int32_t j) { const BatchRec& b = hp.batches[j]; return (double)b.nb * b.nb * b.nq + 200.0 * b.ns * b.nq; };
+  std::stable_sort(hp.ids_small.begin(), hp.ids_small.end(), [&](int32_t x, int32_t y) { return cost(x) > cost(y); });
+  std::stable_sort(hp.ids_large.begin(), hp.ids_large.end(), [&](int32_t x, int32_t y) { return cost(x) > cost(y); });
   // warps per CTA of the large-list weights launch: per-warp distance rows must fit in shared memory
   hp.w_warps_large = 8;
   if (spec->partition == 0 && (size_t)hp.w_max_large * 36 + 512 * 30 + 2048 * 4 + 64 > kSmemLimit) {
@@ -444,15 +421,6 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
   while (spec->partition != 0 && hp.w_warps_large > 1 && weights_smem_bytes(hp.w_max_large, hp.w_warps_large) > kSmemLimit) hp.w_warps_large >>= 1;
   if (spec->partition != 0 && weights_smem_bytes(hp.w_max_large, hp.w_warps_large) > kSmemLimit) {
     err = "too many atoms inside the SSF support of one batch for the weights kernel"; return XC_EUNSUPPORTED;
-  }
-  // work-item ranges per chunk (lists are in batch order)
-  {
-    size_t i64 = 0, i32 = 0, ip = 0;
-    for (auto& c : hp.chunks) {
-      c.i64_0 = (int64_t)i64; while (i64 < hp.items64.size() && hp.items64[i64].batch < c.b1) ++i64; c.i64_1 = (int64_t)i64;
-      c.i32_0 = (int64_t)i32; while (i32 < hp.items32.size() && hp.items32[i32].batch < c.b1) ++i32; c.i32_1 = (int64_t)i32;
-      c.p0 = (int64_t)ip; while (ip < hp.pot_items.size() && hp.pot_items[ip].batch < c.b1) ++ip; c.p1 = (int64_t)ip;
-    }
   }
   return XC_OK;
 }
