@@ -132,6 +132,13 @@ int xc_partition_weights(const xc_atom* atoms /*[host]*/, int32_t natoms, int32_
 int xc_functional(int32_t functional, int64_t n, const double* drho, const double* dsigma, double rho_tol,
                   double* df, double* dvrho, double* dvsigma, void* cuda_stream);
 
+/* FP64 pipe microbenchmark of `device` (no memory traffic, register-resident chains; CUDA events, best of `reps`
+ * launches): kind 0 = DFMA chains, 1 = DMMA (mma.sync m8n8k4 f64, the instruction of the batch kernel's contractions).
+ * MEASURED_PEAKS.json has no FP64 entry, so bench.py measures the denominator of the FP64 roofline with this call
+ * (SURVEY.md 8(d) "FP64 peak ... must be measured on the box").  tflops [host] out; sm_clock_mhz_est [host, may be
+ * NULL] = the SM clock implied by 64 FP64 FMA/clk/SM.  Errors: XC_EINVAL, XC_ECUDA, XC_ENOMEM. */
+int xc_measure_fp64_peak(int32_t kind, int32_t device, int32_t reps, double* tflops, double* sm_clock_mhz_est);
+
 const char* xc_strerror(int code);
 const char* xc_last_error(void);
 

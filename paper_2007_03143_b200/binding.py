@@ -63,6 +63,7 @@ def _load():
                                  C.POINTER(XcGridSpec), C.c_int32, vp, C.c_int64, vp, C.c_int64, dp, dp, vp]
     lib.xc_partition_weights.argtypes = [C.POINTER(XcAtom), C.c_int32, C.c_int32, C.c_int64, vp, vp, vp, vp, vp, vp, vp]
     lib.xc_functional.argtypes = [C.c_int32, C.c_int64, vp, vp, C.c_double, vp, vp, vp, vp]
+    lib.xc_measure_fp64_peak.argtypes = [C.c_int32, C.c_int32, C.c_int32, dp, dp]
     for name in EXPORTED:
         getattr(lib, name)  # fail loudly if a declared symbol is missing
     return lib
@@ -70,7 +71,7 @@ def _load():
 
 EXPORTED = ["xc_plan_create", "xc_plan_info", "xc_plan_export", "xc_eval", "xc_eval_host", "xc_eval_diagnostics",
             "xc_eval_timings", "xc_plan_stats", "xc_plan_destroy", "xc_integrate", "xc_partition_weights",
-            "xc_functional", "xc_strerror", "xc_last_error"]
+            "xc_functional", "xc_measure_fp64_peak", "xc_strerror", "xc_last_error"]
 
 _lib = _load()
 
@@ -261,3 +262,10 @@ def functional(kind, rho, sigma, rho_tol=1e-15, stream=None):
                               C.c_void_p(f.data_ptr()), C.c_void_p(vr.data_ptr()), C.c_void_p(vs.data_ptr()),
                               _stream_ptr(stream)))
     return f, vr, vs
+
+
+def measure_fp64_peak(kind=1, device=0, reps=5):
+    """FP64 pipe rate of `device` in TFLOP/s (kind 0 = DFMA, 1 = DMMA) and the SM clock it implies (MHz)."""
+    t, c = C.c_double(), C.c_double()
+    _check(_lib.xc_measure_fp64_peak(kind, device, reps, C.byref(t), C.byref(c)))
+    return t.value, c.value
