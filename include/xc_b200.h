@@ -112,8 +112,10 @@ int xc_eval_diagnostics(xc_plan* plan, double* w, double* rho, double* grad_rho,
 int xc_eval_timings(const xc_plan* plan, float ms[5], int32_t* launches);
 
 /* Algorithmic sizes of the plan used by the roofline report: [0] sum_j N_b^j N_q^j (function-points),
- * [1] sum_j (N_b^j)^2, [2] sum_j 4 (N_b^j)^2 N_q^j, [3] max N_b^j, [4] mean N_q^j, [5] bytes of the packed-P^j buffer. */
-int xc_plan_stats(const xc_plan* plan, double stats[6]);
+ * [1] sum_j (N_b^j)^2, [2] sum_j 4 (N_b^j)^2 N_q^j, [3] max N_b^j, [4] mean N_q^j, [5] bytes of the packed-P^j buffer,
+ * [6] mean and [7] max length of the per-batch partner-atom lists of step (a), [8] mean and [9] max length of the
+ * owner-atom lists, [10] max |S_j| (shells), [11] reserved (0). */
+int xc_plan_stats(const xc_plan* plan, double stats[12]);
 
 int xc_plan_destroy(xc_plan* plan);
 

@@ -148,9 +148,11 @@ class Plan:
                    spec, device)
 
     def stats(self):
-        s = (C.c_double * 6)()
+        s = (C.c_double * 12)()
         _check(_lib.xc_plan_stats(self._h, s))
-        return dict(sum_nb_nq=s[0], sum_nb2=s[1], flops=s[2], max_nb=int(s[3]), mean_nq=s[4], workspace_bytes=s[5])
+        return dict(sum_nb_nq=s[0], sum_nb2=s[1], flops=s[2], max_nb=int(s[3]), mean_nq=s[4], workspace_bytes=s[5],
+                    w_partners_mean=s[6], w_partners_max=int(s[7]), w_owners_mean=s[8], w_owners_max=int(s[9]),
+                    max_ns=int(s[10]))
 
     def export(self) -> PlanExport:
         n, nb = self.n_points, self.n_batches

@@ -175,11 +175,15 @@ int xc_plan_info(const xc_plan* p, int64_t* n_points, int64_t* n_batches, int32_
   return XC_OK;
 }
 
-int xc_plan_stats(const xc_plan* p, double stats[6]) {
+int xc_plan_stats(const xc_plan* p, double stats[12]) {
   if (!p || !stats) return fail(XC_EINVAL, "null argument");
   stats[0] = p->hp.sum_nbnq; stats[1] = p->hp.sum_nb2; stats[2] = p->hp.flops; stats[3] = p->hp.max_nb;
   stats[4] = p->hp.batches.empty() ? 0.0 : (double)p->hp.npts / (double)p->hp.batches.size();
   stats[5] = 8.0 * (double)p->hp.ppk_doubles;
+  double snC = 0, snB = 0, mnC = 0, mnB = 0;
+  for (const BatchRec& b : p->hp.batches) { snC += b.wa_nC; snB += b.wa_nB; mnC = std::max(mnC, (double)b.wa_nC); mnB = std::max(mnB, (double)b.wa_nB); }
+  const double nbt = std::max<double>(1.0, (double)p->hp.batches.size());
+  stats[6] = snC / nbt; stats[7] = mnC; stats[8] = snB / nbt; stats[9] = mnB; stats[10] = p->hp.max_ns; stats[11] = 0.0;
   return XC_OK;
 }
 

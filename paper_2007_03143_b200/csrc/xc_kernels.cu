@@ -315,188 +315,288 @@ __global__ void __launch_bounds__(kWeightThreads) k_weights_batched(WeightArgs a
 }
 
 // ------------------------------------------------------------------------------------------------
-// step (a), hot path for SSF: one CTA per batch, one WARP per point, the lanes split the atom list.
-// Exact pruning only; the batch's atom list (planner) is sorted by
-// dmin(atom, batch box) <= r_atom, so every scan stops as soon as dmin reaches its bound, and all control
-// flow is warp-uniform:
-//   0. r_A < (1-a)/2 R_nn(A)  =>  w = w^q.  The other points of the batch are compacted (in order); a batch
-//      of core points never touches the atom list.
-//   1. nearest atom m, r_min                 (32 atoms per step, scan while dmin < r_min)
+// step (a), hot path for SSF: one CTA (16 warps) per batch, one WARP per non-trivial point, the lanes split the
+// atoms.  Exact pruning only.  The batch's atom list (planner) is sorted by dmin(atom, batch box)
+// <= r_atom, so every scan stops as soon as dmin reaches its bound, and all control flow is warp-uniform.
+//
+// Per batch (once): the first kLcap list atoms (x, y, z, dmin) and the dmin of every chunk of 32 in shared memory;
+//   a table 1 / (a R_BC) for the first kTabB (owner) x kTabC (partner) list positions.
+// Per point (one warp, points handed out dynamically):
+//   0. r_A < (1-a)/2 R_nn(A)  =>  w = w^q (decided per thread before; the other points are compacted in order).
+//   1. nearest atom m, r_min (32 atoms per step, scan while dmin < r_min).  Every distance r_C computed on the way
+//      is kept in a per-warp shared-memory row (filled lazily, chunk by chunk) and reused by all cell products.
 //   2. P_A first: P_A = 0 => w = 0 and the point is done.
-//   3. owner candidates B, 32 per step (scan while dmin < kappa r_min): r_B < kappa r_min and mu_Bm < a;
-//      each surviving candidate's cell product P_B is then evaluated by the whole warp.
-//   A cell product scans the partners C, 32 per step (while dmin < kappa r_B): s(mu_BC) = 1 exactly when
-//   r_C >= r_B + a R_BC (tested on squares, no sqrt), and the scan stops as soon as one mu_BC >= a (P_B = 0).
+//   3. owner candidates B, 32 per step, one per lane (scan while dmin < kappa r_min): r_B < kappa r_min, and not
+//      already zeroed by one of the kPre atoms nearest to the batch box or by m (mu_BC >= a <=> r_B - r_C >= a R_BC);
+//      each survivor's cell product P_B is then evaluated by the whole warp.
+//   Cell product: partners C in chunks of 32 while dmin < kappa r_B (beyond, s(mu_BC) = 1 exactly); a chunk whose
+//   32 distances are all >= kappa r_B is skipped; mu_BC / a = (r_B - r_C) / (a R_BC) with 1 / (a R_BC) from the table
+//   or from the coordinates, clamped below at -1 (where the polynomial is exactly 1); the scan stops as soon as one
+//   mu_BC >= a (P_B = 0).  In the table path the factor s(0) = 1/2 of the pair (B, B) is multiplied in and undone by
+//   an exact factor 2.
 //   Lane products are combined by an xor butterfly (same value in every lane) and the owners are summed in
 //   list order, so w is bit-identical from run to run.
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ double ssf_cell_product(const double4* __restrict__ sAt, const int* __restrict__ sId, int nC, int lane,
-                                                   double x, double y, double z, double Bx, double By, double Bz, int Bid,
-                                                   double rB, double rB2) {
+constexpr int kSsfThreads = 512, kSsfWarps = kSsfThreads / 32;
+constexpr int kRcap = 256;                  // per-warp distance row: first kRcap list positions
+constexpr int kTabC = 320;                  // 1/(a R_BC) table: partners (list positions) per owner row
+constexpr int kMaxCh = 128;                 // chunk-start dmin values held in shared memory
+constexpr int kPre = 8;                     // partners used by the lane-parallel owner pre-filter
+constexpr size_t kSsfSmem = 112 * 1024;     // two CTAs per SM
+// shared-memory split (launch_weights_batched): lcap list atoms (28 B each) + fixed parts + tabB table rows
+constexpr size_t kSsfFixed = (size_t)kSsfWarps * kRcap * 8 + (size_t)kMaxCh * 8 + 512 * 2;
+constexpr int kSsfMaxLcap = (int)((kSsfSmem - kSsfFixed - (size_t)8 * kTabC * 8) / 28) / 32 * 32;
+
+struct SsfCtx {
+  const double* sX; const double* sY; const double* sZ; const int* sId; const double* sTab; const double* sDm; double* sRC;
+  const WeightArgs* a; const double* box; int64_t wa_off;
+  int nC, nch, lane, lcap, tabB;
+  double x, y, z;
+  int filled;     // list positions [0, filled) of sRC hold r_C of this point
+};
+
+__device__ __forceinline__ double ssf_poly(double zz) {   // s(mu) for zz = mu / a in [-1, 1]; exactly 1 at -1, 0 at +1
+  const double z2 = zz * zz;
+  return fma(-zz, fma(z2, fma(z2, fma(z2, -5.0 / 32.0, 21.0 / 32.0), -35.0 / 32.0), 35.0 / 32.0), 0.5);
+}
+
+__device__ __forceinline__ double ssf_dmin_box(double cx, double cy, double cz, const double* box) {
+  const double tx = cx < box[0] ? box[0] - cx : (cx > box[3] ? cx - box[3] : 0.0);
+  const double ty = cy < box[1] ? box[1] - cy : (cy > box[4] ? cy - box[4] : 0.0);
+  const double tz = cz < box[2] ? box[2] - cz : (cz > box[5] ? cz - box[5] : 0.0);
+  // a hair below the true distance: the early exits must never cut an atom that matters
+  return sqrt(tx * tx + ty * ty + tz * tz) * (1.0 - 1e-12) - 1e-12;
+}
+
+// coordinates of list entry c: shared memory for c < lcap, global beyond (systems with more atoms than fit)
+__device__ __forceinline__ void ssf_atom(const SsfCtx& s, int c, double& cx, double& cy, double& cz) {
+  if (c < s.lcap) { cx = s.sX[c]; cy = s.sY[c]; cz = s.sZ[c]; return; }
+  const int at = s.a->watoms[s.wa_off + c];
+  cx = s.a->atoms[3 * at]; cy = s.a->atoms[3 * at + 1]; cz = s.a->atoms[3 * at + 2];
+}
+__device__ __forceinline__ double ssf_chunk_dmin(const SsfCtx& s, int ch) {
+  if (ch < kMaxCh) return s.sDm[ch];
+  double cx, cy, cz;
+  ssf_atom(s, ch * 32, cx, cy, cz);
+  return ssf_dmin_box(cx, cy, cz, s.box);
+}
+// number of leading chunks whose first (smallest) dmin is below `bound`
+__device__ __forceinline__ int ssf_nscan(const SsfCtx& s, double bound) {
+  for (int base = 0; base < s.nch; base += 32) {
+    const int ch = base + s.lane;
+    const double v = ch < s.nch ? ssf_chunk_dmin(s, ch) : 1e300;
+    const unsigned m = __ballot_sync(0xffffffffu, v >= bound);
+    if (m) return base + __ffs(m) - 1;
+  }
+  return s.nch;
+}
+
+// r_C of this lane's list position c = c0 + lane (c0 warp-uniform); fills the warp's row on first touch
+__device__ __forceinline__ double ssf_dist(SsfCtx& s, int c0) {
+  const int c = c0 + s.lane;
+  if (c0 < s.filled) return s.sRC[c];
+  double r = 1e300;
+  if (c < s.nC) {
+    double cx, cy, cz;
+    ssf_atom(s, c, cx, cy, cz);
+    const double dx = s.x - cx, dy = s.y - cy, dz = s.z - cz;
+    r = sqrt(dx * dx + dy * dy + dz * dz);
+  }
+  if (c0 < kRcap && c0 == s.filled) { s.sRC[c] = r; s.filled = c0 + 32; __syncwarp(); }
+  return r;
+}
+
+// P_B = prod_C s(mu_BC).  bb = list position of B (warp-uniform, -1: not in the list), rB = r_B.
+__device__ __forceinline__ double ssf_cell_product(SsfCtx& s, int bb, double Bx, double By, double Bz, double rB) {
   const unsigned FULL = 0xffffffffu;
   const double kappa = (1.0 + 0.64) / (1.0 - 0.64);
-  const double krB = kappa * rB, f4 = (4.0 * 0.64 * 0.64) * rB2;
+  const double krB = kappa * rB;
+  const int nscan = ssf_nscan(s, krB);                     // every later C has r_C >= kappa r_B: factor 1
+  const bool tab = bb >= 0 && bb < s.tabB;
   double part = 1.0;
-  for (int c0 = 0; c0 < nC; c0 += 32) {
-    if (sAt[c0].w >= krB) break;                          // every later C has r_C >= kappa r_B: factor 1
-    const int c = c0 + lane;
-    bool dead = false;
-    if (c < nC) {
-      const double4 at = sAt[c];
-      if (at.w < krB && sId[c] != Bid) {
-        const double dx = x - at.x, dy = y - at.y, dz = z - at.z;
-        const double d2 = dx * dx + dy * dy + dz * dz;                 // r_C^2
-        const double ex = Bx - at.x, ey = By - at.y, ez = Bz - at.z;
-        const double R2 = ex * ex + ey * ey + ez * ez;                 // R_BC^2
-        // s(mu_BC) = 1 exactly  <=>  r_C >= r_B + a R_BC  <=>  t >= 0 and t^2 >= 4 a^2 r_B^2 R_BC^2,
-        // t = r_C^2 - r_B^2 - a^2 R_BC^2   (no square root)
-        const double t = d2 - rB2 - (0.64 * 0.64) * R2;
-        if (!(t >= 0.0 && t * t >= f4 * R2)) {
-          const double zz = (rB - sqrt(d2)) * rsqrt(R2) * (1.0 / 0.64);   // mu_BC / a
-          if (zz >= 1.0) {
-            dead = true;                                               // s = 0: P_B = 0
-          } else if (zz > -1.0) {
-            const double z2 = zz * zz;
-            part *= 0.5 - zz * (35.0 + z2 * (-35.0 + z2 * (21.0 - 5.0 * z2))) * (1.0 / 32.0);
-          }
-        }
+  for (int ch = 0; ch < nscan; ++ch) {
+    const int c0 = ch << 5, c = c0 + s.lane;
+    const double rC = ssf_dist(s, c0);
+    if (!__any_sync(FULL, rC < krB)) continue;             // 32 factors exactly 1
+    double zz;
+    if (tab && c0 < kTabC) {
+      zz = (rB - rC) * s.sTab[bb * kTabC + c];             // (B, B): 0, factor 1/2; c >= nC: r_C = 1e300, entry 1
+    } else {
+      zz = -1.0;                                           // factor exactly 1
+      if (c < s.nC && c != bb) {
+        double cx, cy, cz;
+        ssf_atom(s, c, cx, cy, cz);
+        const double ex = Bx - cx, ey = By - cy, ez = Bz - cz;
+        zz = (rB - rC) * (rsqrt(ex * ex + ey * ey + ez * ez) * (1.0 / 0.64));   // mu_BC / a
       }
     }
-    if (__any_sync(FULL, dead)) return 0.0;
+    if (__any_sync(FULL, zz >= 1.0)) return 0.0;           // s = 0: P_B = 0
+    zz = zz < -1.0 ? -1.0 : zz;
+    part *= ssf_poly(zz);
   }
 #pragma unroll
   for (int o = 16; o >= 1; o >>= 1) part *= __shfl_xor_sync(FULL, part, o);
+  // table path: the chunk of B itself is always visited (dmin_B <= r_B < kappa r_B) and contributed s(0) = 1/2
+  if (tab) part *= 2.0;
   return part;
 }
 
-__global__ void __launch_bounds__(kWeightThreads, 4) k_weights_ssf(WeightArgs a, const int32_t* __restrict__ batch_ids) {
+__global__ void __launch_bounds__(kSsfThreads, 2) k_weights_ssf(WeightArgs a, const int32_t* __restrict__ batch_ids, int lcap, int tabB) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  __shared__ int sCnt[2 * (kWeightThreads / 32)];
+  __shared__ int sCnt[kSsfWarps];
+  __shared__ int sNext;
   const unsigned FULL = 0xffffffffu;
   const int bid = batch_ids[blockIdx.x];
   const BatchRec b = a.batches[bid];
   const int nC = b.wa_nC, nB = b.wa_nB;
-  double4* sAt = (double4*)smem_raw;                     // x, y, z, dmin
-  int* sId = (int*)(sAt + nC);
-  short* sList = (short*)(sId + nC);                     // compacted non-trivial points of the batch (<= 512)
+  double* sX = (double*)smem_raw;                        // [lcap] x 3
+  double* sY = sX + lcap;
+  double* sZ = sY + lcap;
+  double* sRCall = sZ + lcap;                            // [kSsfWarps][kRcap]
+  double* sDm = sRCall + kSsfWarps * kRcap;              // [kMaxCh]
+  double* sTab = sDm + kMaxCh;                           // [tabB][kTabC]
+  int* sId = (int*)(sTab + tabB * kTabC);                // [lcap]
+  short* sList = (short*)(sId + lcap);                   // compacted non-trivial points of the batch (<= 512)
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const double aa = 0.64, kappa = (1.0 + aa) / (1.0 - aa);
+  const double* box = a.wbox + (size_t)6 * bid;
 
   // ---- 0. trivial points, ordered compaction of the others ----
-  int rank[2];
-  bool live[2];
-#pragma unroll
-  for (int r = 0; r < 2; ++r) {
-    const int p = r * kWeightThreads + threadIdx.x;
-    live[r] = false;
+  bool live = false;
+  {
+    const int p = threadIdx.x;
     if (p < b.nq) {
       const int64_t gi = (int64_t)b.pt_off + p;
       const int A = a.parent[gi];
       bool trivial = a.natoms == 1;
       if (!trivial) {
-        double dx = a.px[gi] - a.atoms[3 * A], dy = a.py[gi] - a.atoms[3 * A + 1], dz = a.pz[gi] - a.atoms[3 * A + 2];
+        const double dx = a.px[gi] - a.atoms[3 * A], dy = a.py[gi] - a.atoms[3 * A + 1], dz = a.pz[gi] - a.atoms[3 * A + 2];
         trivial = sqrt(dx * dx + dy * dy + dz * dz) < 0.5 * (1.0 - aa) * a.rnn[A];
       }
       if (trivial) a.w[gi] = a.wq[gi];
-      live[r] = !trivial;
+      live = !trivial;
     }
-    const unsigned mask = __ballot_sync(FULL, live[r]);
-    rank[r] = __popc(mask & ((1u << lane) - 1u));
-    if (lane == 0) sCnt[r * (kWeightThreads / 32) + warp] = __popc(mask);
   }
+  const unsigned lmask = __ballot_sync(FULL, live);
+  if (lane == 0) sCnt[warp] = __popc(lmask);
+  if (threadIdx.x == 0) sNext = kSsfWarps;
   __syncthreads();
-  int total = 0;
+  int total = 0, off = 0;
 #pragma unroll
-  for (int r = 0; r < 2; ++r) {
-    int off = 0;
-    for (int k = 0; k < 2 * (kWeightThreads / 32); ++k) {
-      if (k < r * (kWeightThreads / 32) + warp) off += sCnt[k];
-      if (r == 0) total += sCnt[k];
-    }
-    if (live[r]) sList[off + rank[r]] = (short)(r * kWeightThreads + threadIdx.x);
+  for (int k = 0; k < kSsfWarps; ++k) {
+    if (k < warp) off += sCnt[k];
+    total += sCnt[k];
   }
+  if (live) sList[off + __popc(lmask & ((1u << lane) - 1u))] = (short)threadIdx.x;
   if (total == 0) return;
-  {
-    const double* box = a.wbox + (size_t)6 * bid;
-    for (int c = threadIdx.x; c < nC; c += kWeightThreads) {
-      int at = a.watoms[b.wa_off + c];
-      double cx = a.atoms[3 * at], cy = a.atoms[3 * at + 1], cz = a.atoms[3 * at + 2];
-      double tx = cx < box[0] ? box[0] - cx : (cx > box[3] ? cx - box[3] : 0.0);
-      double ty = cy < box[1] ? box[1] - cy : (cy > box[4] ? cy - box[4] : 0.0);
-      double tz = cz < box[2] ? box[2] - cz : (cz > box[5] ? cz - box[5] : 0.0);
-      // a hair below the true distance: the early exits must never cut an atom that matters
-      sAt[c] = make_double4(cx, cy, cz, sqrt(tx * tx + ty * ty + tz * tz) * (1.0 - 1e-12) - 1e-12);
-      sId[c] = at;
-    }
+  const int nS = min(nC, lcap), nch = (nC + 31) >> 5;
+  for (int c = threadIdx.x; c < nS; c += kSsfThreads) {
+    const int at = a.watoms[b.wa_off + c];
+    const double cx = a.atoms[3 * at], cy = a.atoms[3 * at + 1], cz = a.atoms[3 * at + 2];
+    sX[c] = cx; sY[c] = cy; sZ[c] = cz;
+    sId[c] = at;
+    if ((c & 31) == 0 && (c >> 5) < kMaxCh) sDm[c >> 5] = ssf_dmin_box(cx, cy, cz, box);
+  }
+  for (int ch = (lcap >> 5) + threadIdx.x; ch < min(nch, kMaxCh); ch += kSsfThreads) {
+    const int at = a.watoms[b.wa_off + ch * 32];
+    sDm[ch] = ssf_dmin_box(a.atoms[3 * at], a.atoms[3 * at + 1], a.atoms[3 * at + 2], box);
   }
   __syncthreads();
+  if (total < 8) tabB = 0;                                 // too few points to pay for the table
+  {
+    const int tb = min(nS, tabB), tc = min((nC + 31) & ~31, kTabC);
+    for (int e = threadIdx.x; e < tb * tc; e += kSsfThreads) {
+      const int bb = e / tc, c = e - bb * tc;
+      double v = 1.0;                                      // neutral entry for c >= nC (r_C = 1e300 there)
+      if (c < nC) {
+        double cx, cy, cz;
+        if (c < lcap) { cx = sX[c]; cy = sY[c]; cz = sZ[c]; }
+        else { const int at = a.watoms[b.wa_off + c]; cx = a.atoms[3 * at]; cy = a.atoms[3 * at + 1]; cz = a.atoms[3 * at + 2]; }
+        const double ex = sX[bb] - cx, ey = sY[bb] - cy, ez = sZ[bb] - cz;
+        v = bb == c ? 0.0 : rsqrt(ex * ex + ey * ey + ez * ez) * (1.0 / 0.64);
+      }
+      sTab[bb * kTabC + c] = v;
+    }
+    tabB = tb;
+    __syncthreads();
+  }
 
-  for (int n = warp; n < total; n += kWeightThreads / 32) {
+  SsfCtx s;
+  s.sX = sX; s.sY = sY; s.sZ = sZ; s.sId = sId; s.sTab = sTab; s.sDm = sDm; s.sRC = sRCall + warp * kRcap; s.a = &a; s.box = box;
+  s.wa_off = b.wa_off; s.nC = nC; s.nch = nch; s.lane = lane; s.lcap = lcap; s.tabB = tabB;
+  for (int n = warp; n < total;) {
     const int64_t gi = (int64_t)b.pt_off + sList[n];
-    const double x = a.px[gi], y = a.py[gi], z = a.pz[gi];
+    s.x = a.px[gi]; s.y = a.py[gi]; s.z = a.pz[gi];
+    s.filled = 0;
     const int A = a.parent[gi];
+    __syncwarp();                                          // the previous point's readers of the row are done
     // ---- 1. nearest atom ----
-    double rmin2 = 1e300;
+    double rmin = 1e300;
     int im = 0;
     for (int c0 = 0; c0 < nC; c0 += 32) {
-      const double dm = sAt[c0].w;
-      if (dm > 0.0 && dm * dm >= rmin2) break;
-      const int c = c0 + lane;
-      double d2 = 1e300;
-      if (c < nC) { const double4 at = sAt[c]; const double dx = x - at.x, dy = y - at.y, dz = z - at.z; d2 = dx * dx + dy * dy + dz * dz; }
-      int ci = c;
-#pragma unroll
-      for (int o = 16; o >= 1; o >>= 1) {
-        const double od = __shfl_xor_sync(FULL, d2, o);
-        const int oi = __shfl_xor_sync(FULL, ci, o);
-        if (od < d2 || (od == d2 && oi < ci)) { d2 = od; ci = oi; }
-      }
-      if (d2 < rmin2) { rmin2 = d2; im = ci; }
+      if (ssf_chunk_dmin(s, c0 >> 5) >= rmin) break;
+      const double r = ssf_dist(s, c0);
+      // argmin over the lanes: r >= 0, so the bit patterns order like the values
+      const unsigned hi = (unsigned)__double2hiint(r);
+      const unsigned mhi = __reduce_min_sync(FULL, hi);
+      const unsigned lo = hi == mhi ? (unsigned)__double2loint(r) : 0xffffffffu;
+      const unsigned mlo = __reduce_min_sync(FULL, lo);
+      const double rm = __hiloint2double((int)mhi, (int)mlo);
+      if (rm < rmin) { rmin = rm; im = c0 + __ffs(__ballot_sync(FULL, hi == mhi && lo == mlo)) - 1; }
     }
-    const double rmin = sqrt(rmin2), own_lim = kappa * rmin, own_lim2 = own_lim * own_lim;
-    const double4 atm = sAt[im];
-    const int mid = sId[im];
+    const double own_lim = kappa * rmin;
     // ---- 2. the parent's cell product ----
     const double Ax = a.atoms[3 * A], Ay = a.atoms[3 * A + 1], Az = a.atoms[3 * A + 2];
-    double rA2;
-    { const double dx = x - Ax, dy = y - Ay, dz = z - Az; rA2 = dx * dx + dy * dy + dz * dz; }
-    const double rA = sqrt(rA2);
-    double PA = 0.0;
-    if (!(rA >= own_lim && rA > rmin)) PA = ssf_cell_product(sAt, sId, nC, lane, x, y, z, Ax, Ay, Az, A, rA, rA2);
+    double rA;
+    { const double dx = s.x - Ax, dy = s.y - Ay, dz = s.z - Az; rA = sqrt(dx * dx + dy * dy + dz * dz); }
     double result = 0.0;
-    if (PA != 0.0) {
-      // ---- 3. the other owners ----
-      double sum = PA;
-      for (int b0 = 0; b0 < nB; b0 += 32) {
-        if (sAt[b0].w >= own_lim) break;
-        const int bb = b0 + lane;
-        bool cand = false;
-        double4 at = make_double4(0.0, 0.0, 0.0, 0.0);
-        double d2 = 0.0;
-        int cid = -1;
-        if (bb < nB) {
-          at = sAt[bb]; cid = sId[bb];
-          const double dx = x - at.x, dy = y - at.y, dz = z - at.z;
-          d2 = dx * dx + dy * dy + dz * dz;
-          cand = at.w < own_lim && cid != A && d2 < own_lim2;          // else r_B >= kappa r_min: P_B = 0 exactly
-          if (cand && cid != mid) {                                    // mu_Bm >= a  =>  P_B = 0
-            const double ex = at.x - atm.x, ey = at.y - atm.y, ez = at.z - atm.z;
-            cand = (sqrt(d2) - rmin) * rsqrt(ex * ex + ey * ey + ez * ez) < aa;
+    if (!(rA >= own_lim && rA > rmin)) {
+      int ia = -1;                                         // list position of the parent
+      for (int c0 = 0; c0 < nC && ia < 0; c0 += 32) {
+        const int c = c0 + lane;
+        const unsigned m = __ballot_sync(FULL, c < nC && (c < lcap ? sId[c] : a.watoms[b.wa_off + c]) == A);
+        if (m) ia = c0 + __ffs(m) - 1;
+      }
+      const double PA = ssf_cell_product(s, ia, Ax, Ay, Az, rA);
+      if (PA != 0.0) {
+        // ---- 3. the other owners ----
+        double sum = PA;
+        double mx, my, mz;
+        ssf_atom(s, im, mx, my, mz);
+        const int nown = min(ssf_nscan(s, own_lim) << 5, nB);
+        for (int b0 = 0; b0 < nown; b0 += 32) {
+          const int bb = b0 + lane;
+          const double rB = ssf_dist(s, b0);
+          double bx = 0.0, by = 0.0, bz = 0.0;
+          bool cand = bb < nB && bb != ia && rB < own_lim;   // else r_B >= kappa r_min: P_B = 0 exactly
+          if (cand) ssf_atom(s, bb, bx, by, bz);
+          // pre-filter: mu_BC >= a for one of the first kPre list atoms or the nearest atom  =>  P_B = 0
+          const int npre = min(kPre, nC);
+          for (int k = 0; k < npre; ++k) {                   // positions < 32 of the row are always filled (scan 1)
+            const double u = rB - s.sRC[k];
+            const double ex = bx - sX[k], ey = by - sY[k], ez = bz - sZ[k];
+            if (k != bb && u > 0.0 && u * u >= (aa * aa) * (ex * ex + ey * ey + ez * ez)) cand = false;
+          }
+          if (im >= npre) {
+            const double u = rB - rmin;
+            const double ex = bx - mx, ey = by - my, ez = bz - mz;
+            if (im != bb && u > 0.0 && u * u >= (aa * aa) * (ex * ex + ey * ey + ez * ez)) cand = false;
+          }
+          unsigned mask = __ballot_sync(FULL, cand);
+          while (mask) {
+            const int src = __ffs(mask) - 1;
+            mask &= mask - 1;
+            const int bs = b0 + src;
+            double Bx, By, Bz;
+            ssf_atom(s, bs, Bx, By, Bz);
+            sum += ssf_cell_product(s, bs, Bx, By, Bz, __shfl_sync(FULL, rB, src));
           }
         }
-        unsigned mask = __ballot_sync(FULL, cand);
-        while (mask) {
-          const int src = __ffs(mask) - 1;
-          mask &= mask - 1;
-          const double Bx = __shfl_sync(FULL, at.x, src), By = __shfl_sync(FULL, at.y, src), Bz = __shfl_sync(FULL, at.z, src);
-          const double rB2 = __shfl_sync(FULL, d2, src);
-          const int Bid = __shfl_sync(FULL, cid, src);
-          sum += ssf_cell_product(sAt, sId, nC, lane, x, y, z, Bx, By, Bz, Bid, sqrt(rB2), rB2);
-        }
+        result = a.wq[gi] * PA / sum;
       }
-      result = a.wq[gi] * PA / sum;
     }
-    if (lane == 0) a.w[gi] = result;
+    if (lane == 0) { a.w[gi] = result; n = atomicAdd(&sNext, 1); }
+    n = __shfl_sync(FULL, n, 0);
   }
 }
 
@@ -925,10 +1025,12 @@ cudaError_t launch_weights_batched(int partition, const WeightArgs& a, const int
   size_t smem = weights_smem_bytes(max_list, nwarps);
   cudaError_t e;
   if (partition == 0) {
-    smem = (size_t)max_list * 36 + 1024 + 64;   // list: x,y,z,dmin,id; compacted point list
-    e = cudaFuncSetAttribute(k_weights_ssf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(smem, 1024));
+    // shared-memory split: the whole atom list if it fits (28 B per atom), the rest for rows of the 1/(a R_BC) table
+    const int lcap = std::min((max_list + 31) / 32 * 32, kSsfMaxLcap);
+    const int tabB = std::min(32, (int)((kSsfSmem - kSsfFixed - (size_t)lcap * 28) / ((size_t)kTabC * 8)));
+    e = cudaFuncSetAttribute(k_weights_ssf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSsfSmem);
     if (e != cudaSuccess) return e;
-    k_weights_ssf<<<nbatches, kWeightThreads, smem, st>>>(a, batch_ids);
+    k_weights_ssf<<<nbatches, kSsfThreads, kSsfSmem, st>>>(a, batch_ids, lcap, tabB);
   } else {
     e = cudaFuncSetAttribute(k_weights_batched<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(smem, 1024));
     if (e != cudaSuccess) return e;

@@ -413,14 +413,12 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
   auto cost = [&](int32_t j) { const BatchRec& b = hp.batches[j]; return (double)b.nb * b.nb * b.nq + 200.0 * b.ns * b.nq; };
   std::stable_sort(hp.ids_small.begin(), hp.ids_small.end(), [&](int32_t x, int32_t y) { return cost(x) > cost(y); });
   std::stable_sort(hp.ids_large.begin(), hp.ids_large.end(), [&](int32_t x, int32_t y) { return cost(x) > cost(y); });
-  // warps per CTA of the large-list weights launch: per-warp distance rows must fit in shared memory
+  // Becke-88 weights launch: warps per CTA such that the per-warp distance rows fit in shared memory
+  // (the SSF kernel has a fixed footprint and reads list entries beyond its cache from global memory)
   hp.w_warps_large = 8;
-  if (spec->partition == 0 && (size_t)hp.w_max_large * 36 + 512 * 30 + 2048 * 4 + 64 > kSmemLimit) {
-    err = "too many atoms inside the SSF support of one batch for the weights kernel"; return XC_EUNSUPPORTED;
-  }
   while (spec->partition != 0 && hp.w_warps_large > 1 && weights_smem_bytes(hp.w_max_large, hp.w_warps_large) > kSmemLimit) hp.w_warps_large >>= 1;
   if (spec->partition != 0 && weights_smem_bytes(hp.w_max_large, hp.w_warps_large) > kSmemLimit) {
-    err = "too many atoms inside the SSF support of one batch for the weights kernel"; return XC_EUNSUPPORTED;
+    err = "too many atoms for the Becke-88 weights kernel"; return XC_EUNSUPPORTED;
   }
   return XC_OK;
 }
