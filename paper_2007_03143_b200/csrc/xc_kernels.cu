@@ -660,16 +660,44 @@ __device__ __forceinline__ void fixed_add(unsigned long long* hi, unsigned long 
 //                 symmetric product (half the flops); the scaling by a_i is applied to the A fragment.
 //   per batch  6  increment of V (Eq. (17)): one fixed-point add per lower-triangle element.
 // ------------------------------------------------------------------------------------------------
-template <int T>
+// X^T tile of one warp: C[u][v] += A_u(16 points x 4 nu) * B_v(4 nu x 8 mu) over all k-steps; NV mu-tiles (compile
+// time), B fragments (packed P^j, global/L1) prefetched one k-step ahead.
+template <int NV, int NTW, int BS>
+__device__ __forceinline__ void xgemm_tile(double (&C)[2][NTW][2], const double* __restrict__ Ap, const double* __restrict__ Bp,
+                                           int nks, int astep, int bstep) {
+  double Bn[NV];
+#pragma unroll
+  for (int v = 0; v < NV; ++v) Bn[v] = __ldg(Bp + v * BS);
+  for (int ks = 0; ks < nks; ++ks) {
+    const double A0 = Ap[0], A1 = Ap[8];
+    double Bc[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) Bc[v] = Bn[v];
+    Ap += astep;
+    Bp += bstep;
+    if (ks + 1 < nks) {
+#pragma unroll
+      for (int v = 0; v < NV; ++v) Bn[v] = __ldg(Bp + v * BS);
+    }
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+      dmma884(C[0][v][0], C[0][v][1], A0, Bc[v]);
+      dmma884(C[1][v][0], C[1][v][1], A1, Bc[v]);
+    }
+  }
+}
+
+template <int NT, int T>
 struct BatchCfg {
+  static constexpr int NW = NT / 32;           // warps per CTA
   static constexpr int WP = T / 16;            // warps along points in the X GEMM
-  static constexpr int WM = 16 / WP;           // warps along mu
+  static constexpr int WM = NW / WP;           // warps along mu
   static constexpr int LD = T + 4;             // == 4 (mod 16) doubles: conflict-free fragment reads
 };
 
-template <int T, bool GGA, int NTW, int ROUNDS>
-__global__ void __launch_bounds__(kBatchThreads, 1) k_xc_batch(BatchArgs a, const int32_t* __restrict__ batch_ids) {
-  using Cfg = BatchCfg<T>;
+template <int NT, int T, bool GGA, int NTW, int ROUNDS>
+__global__ void __launch_bounds__(NT, NT == 256 ? 2 : 1) k_xc_batch(BatchArgs a, const int32_t* __restrict__ batch_ids) {
+  using Cfg = BatchCfg<NT, T>;
   constexpr int LD = Cfg::LD;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -698,16 +726,16 @@ __global__ void __launch_bounds__(kBatchThreads, 1) k_xc_batch(BatchArgs a, cons
   {
     const int32_t* fidx = a.bfidx + b.f_off;
     const int32_t* finfo = a.bfinfo + b.f_off;
-    for (int k = tid; k < ns; k += kBatchThreads) {
+    for (int k = tid; k < ns; k += NT) {
       ShellRec r = a.shells[a.bshells[b.sh_off + k]];
       r._pad = a.bsfoff[b.sh_off + k];
       sSh[k] = r;
     }
-    for (int f = tid; f < nb16; f += kBatchThreads) {
+    for (int f = tid; f < nb16; f += NT) {
       sIdx[f] = f < nb ? fidx[f] : 0;
       sInfo[f] = f < nb ? finfo[f] : 0;
     }
-    for (int e = tid; e < (nb16 - nb) * LD; e += kBatchThreads) {
+    for (int e = tid; e < (nb16 - nb) * LD; e += NT) {
       sPhi[(size_t)nb * LD + e] = 0.0;
       if (GGA) sZ[(size_t)nb * LD + e] = 0.0;
     }
@@ -716,7 +744,7 @@ __global__ void __launch_bounds__(kBatchThreads, 1) k_xc_batch(BatchArgs a, cons
   double V[ROUNDS][2][2][2];
 #pragma unroll
   for (int r = 0; r < ROUNDS; ++r) {
-    const int q = warp + 16 * r;
+    const int q = warp + Cfg::NW * r;
     int bm = (int)((sqrtf(8.0f * q + 1.0f) - 1.0f) * 0.5f);
     while ((bm + 1) * (bm + 2) / 2 <= q) ++bm;
     while (bm * (bm + 1) / 2 > q) --bm;
@@ -743,7 +771,7 @@ __global__ void __launch_bounds__(kBatchThreads, 1) k_xc_batch(BatchArgs a, cons
     __syncthreads();
 
     // ---- 1. collocation (Eq. (7); same shell across a warp) ----
-    for (int e = tid; e < ns * T; e += kBatchThreads) {
+    for (int e = tid; e < ns * T; e += NT) {
       const int slot = e / T, i = e - slot * T;
       const ShellRec sh = sSh[slot];
       const double dx = sx[i] - sh.x, dy = sy[i] - sh.y, dz = sz[i] - sh.z;
@@ -781,19 +809,15 @@ __global__ void __launch_bounds__(kBatchThreads, 1) k_xc_batch(BatchArgs a, cons
         for (int v = 0; v < NTW; ++v) C[u][v][0] = C[u][v][1] = 0.0;
       const double* Ap = sPhi + (size_t)t4 * LD + wp * 16 + g4;
       const double* Bp = ppk + (size_t)wm * 32 + lane;
-#pragma unroll 2
-      for (int ks = 0; ks < nks; ++ks) {
-        const double A0 = Ap[0], A1 = Ap[8];
-#pragma unroll
-        for (int v = 0; v < NTW; ++v) {
-          if (wm + v * Cfg::WM < ntile) {
-            const double Bv = __ldg(Bp + (size_t)v * Cfg::WM * 32);
-            dmma884(C[0][v][0], C[0][v][1], A0, Bv);
-            dmma884(C[1][v][0], C[1][v][1], A1, Bv);
-          }
-        }
-        Ap += 4 * LD;
-        Bp += (size_t)ntile * 32;
+      // number of mu-tiles of this warp (warp-uniform): one fully unrolled loop per count, so that no DMMA is
+      // ever issued predicated-off (a predicated-off DMMA still takes its slot in the FP64 tensor pipe)
+      const int nv = wm < ntile ? min(NTW, (ntile - wm + Cfg::WM - 1) / Cfg::WM) : 0;
+      switch (nv) {
+        case 1: xgemm_tile<1, NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
+        case 2: xgemm_tile<2, NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
+        case 3: xgemm_tile<3, NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
+        case 4: xgemm_tile<(NTW >= 4 ? 4 : 1), NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
+        default: break;
       }
       // epilogue: Eqs. (13),(14)
       double rho_acc[2] = {0.0, 0.0}, gx_acc[2] = {0.0, 0.0}, gy_acc[2] = {0.0, 0.0}, gz_acc[2] = {0.0, 0.0};
@@ -889,7 +913,7 @@ __global__ void __launch_bounds__(kBatchThreads, 1) k_xc_batch(BatchArgs a, cons
 
     // ---- 4. GGA: Z (Eq. (20)) ----
     if (GGA) {
-      for (int e = tid; e < nb * T; e += kBatchThreads) {
+      for (int e = tid; e < nb * T; e += NT) {
         const int mu = e / T, i = e - mu * T;
         const int info = sInfo[mu];
         const int slot = info >> 8;
@@ -1052,22 +1076,22 @@ cudaError_t launch_pack(const BatchArgs& a, const int32_t* batch_ids, int nbatch
   return cudaGetLastError();
 }
 
-template <int T, bool GGA, int NTW, int ROUNDS>
+template <int NT, int T, bool GGA, int NTW, int ROUNDS>
 static cudaError_t launch_batch_t(const BatchArgs& a, const int32_t* batch_ids, int nbatches, size_t smem, cudaStream_t st) {
-  cudaError_t e = cudaFuncSetAttribute(k_xc_batch<T, GGA, NTW, ROUNDS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaError_t e = cudaFuncSetAttribute(k_xc_batch<NT, T, GGA, NTW, ROUNDS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  k_xc_batch<T, GGA, NTW, ROUNDS><<<nbatches, kBatchThreads, smem, st>>>(a, batch_ids);
+  k_xc_batch<NT, T, GGA, NTW, ROUNDS><<<nbatches, NT, smem, st>>>(a, batch_ids);
   return cudaGetLastError();
 }
 
-// cls 0: N_b^j <= kSmallNb, tiles of 64 points; cls 1: N_b^j <= kMaxNb, tiles of 32 points
+// cls 0: N_b^j <= kSmallNb, 8 warps, two CTAs per SM; cls 1: N_b^j <= kMaxNb, 16 warps; tiles of 32 points
 cudaError_t launch_batch(int cls, bool gga, const BatchArgs& a, const int32_t* batch_ids, int nbatches, size_t smem,
                          cudaStream_t st) {
   if (nbatches <= 0) return cudaSuccess;
-  if (cls == 0) return gga ? launch_batch_t<64, true, 4, 2>(a, batch_ids, nbatches, smem, st)
-                           : launch_batch_t<64, false, 4, 2>(a, batch_ids, nbatches, smem, st);
-  return gga ? launch_batch_t<32, true, 3, 5>(a, batch_ids, nbatches, smem, st)
-             : launch_batch_t<32, false, 3, 5>(a, batch_ids, nbatches, smem, st);
+  if (cls == 0) return gga ? launch_batch_t<256, 32, true, 4, 4>(a, batch_ids, nbatches, smem, st)
+                           : launch_batch_t<256, 32, false, 4, 4>(a, batch_ids, nbatches, smem, st);
+  return gga ? launch_batch_t<512, 32, true, 3, 5>(a, batch_ids, nbatches, smem, st)
+             : launch_batch_t<512, 32, false, 3, 5>(a, batch_ids, nbatches, smem, st);
 }
 
 cudaError_t launch_finalize(int nbasis, const unsigned long long* vhi, const unsigned long long* vlo, double* V,

@@ -400,8 +400,8 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     hp.sum_nbnq += (double)b.nb * b.nq; hp.sum_nb2 += (double)b.nb * b.nb; hp.flops += 4.0 * b.nb * (double)b.nb * b.nq;
     hp.max_nb = std::max(hp.max_nb, b.nb); hp.max_ns = std::max(hp.max_ns, b.ns);
     if (b.nb == 0) continue;  // nothing to integrate: rho = 0 on every point
-    size_t s64 = batch_smem_bytes(64, gga, b.nb, b.ns);
-    if (b.nb <= kSmallNb && s64 <= kSmemLimit) {
+    size_t s64 = batch_smem_bytes(32, gga, b.nb, b.ns);
+    if (b.nb <= kSmallNb && s64 <= kSmemLimit / 2 - 2048) {
       hp.smem_small = std::max(hp.smem_small, s64);
       hp.ids_small.push_back((int32_t)j);
     } else {
