@@ -37,7 +37,7 @@ inline int ncart(int L) { return (L + 1) * (L + 2) / 2; }
 inline int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
 
 // shared-memory footprint of the batch kernel for a batch (bytes); T = points per tile
-size_t batch_smem_bytes(int T, bool gga, int nb, int ns);
+size_t batch_smem_bytes(int T, bool gga, int nb, int ns, int npr, int nthreads);   // npr: primitives of the batch's shells
 size_t weights_smem_bytes(int nC, int warps);
 
 struct HostPlan {

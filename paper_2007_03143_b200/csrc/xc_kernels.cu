@@ -20,6 +20,21 @@
 
 namespace xcb {
 
+// Optional per-phase cycle counters of the batch kernel (thread 0 of every CTA; development builds only:
+// compile with -DXC_PHASE_TIMING, read with xc_debug_phase).  Compiled out of the product library.
+#ifdef XC_PHASE_TIMING
+__device__ unsigned long long g_phase[16];
+#define PH_DECL long long _pt = clock64();
+#define PH(k) do { if (threadIdx.x == 0) { long long _n = clock64(); atomicAdd(&g_phase[k], (unsigned long long)(_n - _pt)); _pt = _n; } } while (0)
+extern "C" void xc_debug_phase(unsigned long long* out, int reset) {
+  if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(g_phase, z, sizeof(z)); }
+  else { cudaDeviceSynchronize(); cudaMemcpyFromSymbol(out, g_phase, sizeof(unsigned long long) * 16); }
+}
+#else
+#define PH_DECL
+#define PH(k)
+#endif
+
 // ------------------------------------------------------------------------------------------------
 // small device helpers
 // ------------------------------------------------------------------------------------------------
@@ -30,6 +45,43 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 }
 __device__ __forceinline__ double pw012(double v, int n) { return n == 0 ? 1.0 : (n == 1 ? v : v * v); }
 __device__ __forceinline__ double dpw012(double v, int n) { return n == 0 ? 0.0 : (n == 1 ? 1.0 : 2.0 * v); }
+
+// exp(-arg) for 0 <= arg < 708 (the result stays a normal number), <= 1 ulp: arg = -(n ln2/64 + r), n = 64 k + j,
+// exp(-arg) = 2^k 2^(j/64) (1 + p(r)), |r| <= ln2/128, p of degree 5 in Estrin form.  The dependent FP64 chain is 9
+// operations (the library exp: ~25), which is what the collocation stage waits on when the FP64 pipe is shared
+// with another CTA's DMMAs.  tab = 2^(j/64), j = 0..63, correctly rounded (shared-memory copy of kExp2Tab).
+__device__ const double kExp2Tab[64] = {
+    0x1.0000000000000p+0, 0x1.02c9a3e778061p+0, 0x1.059b0d3158574p+0, 0x1.0874518759bc8p+0,
+    0x1.0b5586cf9890fp+0, 0x1.0e3ec32d3d1a2p+0, 0x1.11301d0125b51p+0, 0x1.1429aaea92de0p+0,
+    0x1.172b83c7d517bp+0, 0x1.1a35beb6fcb75p+0, 0x1.1d4873168b9aap+0, 0x1.2063b88628cd6p+0,
+    0x1.2387a6e756238p+0, 0x1.26b4565e27cddp+0, 0x1.29e9df51fdee1p+0, 0x1.2d285a6e4030bp+0,
+    0x1.306fe0a31b715p+0, 0x1.33c08b26416ffp+0, 0x1.371a7373aa9cbp+0, 0x1.3a7db34e59ff7p+0,
+    0x1.3dea64c123422p+0, 0x1.4160a21f72e2ap+0, 0x1.44e086061892dp+0, 0x1.486a2b5c13cd0p+0,
+    0x1.4bfdad5362a27p+0, 0x1.4f9b2769d2ca7p+0, 0x1.5342b569d4f82p+0, 0x1.56f4736b527dap+0,
+    0x1.5ab07dd485429p+0, 0x1.5e76f15ad2148p+0, 0x1.6247eb03a5585p+0, 0x1.6623882552225p+0,
+    0x1.6a09e667f3bcdp+0, 0x1.6dfb23c651a2fp+0, 0x1.71f75e8ec5f74p+0, 0x1.75feb564267c9p+0,
+    0x1.7a11473eb0187p+0, 0x1.7e2f336cf4e62p+0, 0x1.82589994cce13p+0, 0x1.868d99b4492edp+0,
+    0x1.8ace5422aa0dbp+0, 0x1.8f1ae99157736p+0, 0x1.93737b0cdc5e5p+0, 0x1.97d829fde4e50p+0,
+    0x1.9c49182a3f090p+0, 0x1.a0c667b5de565p+0, 0x1.a5503b23e255dp+0, 0x1.a9e6b5579fdbfp+0,
+    0x1.ae89f995ad3adp+0, 0x1.b33a2b84f15fbp+0, 0x1.b7f76f2fb5e47p+0, 0x1.bcc1e904bc1d2p+0,
+    0x1.c199bdd85529cp+0, 0x1.c67f12e57d14bp+0, 0x1.cb720dcef9069p+0, 0x1.d072d4a07897cp+0,
+    0x1.d5818dcfba487p+0, 0x1.da9e603db3285p+0, 0x1.dfc97337b9b5fp+0, 0x1.e502ee78b3ff6p+0,
+    0x1.ea4afa2a490dap+0, 0x1.efa1bee615a27p+0, 0x1.f50765b6e4540p+0, 0x1.fa7c1819e90d8p+0};
+
+__device__ __forceinline__ double exp_neg(double arg, const double* __restrict__ tab) {
+  const double kMagic = 6755399441055744.0;                 // 1.5 * 2^52: the low word of (t + kMagic) is round(t)
+  double kd = fma(arg, -92.332482616893656768, kMagic);     // -64 / ln2
+  const int n = __double2loint(kd);
+  kd -= kMagic;
+  double r = fma(-kd, 0x1.62e42feep-7, -arg);               // ln2 / 64, high part (32 significant bits: exact product)
+  r = fma(-kd, 0x1.a39ef358p-39, r);
+  const double r2 = r * r;
+  const double qa = fma(r, 1.0 / 6.0, 0.5), qb = fma(r, 1.0 / 120.0, 1.0 / 24.0);
+  const double pr = fma(r2, fma(r2, qb, qa), r);
+  const double tj = tab[n & 63];
+  const double res = fma(tj, pr, tj);
+  return __hiloint2double(__double2hiint(res) + ((n >> 6) << 20), __double2loint(res));
+}
 
 // gradient of  x^l y^m z^n R0(r^2)  given R1 = dR0/d(r^2) * 2  (i.e. d/dx R0 = x R1)
 __device__ __forceinline__ void grad_cart(int info, double dx, double dy, double dz, double R0, double R1,
@@ -647,27 +699,39 @@ __device__ __forceinline__ void fixed_add(unsigned long long* hi, unsigned long 
 }
 
 // ------------------------------------------------------------------------------------------------
-// batch kernel: ONE CTA (512 threads, 16 warps) = one batch B_j, Alg. 4 l.4.3-4.10 fused.  The CTA walks
-// over the batch's points in tiles of T; nothing but the packed P^j is read from and nothing but the final
-// V^j increment is written to global memory:
-//   per tile   1  collocation: R0, R1 per (shell, point) -> sR (GGA); Phi -> sPhi[nu][i]            Eq. (7)
+// batch kernel: ONE CTA = one batch B_j, Alg. 4 l.4.3-4.10 fused.  The CTA walks over the batch's points in
+// tiles of T; nothing but the packed P^j is read from and nothing but the final V^j increment is written to
+// global memory:
+//   per batch  0  shell records, primitive table (alpha, d), collocation order, 2^(j/64) table -> shared memory
+//   per tile   1  collocation per (shell, point): R0, R1 -> sR (GGA); Phi -> sPhi[nu][i]              Eq. (7)
 //              2  X^T = Phi^T P^j on DMMA (M = points, N = mu, K = nu): A from sPhi, B = packed P^j    Eq. (15)
-//                 epilogue in registers: rho_i += Phi X, grad rho_i += grad Phi X                    Eqs. (13),(14)
+//                 LDA: rho_i += Phi X in the epilogue, straight from the accumulator registers          Eq. (13)
+//                 GGA: X^T -> shared memory (the Z buffer), then one pass per (shell, point):          Eqs. (13),(14)
+//                      with m_c the monomials of the shell, S0 = sum_c X_c m_c, G = sum_c X_c grad m_c:
+//                      rho_i += R0 S0, grad rho_i += R0 G + R1 S0 (r_i - R)
 //              3  functional at the T points; E / N_el partials                                     Eqs. (19),(16)
-//              4  GGA: Z = 1/2 a Phi + g . grad Phi -> sZ                                            Eq. (20)
+//              4  GGA: Z_c = m_c (a R0 + R1 g.(r_i - R)) + R0 g.grad m_c per (shell, point) -> sZ       Eq. (20)
 //              5  V^j += Z Phi^T + Phi Z^T on DMMA, lower-triangle 16x16 blocks, accumulators in     Eq. (18)
 //                 REGISTERS over all tiles of the batch.  LDA: Z = 1/2 a Phi, so V^j = (a Phi) Phi^T is one
 //                 symmetric product (half the flops); the scaling by a_i is applied to the A fragment.
 //   per batch  6  increment of V (Eq. (17)): one fixed-point add per lower-triangle element.
 // ------------------------------------------------------------------------------------------------
 // X^T tile of one warp: C[u][v] += A_u(16 points x 4 nu) * B_v(4 nu x 8 mu) over all k-steps; NV mu-tiles (compile
-// time), B fragments (packed P^j, global/L1) prefetched one k-step ahead.
+// time), B fragments (packed P^j, global/L1) loaded one k-step ahead into registers and kPfDist k-steps ahead
+// into L1 (the fragments of a batch are re-read for every tile, from L2 once they have left L1).
+constexpr int kPfDist = 4;
 template <int NV, int NTW, int BS>
 __device__ __forceinline__ void xgemm_tile(double (&C)[2][NTW][2], const double* __restrict__ Ap, const double* __restrict__ Bp,
                                            int nks, int astep, int bstep) {
   double Bn[NV];
 #pragma unroll
   for (int v = 0; v < NV; ++v) Bn[v] = __ldg(Bp + v * BS);
+#pragma unroll
+  for (int d = 1; d < kPfDist; ++d)
+    if (d < nks) {
+#pragma unroll
+      for (int v = 0; v < NV; ++v) asm volatile("prefetch.global.L1 [%0];" ::"l"(Bp + (size_t)d * bstep + v * BS));
+    }
   for (int ks = 0; ks < nks; ++ks) {
     const double A0 = Ap[0], A1 = Ap[8];
     double Bc[NV];
@@ -675,6 +739,10 @@ __device__ __forceinline__ void xgemm_tile(double (&C)[2][NTW][2], const double*
     for (int v = 0; v < NV; ++v) Bc[v] = Bn[v];
     Ap += astep;
     Bp += bstep;
+    if (ks + kPfDist < nks) {
+#pragma unroll
+      for (int v = 0; v < NV; ++v) asm volatile("prefetch.global.L1 [%0];" ::"l"(Bp + (size_t)(kPfDist - 1) * bstep + v * BS));
+    }
     if (ks + 1 < nks) {
 #pragma unroll
       for (int v = 0; v < NV; ++v) Bn[v] = __ldg(Bp + v * BS);
@@ -693,10 +761,11 @@ struct BatchCfg {
   static constexpr int WP = T / 16;            // warps along points in the X GEMM
   static constexpr int WM = NW / WP;           // warps along mu
   static constexpr int LD = T + 4;             // == 4 (mod 16) doubles: conflict-free fragment reads
+  static constexpr int NG = NT / T;            // thread groups of the per-(shell, point) passes
 };
 
-template <int NT, int T, bool GGA, int NTW, int ROUNDS>
-__global__ void __launch_bounds__(NT, NT == 256 ? 2 : 1) k_xc_batch(BatchArgs a, const int32_t* __restrict__ batch_ids) {
+template <int NT, int T, bool GGA, int NTW, int ROUNDS, int MINB>
+__global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_t* __restrict__ batch_ids) {
   using Cfg = BatchCfg<NT, T>;
   constexpr int LD = Cfg::LD;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -713,14 +782,16 @@ __global__ void __launch_bounds__(NT, NT == 256 ? 2 : 1) k_xc_batch(BatchArgs a,
   double* sPhi = (double*)sp; sp += (size_t)nb16 * LD * 8;
   double* sZ = (double*)sp; if (GGA) sp += (size_t)nb16 * LD * 8;
   double* sR = (double*)sp; if (GGA) sp += (size_t)ns * T * 16;
-  double* sPt = (double*)sp; sp += (size_t)12 * T * 8;
-  double* sRed = (double*)sp; sp += (size_t)1024 * 8;   // [WM][4][T], WM*4*T == 1024
+  double* sPt = (double*)sp; sp += (size_t)16 * T * 8;  // points x, y, z, w of two tiles (double buffer) + 8 T scratch
+  double* sRed = (double*)sp; sp += (size_t)NT * 4 * 8; // partial rho / grad rho: [groups][4][T]
+  double* sExpT = (double*)sp; sp += (size_t)64 * 8;    // 2^(j/64)
   ShellRec* sSh = (ShellRec*)sp; sp += (size_t)ns * sizeof(ShellRec);
   int* sInfo = (int*)sp; sp += (size_t)nb16 * 4;
-  int* sIdx = (int*)sp;
-  double *sx = sPt, *sy = sPt + T, *sz = sPt + 2 * T, *sw = sPt + 3 * T;
-  double *sE = sPt + 4 * T, *sN = sPt + 5 * T;
-  double *sA = sPt + 8 * T, *sG0 = sPt + 9 * T, *sG1 = sPt + 10 * T, *sG2 = sPt + 11 * T;
+  int* sIdx = (int*)sp; sp += (size_t)nb16 * 4;
+  int* sOrd = (int*)sp; sp += (size_t)((ns + 3) & ~3) * 4;   // [ns] shell slots, most primitives first
+  double2* sPrim = (double2*)sp;                        // (alpha, d) of the batch's primitives, shell by shell
+  double *sE = sPt + 8 * T, *sN = sPt + 9 * T;
+  double *sA = sPt + 10 * T, *sG0 = sPt + 11 * T, *sG1 = sPt + 12 * T, *sG2 = sPt + 13 * T;
 
   // ---- per batch: metadata, zero padding rows, V^j block assignment ----
   {
@@ -728,7 +799,8 @@ __global__ void __launch_bounds__(NT, NT == 256 ? 2 : 1) k_xc_batch(BatchArgs a,
     const int32_t* finfo = a.bfinfo + b.f_off;
     for (int k = tid; k < ns; k += NT) {
       ShellRec r = a.shells[a.bshells[b.sh_off + k]];
-      r._pad = a.bsfoff[b.sh_off + k];
+      r._pad = a.bsfoff[b.sh_off + k];         // first local function of the shell
+      r.atom = r.prim_off;                     // global primitive offset (the atom index is not used here)
       sSh[k] = r;
     }
     for (int f = tid; f < nb16; f += NT) {
@@ -738,6 +810,28 @@ __global__ void __launch_bounds__(NT, NT == 256 ? 2 : 1) k_xc_batch(BatchArgs a,
     for (int e = tid; e < (nb16 - nb) * LD; e += NT) {
       sPhi[(size_t)nb * LD + e] = 0.0;
       if (GGA) sZ[(size_t)nb * LD + e] = 0.0;
+    }
+    for (int k = tid; k < 64; k += NT) sExpT[k] = kExp2Tab[k];
+    if (tid < T) {                               // points of the first tile
+      const int64_t gi = (int64_t)b.pt_off + min(tid, b.nq - 1);
+      sPt[tid] = a.px[gi]; sPt[T + tid] = a.py[gi]; sPt[2 * T + tid] = a.pz[gi];
+      sPt[3 * T + tid] = tid < b.nq ? a.w[gi] : 0.0;
+    }
+    __syncthreads();
+    // collocation order (shells with the most primitives first, dealt round-robin to the warps) and the
+    // primitive table: shell k's primitives start at the sum of the counts before it
+    for (int k = tid; k < ns; k += NT) {
+      const int ck = sSh[k].nprim * 4 + sSh[k].L;
+      int rank = 0, loc = 0;
+      for (int j = 0; j < ns; ++j) {
+        const int cj = sSh[j].nprim * 4 + sSh[j].L;
+        rank += (cj > ck || (cj == ck && j < k)) ? 1 : 0;
+        loc += j < k ? sSh[j].nprim : 0;
+      }
+      sOrd[rank] = k;
+      const int goff = sSh[k].atom, np = sSh[k].nprim;
+      for (int q = 0; q < np; ++q) sPrim[loc + q] = make_double2(__ldg(a.exps + goff + q), __ldg(a.coefs + goff + q));
+      sSh[k].prim_off = loc;                   // only thread k reads or writes this field from here on ... until the barrier
     }
   }
   int blk_m[ROUNDS], blk_n[ROUNDS];
@@ -758,32 +852,34 @@ __global__ void __launch_bounds__(NT, NT == 256 ? 2 : 1) k_xc_batch(BatchArgs a,
   const double* __restrict__ ppk = a.ppk + b.ppk_off;
   const int wp = warp % Cfg::WP, wm = warp / Cfg::WP;
   double Eacc = 0.0, Nacc = 0.0;
-
-  for (int t0 = 0; t0 < b.nq; t0 += T) {
+  PH_DECL
+  PH(0);
+  for (int t0 = 0, it = 0; t0 < b.nq; t0 += T, ++it) {
     const int npt = min(T, b.nq - t0);         // valid points in this tile
-    __syncthreads();                           // previous tile's readers of sPhi / sZ / sPt are done
-    if (tid < T) {
-      const int li = min(tid, npt - 1);
-      const int64_t gi = (int64_t)b.pt_off + t0 + li;
-      sx[tid] = a.px[gi]; sy[tid] = a.py[gi]; sz[tid] = a.pz[gi];
-      sw[tid] = tid < npt ? a.w[gi] : 0.0;
-    }
-    __syncthreads();
+    const double* sx = sPt + (size_t)(it & 1) * 4 * T;   // this tile's points (written one tile ahead)
+    const double *sy = sx + T, *sz = sx + 2 * T, *sw = sx + 3 * T;
+    __syncthreads();                           // previous tile's readers of sPhi / sZ are done; tables / points visible
+    PH(1);
 
     // ---- 1. collocation (Eq. (7); same shell across a warp) ----
-    for (int e = tid; e < ns * T; e += NT) {
-      const int slot = e / T, i = e - slot * T;
+    for (int q = warp; q < ns * (T / 32); q += Cfg::NW) {
+      const int slot = sOrd[q / (T / 32)], i = (q % (T / 32)) * 32 + lane;
       const ShellRec sh = sSh[slot];
       const double dx = sx[i] - sh.x, dy = sy[i] - sh.y, dz = sz[i] - sh.z;
       const double r2 = dx * dx + dy * dy + dz * dz;
+      const double2* pr = sPrim + sh.prim_off;
       double R0 = 0.0, R1 = 0.0;
       for (int k = 0; k < sh.nprim; ++k) {
-        const double al = __ldg(a.exps + sh.prim_off + k);
-        const double arg = al * r2;
-        if (arg < 746.0) {                     // beyond, exp() underflows to exactly 0: skipping is bit-identical
-          const double ev = __ldg(a.coefs + sh.prim_off + k) * exp(-arg);
+        const double2 ad = pr[k];
+        const double arg = ad.x * r2;
+        if (arg < 708.0) {                     // beyond, exp(-arg) < 3.3e-308: dropped (it cannot change any result)
+#ifdef XC_EXP_STUB
+          const double ev = ad.y * (1.0 - 1e-3 * arg);
+#else
+          const double ev = ad.y * exp_neg(arg, sExpT);
+#endif
           R0 += ev;
-          R1 = fma(-2.0 * al, ev, R1);
+          R1 = fma(-2.0 * ad.x, ev, R1);
         }
       }
       if (GGA) *reinterpret_cast<double2*>(sR + ((size_t)slot * T + i) * 2) = make_double2(R0, R1);
@@ -799,6 +895,7 @@ __global__ void __launch_bounds__(NT, NT == 256 ? 2 : 1) k_xc_batch(BatchArgs a,
       }
     }
     __syncthreads();
+    PH(2);
 
     // ---- 2. X^T = Phi^T P^j and the density reductions ----
     {
@@ -814,70 +911,99 @@ __global__ void __launch_bounds__(NT, NT == 256 ? 2 : 1) k_xc_batch(BatchArgs a,
       const int nv = wm < ntile ? min(NTW, (ntile - wm + Cfg::WM - 1) / Cfg::WM) : 0;
       switch (nv) {
         case 1: xgemm_tile<1, NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
-        case 2: xgemm_tile<2, NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
-        case 3: xgemm_tile<3, NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
+        case 2: xgemm_tile<(NTW >= 2 ? 2 : 1), NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
+        case 3: xgemm_tile<(NTW >= 3 ? 3 : 1), NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
         case 4: xgemm_tile<(NTW >= 4 ? 4 : 1), NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
         default: break;
       }
-      // epilogue: Eqs. (13),(14)
-      double rho_acc[2] = {0.0, 0.0}, gx_acc[2] = {0.0, 0.0}, gy_acc[2] = {0.0, 0.0}, gz_acc[2] = {0.0, 0.0};
-#pragma unroll
-      for (int u = 0; u < 2; ++u) {
-        const int i = wp * 16 + u * 8 + g4;
-        const double xi = sx[i], yi = sy[i], zi = sz[i];
+      if (GGA) {
+        // X^T -> shared memory (the Z buffer, [mu][i]); rows >= nb receive exact zeros (zero padding of the packed P^j)
 #pragma unroll
         for (int v = 0; v < NTW; ++v) {
-          if (wm + v * Cfg::WM < ntile) {
+          if (v < nv) {
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-              const int mu = (wm + v * Cfg::WM) * 8 + t4 * 2 + h;
-              if (mu < nb) {
-                const double X = C[u][v][h];
-                rho_acc[u] = fma(sPhi[(size_t)mu * LD + i], X, rho_acc[u]);
-                if (GGA) {
-                  const int info = sInfo[mu];
-                  const int slot = info >> 8;
-                  const double2 R = *reinterpret_cast<const double2*>(sR + ((size_t)slot * T + i) * 2);
-                  double gx, gy, gz;
-                  grad_cart(info, xi - sSh[slot].x, yi - sSh[slot].y, zi - sSh[slot].z, R.x, R.y, gx, gy, gz);
-                  gx_acc[u] = fma(gx, X, gx_acc[u]);
-                  gy_acc[u] = fma(gy, X, gy_acc[u]);
-                  gz_acc[u] = fma(gz, X, gz_acc[u]);
-                }
+            for (int u = 0; u < 2; ++u)
+#pragma unroll
+              for (int h = 0; h < 2; ++h)
+                sZ[(size_t)((wm + v * Cfg::WM) * 8 + t4 * 2 + h) * LD + wp * 16 + u * 8 + g4] = C[u][v][h];
+          }
+        }
+      } else {
+        // epilogue: Eq. (13)
+        double rho_acc[2] = {0.0, 0.0};
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+          const int i = wp * 16 + u * 8 + g4;
+#pragma unroll
+          for (int v = 0; v < NTW; ++v) {
+            if (v < nv) {
+#pragma unroll
+              for (int h = 0; h < 2; ++h) {
+                const int mu = (wm + v * Cfg::WM) * 8 + t4 * 2 + h;    // rows >= nb of sPhi are zero
+                rho_acc[u] = fma(sPhi[(size_t)mu * LD + i], C[u][v][h], rho_acc[u]);
               }
             }
           }
         }
-      }
-      // reduce over the 4 lanes sharing a point, then over the WM warps (fixed order => deterministic)
+        // reduce over the 4 lanes sharing a point, then over the WM warps (fixed order => deterministic)
 #pragma unroll
-      for (int u = 0; u < 2; ++u) {
-#pragma unroll
-        for (int o = 1; o <= 2; o <<= 1) {
-          rho_acc[u] += __shfl_xor_sync(0xffffffffu, rho_acc[u], o);
-          if (GGA) {
-            gx_acc[u] += __shfl_xor_sync(0xffffffffu, gx_acc[u], o);
-            gy_acc[u] += __shfl_xor_sync(0xffffffffu, gy_acc[u], o);
-            gz_acc[u] += __shfl_xor_sync(0xffffffffu, gz_acc[u], o);
-          }
-        }
-        if (t4 == 0) {
-          const int i = wp * 16 + u * 8 + g4;
-          sRed[(size_t)(wm * 4 + 0) * T + i] = rho_acc[u];
-          if (GGA) {
-            sRed[(size_t)(wm * 4 + 1) * T + i] = gx_acc[u];
-            sRed[(size_t)(wm * 4 + 2) * T + i] = gy_acc[u];
-            sRed[(size_t)(wm * 4 + 3) * T + i] = gz_acc[u];
-          }
+        for (int u = 0; u < 2; ++u) {
+          rho_acc[u] += __shfl_xor_sync(0xffffffffu, rho_acc[u], 1);
+          rho_acc[u] += __shfl_xor_sync(0xffffffffu, rho_acc[u], 2);
+          if (t4 == 0) sRed[(size_t)(wm * 4) * T + wp * 16 + u * 8 + g4] = rho_acc[u];
         }
       }
     }
     __syncthreads();
+    if (GGA) {
+      // density pass per (shell, point): thread = (group, point); a group walks over the shells group, group + NG, ...
+      const int i = tid % T, grp = tid / T;
+      const double xi = sx[i], yi = sy[i], zi = sz[i];
+      double rho = 0.0, gx = 0.0, gy = 0.0, gz = 0.0;
+      for (int slot = grp; slot < ns; slot += Cfg::NG) {
+        const ShellRec sh = sSh[slot];
+        const double dx = xi - sh.x, dy = yi - sh.y, dz = zi - sh.z;
+        const double2 R = *reinterpret_cast<const double2*>(sR + ((size_t)slot * T + i) * 2);
+        const double* xp = sZ + (size_t)sh._pad * LD + i;
+        double S0, Gx, Gy, Gz;
+        if (sh.L == 0) {
+          S0 = xp[0]; Gx = Gy = Gz = 0.0;
+        } else if (sh.L == 1) {
+          Gx = xp[0]; Gy = xp[LD]; Gz = xp[2 * LD];
+          S0 = fma(Gx, dx, fma(Gy, dy, Gz * dz));
+        } else {
+          const double Xxx = xp[0], Xxy = xp[LD], Xxz = xp[2 * LD], Xyy = xp[3 * LD], Xyz = xp[4 * LD], Xzz = xp[5 * LD];
+          Gx = fma(2.0 * Xxx, dx, fma(Xxy, dy, Xxz * dz));
+          Gy = fma(Xxy, dx, fma(2.0 * Xyy, dy, Xyz * dz));
+          Gz = fma(Xxz, dx, fma(Xyz, dy, 2.0 * Xzz * dz));
+          S0 = 0.5 * fma(Gx, dx, fma(Gy, dy, Gz * dz));
+        }
+        rho = fma(R.x, S0, rho);
+        const double t = R.y * S0;
+        gx = fma(R.x, Gx, fma(t, dx, gx));
+        gy = fma(R.x, Gy, fma(t, dy, gy));
+        gz = fma(R.x, Gz, fma(t, dz, gz));
+      }
+      sRed[(size_t)(grp * 4 + 0) * T + i] = rho;
+      sRed[(size_t)(grp * 4 + 1) * T + i] = gx;
+      sRed[(size_t)(grp * 4 + 2) * T + i] = gy;
+      sRed[(size_t)(grp * 4 + 3) * T + i] = gz;
+      __syncthreads();
+    }
+    PH(3);
 
-    // ---- 3. functional (Eq. (19)), E and N_el partials (Eq. (16)) ----
+    // ---- 3. functional (Eq. (19)), E and N_el partials (Eq. (16)); the warps after the first T threads fetch
+    //         the next tile's points into the other buffer ----
+    if (tid >= T && tid < 2 * T && t0 + T < b.nq) {
+      const int li = tid - T, nn = min(T, b.nq - t0 - T);
+      const int64_t gi = (int64_t)b.pt_off + t0 + T + min(li, nn - 1);
+      double* nx = sPt + (size_t)((it + 1) & 1) * 4 * T;
+      nx[li] = a.px[gi]; nx[T + li] = a.py[gi]; nx[2 * T + li] = a.pz[gi];
+      nx[3 * T + li] = li < nn ? a.w[gi] : 0.0;
+    }
     if (tid < T) {
       double rho = 0.0, gx = 0.0, gy = 0.0, gz = 0.0;
-      for (int q = 0; q < Cfg::WM; ++q) {
+      for (int q = 0; q < (GGA ? Cfg::NG : Cfg::WM); ++q) {
         rho += sRed[(size_t)(q * 4 + 0) * T + tid];
         if (GGA) {
           gx += sRed[(size_t)(q * 4 + 1) * T + tid];
@@ -907,22 +1033,39 @@ __global__ void __launch_bounds__(NT, NT == 256 ? 2 : 1) k_xc_batch(BatchArgs a,
       if (lane == 0) { sE[warp] = e; sN[warp] = n; }
     }
     __syncthreads();
+    PH(4);
     if (tid == 0) {
       for (int q = 0; q < T / 32; ++q) { Eacc += sE[q]; Nacc += sN[q]; }
     }
 
-    // ---- 4. GGA: Z (Eq. (20)) ----
+    // ---- 4. GGA: Z (Eq. (20)) per (shell, point); overwrites X^T ----
     if (GGA) {
-      for (int e = tid; e < nb * T; e += NT) {
-        const int mu = e / T, i = e - mu * T;
-        const int info = sInfo[mu];
-        const int slot = info >> 8;
+      const int i = tid % T, grp = tid / T;
+      const double xi = sx[i], yi = sy[i], zi = sz[i];
+      const double ai = sA[i], g0 = sG0[i], g1 = sG1[i], g2 = sG2[i];
+      for (int slot = grp; slot < ns; slot += Cfg::NG) {
+        const ShellRec sh = sSh[slot];
+        const double dx = xi - sh.x, dy = yi - sh.y, dz = zi - sh.z;
         const double2 R = *reinterpret_cast<const double2*>(sR + ((size_t)slot * T + i) * 2);
-        double gx, gy, gz;
-        grad_cart(info, sx[i] - sSh[slot].x, sy[i] - sSh[slot].y, sz[i] - sSh[slot].z, R.x, R.y, gx, gy, gz);
-        sZ[(size_t)mu * LD + i] = fma(sG0[i], gx, fma(sG1[i], gy, fma(sG2[i], gz, sA[i] * sPhi[(size_t)mu * LD + i])));
+        const double base = fma(ai, R.x, R.y * fma(g0, dx, fma(g1, dy, g2 * dz)));   // a R0 + R1 g.(r - R)
+        double* zp = sZ + (size_t)sh._pad * LD + i;
+        if (sh.L == 0) {
+          zp[0] = base;
+        } else if (sh.L == 1) {
+          zp[0] = fma(dx, base, R.x * g0); zp[LD] = fma(dy, base, R.x * g1); zp[2 * LD] = fma(dz, base, R.x * g2);
+        } else {
+          const double bx = dx * base, by = dy * base;
+          const double r0 = R.x;
+          zp[0] = fma(dx, bx, 2.0 * r0 * dx * g0);
+          zp[LD] = fma(dy, bx, r0 * fma(dy, g0, dx * g1));
+          zp[2 * LD] = fma(dz, bx, r0 * fma(dz, g0, dx * g2));
+          zp[3 * LD] = fma(dy, by, 2.0 * r0 * dy * g1);
+          zp[4 * LD] = fma(dz, by, r0 * fma(dz, g1, dy * g2));
+          zp[5 * LD] = fma(dz * dz, base, 2.0 * r0 * dz * g2);
+        }
       }
       __syncthreads();
+      PH(5);
     }
 
     // ---- 5. V^j += Z Phi^T + Phi Z^T (lower-triangle 16x16 blocks; Eq. (18)) ----
@@ -957,8 +1100,10 @@ __global__ void __launch_bounds__(NT, NT == 256 ? 2 : 1) k_xc_batch(BatchArgs a,
         }
       }
     }
+    PH(6);
   }
 
+  PH(7);
   // ---- 6. increment of V (Eq. (17)), lower triangle; global indices ascend with local ones ----
   if (tid == 0) { a.Epart[bidx] = Eacc; a.Npart[bidx] = Nacc; }
 #pragma unroll
@@ -981,6 +1126,7 @@ __global__ void __launch_bounds__(NT, NT == 256 ? 2 : 1) k_xc_batch(BatchArgs a,
         }
     }
   }
+  PH(8);
 }
 
 // fixed point -> fp64, mirrored.  32x32 tiles, tm >= tn.
@@ -1076,11 +1222,11 @@ cudaError_t launch_pack(const BatchArgs& a, const int32_t* batch_ids, int nbatch
   return cudaGetLastError();
 }
 
-template <int NT, int T, bool GGA, int NTW, int ROUNDS>
+template <int NT, int T, bool GGA, int NTW, int ROUNDS, int MINB>
 static cudaError_t launch_batch_t(const BatchArgs& a, const int32_t* batch_ids, int nbatches, size_t smem, cudaStream_t st) {
-  cudaError_t e = cudaFuncSetAttribute(k_xc_batch<NT, T, GGA, NTW, ROUNDS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaError_t e = cudaFuncSetAttribute(k_xc_batch<NT, T, GGA, NTW, ROUNDS, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  k_xc_batch<NT, T, GGA, NTW, ROUNDS><<<nbatches, NT, smem, st>>>(a, batch_ids);
+  k_xc_batch<NT, T, GGA, NTW, ROUNDS, MINB><<<nbatches, NT, smem, st>>>(a, batch_ids);
   return cudaGetLastError();
 }
 
@@ -1088,10 +1234,15 @@ static cudaError_t launch_batch_t(const BatchArgs& a, const int32_t* batch_ids, 
 cudaError_t launch_batch(int cls, bool gga, const BatchArgs& a, const int32_t* batch_ids, int nbatches, size_t smem,
                          cudaStream_t st) {
   if (nbatches <= 0) return cudaSuccess;
-  if (cls == 0) return gga ? launch_batch_t<256, 32, true, 4, 4>(a, batch_ids, nbatches, smem, st)
-                           : launch_batch_t<256, 32, false, 4, 4>(a, batch_ids, nbatches, smem, st);
-  return gga ? launch_batch_t<512, 32, true, 3, 5>(a, batch_ids, nbatches, smem, st)
-             : launch_batch_t<512, 32, false, 3, 5>(a, batch_ids, nbatches, smem, st);
+#ifdef XC_HIOCC
+  if (cls == 0) return gga ? launch_batch_t<512, 32, true, 2, 2, 2>(a, batch_ids, nbatches, smem, st)
+                           : launch_batch_t<512, 32, false, 2, 2, 2>(a, batch_ids, nbatches, smem, st);
+#else
+  if (cls == 0) return gga ? launch_batch_t<256, 32, true, 4, 4, 2>(a, batch_ids, nbatches, smem, st)
+                           : launch_batch_t<256, 32, false, 4, 4, 2>(a, batch_ids, nbatches, smem, st);
+#endif
+  return gga ? launch_batch_t<512, 32, true, 3, 5, 1>(a, batch_ids, nbatches, smem, st)
+             : launch_batch_t<512, 32, false, 3, 5, 1>(a, batch_ids, nbatches, smem, st);
 }
 
 cudaError_t launch_finalize(int nbasis, const unsigned long long* vhi, const unsigned long long* vlo, double* V,

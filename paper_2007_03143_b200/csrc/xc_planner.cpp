@@ -93,17 +93,20 @@ struct Leaf { int64_t begin, end; };
 
 }  // namespace
 
-size_t batch_smem_bytes(int T, bool gga, int nb, int ns) {
+size_t batch_smem_bytes(int T, bool gga, int nb, int ns, int npr, int nthreads) {
   // must mirror the shared-memory carve of k_xc_batch (xc_kernels.cu)
   size_t nb16 = round_up(nb, 16);
   size_t b = 0;
   b += nb16 * (T + 4) * 8;                       // Phi tile
   if (gga) b += nb16 * (T + 4) * 8;              // Z tile
   if (gga) b += (size_t)ns * T * 2 * 8;          // R0/R1 panel
-  b += (size_t)T * 8 * 12;                       // x,y,z,w, scratch, a,g0,g1,g2
-  b += 1024 * 8;                                 // cross-warp reduction buffer
+  b += (size_t)T * 8 * 16;                       // x,y,z,w of two tiles, scratch, a,g0,g1,g2
+  b += (size_t)nthreads * 4 * 8;                 // cross-warp reduction buffer
+  b += 64 * 8;                                   // 2^(j/64) table of the collocation exp
+  b += (size_t)npr * 16;                         // (exponent, coefficient) of the batch's primitives
   b += (size_t)ns * sizeof(ShellRec);            // shell records
   b += nb16 * 4 * 2;                             // function info + global function index
+  b += (size_t)((ns + 3) & ~3) * 4;              // collocation order
   return b + 64;
 }
 
@@ -224,12 +227,13 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
   std::vector<int> nbs(leaves.size());
 #pragma omp parallel for schedule(dynamic, 64)
   for (int64_t j = 0; j < (int64_t)leaves.size(); ++j) screen(leaves[j], lists[j], nbs[j]);
+  auto prim_sum = [&](const std::vector<int32_t>& sl) { int n = 0; for (int32_t sh : sl) n += hp.shells[sh].nprim; return n; };
   // re-split oversized batches (rare): sequential fix-up pass
   {
     std::vector<Leaf> L2; std::vector<std::vector<int32_t>> S2; std::vector<int> N2;
     bool any = false;
     for (size_t j = 0; j < leaves.size(); ++j)
-      if (nbs[j] > kMaxNb || batch_smem_bytes(32, gga, nbs[j], (int)lists[j].size()) > kSmemLimit) { any = true; break; }
+      if (nbs[j] > kMaxNb || batch_smem_bytes(32, gga, nbs[j], (int)lists[j].size(), prim_sum(lists[j]), kBatchThreads) > kSmemLimit) { any = true; break; }
     if (any) {
       for (size_t j = 0; j < leaves.size(); ++j) {
         std::vector<Leaf> st{leaves[j]};
@@ -239,7 +243,7 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
           std::vector<int32_t> sl; int nb;
           if (first) { sl = lists[j]; nb = nbs[j]; first = false; } else screen(cur, sl, nb);
           int64_t n = cur.end - cur.begin;
-          if (nb <= kMaxNb && batch_smem_bytes(32, gga, nb, (int)sl.size()) <= kSmemLimit) { L2.push_back(cur); S2.push_back(sl); N2.push_back(nb); continue; }
+          if (nb <= kMaxNb && batch_smem_bytes(32, gga, nb, (int)sl.size(), prim_sum(sl), kBatchThreads) <= kSmemLimit) { L2.push_back(cur); S2.push_back(sl); N2.push_back(nb); continue; }
           if (n <= 1) { err = "a single grid point sees more basis functions than the batch kernel supports"; return XC_EUNSUPPORTED; }
           double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
           for (int64_t k = cur.begin; k < cur.end; ++k)
@@ -400,12 +404,14 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     hp.sum_nbnq += (double)b.nb * b.nq; hp.sum_nb2 += (double)b.nb * b.nb; hp.flops += 4.0 * b.nb * (double)b.nb * b.nq;
     hp.max_nb = std::max(hp.max_nb, b.nb); hp.max_ns = std::max(hp.max_ns, b.ns);
     if (b.nb == 0) continue;  // nothing to integrate: rho = 0 on every point
-    size_t s64 = batch_smem_bytes(32, gga, b.nb, b.ns);
+    int npr = 0;
+    for (int k = 0; k < b.ns; ++k) npr += hp.shells[hp.bshells[b.sh_off + k]].nprim;
+    size_t s64 = batch_smem_bytes(32, gga, b.nb, b.ns, npr, kBatchThreads / 2);
     if (b.nb <= kSmallNb && s64 <= kSmemLimit / 2 - 2048) {
       hp.smem_small = std::max(hp.smem_small, s64);
       hp.ids_small.push_back((int32_t)j);
     } else {
-      hp.smem_large = std::max(hp.smem_large, batch_smem_bytes(32, gga, b.nb, b.ns));
+      hp.smem_large = std::max(hp.smem_large, batch_smem_bytes(32, gga, b.nb, b.ns, npr, kBatchThreads));
       hp.ids_large.push_back((int32_t)j);
     }
   }
