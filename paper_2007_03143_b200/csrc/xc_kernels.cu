@@ -102,22 +102,27 @@ __device__ __forceinline__ void grad_cart(int info, double dx, double dy, double
 #define XC_CX 0.7385587663820224058842300326808360  // (3/4)(3/pi)^(1/3)
 #define XC_RSFAC 0.6203504908994000166680068120477781  // (3/(4 pi))^(1/3)
 
+// The point functional is evaluated by ONE warp per tile while the other warps wait, so its dependent chain is kept
+// short: one rcbrt and one rsqrt give every power of rho and r_s, and the reciprocals are merged (4 divisions each).
 __device__ __forceinline__ void lda_slater_vwn5(double rho, double& f, double& vr) {
   const double A = 0.0310907, x0 = -0.10498, b = 3.72744, c = 12.9352;
   const double Q = 6.1519908197590802321728722658;         // sqrt(4c - b^2)
   const double Xx0 = x0 * x0 + b * x0 + c;
   const double bx0 = b * x0 / Xx0;
-  double r13 = cbrt(rho);
-  double rs = XC_RSFAC / r13;
-  double x = sqrt(rs);
-  double X = fma(x, x + b, c);
-  double tb = 2.0 * x + b;
-  double at = atan(Q / tb);
-  double xm = x - x0;
-  double eps = A * (log(x * x / X) + (2.0 * b / Q) * at - bx0 * (log(xm * xm / X) + (2.0 * (b + 2.0 * x0) / Q) * at));
-  double q2 = 1.0 / (Q * Q + tb * tb);
-  double deps = A * (2.0 / x - tb / X - 4.0 * b * q2 - bx0 * (2.0 / xm - tb / X - 4.0 * (2.0 * x0 + b) * q2));
-  double vc = eps - (x / 6.0) * deps;
+  const double ir13 = rcbrt(rho);
+  const double r13 = rho * ir13 * ir13;
+  const double rs = XC_RSFAC * ir13;
+  const double isx = rsqrt(rs);
+  const double x = rs * isx;                                // sqrt(r_s)
+  const double X = fma(x, x + b, c);
+  const double tb = 2.0 * x + b;
+  const double xm = x - x0;
+  const double iX = 1.0 / X, itb = 1.0 / tb, ixm = 1.0 / xm;
+  const double at = atan(Q * itb);
+  const double eps = A * (log(x * x * iX) + (2.0 * b / Q) * at - bx0 * (log(xm * xm * iX) + (2.0 * (b + 2.0 * x0) / Q) * at));
+  const double q2 = 1.0 / (Q * Q + tb * tb);
+  const double deps = A * (2.0 * isx - tb * iX - 4.0 * b * q2 - bx0 * (2.0 * ixm - tb * iX - 4.0 * (2.0 * x0 + b) * q2));
+  const double vc = eps - (x / 6.0) * deps;
   f = rho * (eps - XC_CX * r13);
   vr = vc - (4.0 / 3.0) * XC_CX * r13;
 }
@@ -128,41 +133,47 @@ __device__ __forceinline__ void gga_pbe(double rho, double sigma, double& f, dou
   const double A = 0.0310907, a1 = 0.21370, b1 = 7.5957, b2 = 3.5876, b3 = 1.6382, b4 = 0.49294;
   const double c_s2 = 38.283120002509214;      // 4 (3 pi^2)^(2/3)
   const double c_t2 = 0.06346820609770369;     // pi / (16 (3 pi^2)^(1/3))
-  double r13 = cbrt(rho);
-  double r43 = rho * r13;
+  const double ir13 = rcbrt(rho);
+  const double ir23 = ir13 * ir13;
+  const double r13 = rho * ir23;
+  const double r43 = rho * r13;
+  const double ir43 = ir23 * ir23, irho = ir23 * ir13;
   // exchange
-  double s2 = sigma / (c_s2 * r43 * r43);
-  double den = 1.0 / (kappa + mu * s2);
-  double F = 1.0 + kappa - kappa * kappa * den;
-  double dF = kappa * kappa * mu * den * den;
-  double fx = -XC_CX * r43 * F;
-  double vxr = -(4.0 / 3.0) * XC_CX * r13 * (F - 2.0 * s2 * dF);
-  double vxs = -XC_CX * dF / (c_s2 * r43);
+  const double s2 = sigma * (ir43 * ir43) * (1.0 / c_s2);
+  const double den = 1.0 / (kappa + mu * s2);
+  const double F = 1.0 + kappa - kappa * kappa * den;
+  const double dF = kappa * kappa * mu * den * den;
+  const double fx = -XC_CX * r43 * F;
+  const double vxr = -(4.0 / 3.0) * XC_CX * r13 * (F - 2.0 * s2 * dF);
+  const double vxs = -XC_CX * dF * ir43 * (1.0 / c_s2);
   // PW92
-  double rs = XC_RSFAC / r13;
-  double srs = sqrt(rs);
-  double q = 2.0 * A * (srs * (b1 + b3 * rs) + rs * (b2 + b4 * rs));
-  double dq = 2.0 * A * (0.5 * b1 / srs + b2 + 1.5 * b3 * srs + 2.0 * b4 * rs);
-  double lg = log1p(1.0 / q);
-  double eu = -2.0 * A * (1.0 + a1 * rs) * lg;
-  double deu_drs = -2.0 * A * a1 * lg + 2.0 * A * (1.0 + a1 * rs) * dq / (q * (q + 1.0));
-  double deu = -deu_drs * rs / (3.0 * rho);    // d eps_unif / d rho
+  const double rs = XC_RSFAC * ir13;
+  const double isrs = rsqrt(rs);
+  const double srs = rs * isrs;
+  const double q = 2.0 * A * (srs * (b1 + b3 * rs) + rs * (b2 + b4 * rs));
+  const double dq = 2.0 * A * (0.5 * b1 * isrs + b2 + 1.5 * b3 * srs + 2.0 * b4 * rs);
+  const double tq = 1.0 / (q * (q + 1.0));
+  const double lg = log1p(tq * (q + 1.0));     // log(1 + 1/q)
+  const double eu = -2.0 * A * (1.0 + a1 * rs) * lg;
+  const double deu_drs = -2.0 * A * a1 * lg + 2.0 * A * (1.0 + a1 * rs) * dq * tq;
+  const double deu = -deu_drs * rs * irho * (1.0 / 3.0);    // d eps_unif / d rho
   // H
-  double r73 = r43 * rho;
-  double yfac = c_t2 / r73;
-  double y = sigma * yfac;
-  double Em1 = expm1(-eu / gamma);
-  double Ac = (beta / gamma) / Em1;
-  double Ay = Ac * y;
-  double N = 1.0 + Ay, D = 1.0 + Ay + Ay * Ay;
-  double G = (beta / gamma) * y * N / D;
-  double H = gamma * log1p(G);
-  double iD2G = 1.0 / (D * D * (1.0 + G));
-  double dHdy = beta * (1.0 + 2.0 * Ay) * iD2G;
-  double dHdA = -beta * y * Ay * y * (2.0 + Ay) * iD2G;
-  double dAde = Ac * Ac * (Em1 + 1.0) / beta;
-  double vcs = rho * dHdy * yfac;
-  double vcr = eu + H + rho * (deu + dHdy * (-(7.0 / 3.0) * y / rho) + dHdA * dAde * deu);
+  const double yfac = c_t2 * ir43 * irho;      // c_t2 / rho^(7/3)
+  const double y = sigma * yfac;
+  const double Em1 = expm1(-eu * (1.0 / gamma));
+  const double Ac = (beta / gamma) / Em1;
+  const double Ay = Ac * y;
+  const double N = 1.0 + Ay, D = 1.0 + Ay + Ay * Ay;
+  const double cyN = (beta / gamma) * y * N;
+  const double Du = D + cyN;                   // D (1 + G)
+  const double iDDu = 1.0 / (D * Du);          // 1 / (D^2 (1 + G))
+  const double G = cyN * (iDDu * Du);
+  const double H = gamma * log1p(G);
+  const double dHdy = beta * (1.0 + 2.0 * Ay) * iDDu;
+  const double dHdA = -beta * y * Ay * y * (2.0 + Ay) * iDDu;
+  const double dAde = Ac * Ac * (Em1 + 1.0) * (1.0 / beta);
+  const double vcs = rho * dHdy * yfac;
+  const double vcr = eu + H + rho * (deu + dHdy * (-(7.0 / 3.0) * y * irho) + dHdA * dAde * deu);
   f = fx + rho * (eu + H);
   vr = vxr + vcr;
   vs = vxs + vcs;
