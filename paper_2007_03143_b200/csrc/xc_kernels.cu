@@ -477,6 +477,21 @@ __device__ __forceinline__ double ssf_cell_product(SsfCtx& s, int bb, double Bx,
   const int nscan = ssf_nscan(s, krB);                     // every later C has r_C >= kappa r_B: factor 1
   const bool tab = bb >= 0 && bb < s.tabB;
   double part = 1.0;
+  if (tab && s.filled >= s.nC) {
+    // short list (the whole row was filled up front and every partner is in the table): no chunk tests; a factor
+    // that is exactly 1 comes out of the clamped polynomial as exactly 1
+    const double* trow = s.sTab + bb * kTabC + s.lane;
+    const double* rrow = s.sRC + s.lane;
+    for (int ch = 0; ch < nscan; ++ch) {
+      double zz = (rB - rrow[ch << 5]) * trow[ch << 5];     // (B, B): 0, factor 1/2; c >= nC: r_C = 1e300, entry 1
+      if (__any_sync(FULL, zz >= 1.0)) return 0.0;         // s = 0: P_B = 0
+      zz = zz < -1.0 ? -1.0 : zz;
+      part *= ssf_poly(zz);
+    }
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) part *= __shfl_xor_sync(FULL, part, o);
+    return part * 2.0;
+  }
   for (int ch = 0; ch < nscan; ++ch) {
     const int c0 = ch << 5, c = c0 + s.lane;
     const double rC = ssf_dist(s, c0);
@@ -608,6 +623,9 @@ __global__ void __launch_bounds__(kSsfThreads, 2) k_weights_ssf(WeightArgs a, co
       if (rm < rmin) { rmin = rm; im = c0 + __ffs(__ballot_sync(FULL, hi == mhi && lo == mlo)) - 1; }
     }
     const double own_lim = kappa * rmin;
+    if (nC <= kRcap) {                                     // short list: complete the row now (fast cell products)
+      for (int c0 = s.filled; c0 < nC; c0 += 32) ssf_dist(s, c0);
+    }
     // ---- 2. the parent's cell product ----
     const double Ax = a.atoms[3 * A], Ay = a.atoms[3 * A + 1], Az = a.atoms[3 * A + 2];
     double rA;
