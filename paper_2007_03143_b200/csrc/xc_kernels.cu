@@ -1098,34 +1098,33 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
     }
 
     // ---- 5. V^j += Z Phi^T + Phi Z^T (lower-triangle 16x16 blocks; Eq. (18)) ----
-#pragma unroll 2
-    for (int kk = 0; kk < T / 4; ++kk) {
-      const int i = kk * 4 + t4;
-      const double ai = GGA ? 0.0 : sA[i];
+    // block by block (one block's fragment addresses live at a time), all T/4 k-steps of the tile per block
 #pragma unroll
-      for (int r = 0; r < ROUNDS; ++r) {
-        if (blk_m[r] >= 0) {
-          const double* pm = sPhi + (size_t)(blk_m[r] * 16 + g4) * LD + i;
-          const double* pn = sPhi + (size_t)(blk_n[r] * 16 + g4) * LD + i;
-          const bool diag = blk_m[r] == blk_n[r];
-          if (GGA) {
-            const double* zm = sZ + (size_t)(blk_m[r] * 16 + g4) * LD + i;
-            const double* zn = sZ + (size_t)(blk_n[r] * 16 + g4) * LD + i;
-            const double Pm0 = pm[0], Pm1 = pm[8 * LD], Zm0 = zm[0], Zm1 = zm[8 * LD];
-            const double Pn0 = pn[0], Pn1 = pn[8 * LD], Zn0 = zn[0], Zn1 = zn[8 * LD];
-            dmma884(V[r][0][0][0], V[r][0][0][1], Zm0, Pn0); dmma884(V[r][0][0][0], V[r][0][0][1], Pm0, Zn0);
-            dmma884(V[r][1][0][0], V[r][1][0][1], Zm1, Pn0); dmma884(V[r][1][0][0], V[r][1][0][1], Pm1, Zn0);
-            dmma884(V[r][1][1][0], V[r][1][1][1], Zm1, Pn1); dmma884(V[r][1][1][0], V[r][1][1][1], Pm1, Zn1);
-            if (!diag) { dmma884(V[r][0][1][0], V[r][0][1][1], Zm0, Pn1); dmma884(V[r][0][1][0], V[r][0][1][1], Pm0, Zn1); }
-          } else {
-            const double Pm0 = pm[0], Pm1 = pm[8 * LD];
-            const double Pn0 = pn[0], Pn1 = pn[8 * LD];
-            const double Zm0 = ai * Pm0, Zm1 = ai * Pm1;
-            dmma884(V[r][0][0][0], V[r][0][0][1], Zm0, Pn0);
-            dmma884(V[r][1][0][0], V[r][1][0][1], Zm1, Pn0);
-            dmma884(V[r][1][1][0], V[r][1][1][1], Zm1, Pn1);
-            if (!diag) dmma884(V[r][0][1][0], V[r][0][1][1], Zm0, Pn1);
-          }
+    for (int r = 0; r < ROUNDS; ++r) {
+      if (blk_m[r] < 0) continue;
+      const int om = (blk_m[r] * 16 + g4) * LD + t4, on = (blk_n[r] * 16 + g4) * LD + t4;
+      const bool diag = blk_m[r] == blk_n[r];
+      if (GGA) {
+#pragma unroll 4
+        for (int kk = 0; kk < T / 4; ++kk) {
+          const double Pm0 = sPhi[om + 4 * kk], Pm1 = sPhi[om + 8 * LD + 4 * kk], Zm0 = sZ[om + 4 * kk], Zm1 = sZ[om + 8 * LD + 4 * kk];
+          const double Pn0 = sPhi[on + 4 * kk], Pn1 = sPhi[on + 8 * LD + 4 * kk], Zn0 = sZ[on + 4 * kk], Zn1 = sZ[on + 8 * LD + 4 * kk];
+          dmma884(V[r][0][0][0], V[r][0][0][1], Zm0, Pn0); dmma884(V[r][0][0][0], V[r][0][0][1], Pm0, Zn0);
+          dmma884(V[r][1][0][0], V[r][1][0][1], Zm1, Pn0); dmma884(V[r][1][0][0], V[r][1][0][1], Pm1, Zn0);
+          dmma884(V[r][1][1][0], V[r][1][1][1], Zm1, Pn1); dmma884(V[r][1][1][0], V[r][1][1][1], Pm1, Zn1);
+          if (!diag) { dmma884(V[r][0][1][0], V[r][0][1][1], Zm0, Pn1); dmma884(V[r][0][1][0], V[r][0][1][1], Pm0, Zn1); }
+        }
+      } else {
+#pragma unroll 4
+        for (int kk = 0; kk < T / 4; ++kk) {
+          const double ai = sA[4 * kk + t4];
+          const double Pm0 = sPhi[om + 4 * kk], Pm1 = sPhi[om + 8 * LD + 4 * kk];
+          const double Pn0 = sPhi[on + 4 * kk], Pn1 = sPhi[on + 8 * LD + 4 * kk];
+          const double Zm0 = ai * Pm0, Zm1 = ai * Pm1;
+          dmma884(V[r][0][0][0], V[r][0][0][1], Zm0, Pn0);
+          dmma884(V[r][1][0][0], V[r][1][0][1], Zm1, Pn0);
+          dmma884(V[r][1][1][0], V[r][1][1][1], Zm1, Pn1);
+          if (!diag) dmma884(V[r][0][1][0], V[r][0][1][1], Zm0, Pn1);
         }
       }
     }
