@@ -12,7 +12,7 @@ namespace xcb {
 constexpr int kMaxL = 2;
 constexpr int kMaxPrim = 16;
 constexpr int kBatchThreads = 512;  // 16 warps per batch CTA
-constexpr int kSmallNb = 112;   // N_b^j limit of the 64-point-tile instantiation (<= 28 lower-triangle 16x16 blocks = 2 per warp)
+constexpr int kSmallNb = 112;   // N_b^j limit of the 64-point-tile instantiation (<= 28 lower-triangle 16x16 blocks = 2 per warp of 16)
 constexpr int kMaxNb = 192;     // N_b^j limit of the batch kernel (<= 78 blocks = 5 per warp); the planner splits larger batches
 constexpr size_t kSmemLimit = 227 * 1024;
 constexpr int kWeightSmallList = 192; // atom-list length that separates the two launches of the weights kernel

@@ -1258,17 +1258,12 @@ static cudaError_t launch_batch_t(const BatchArgs& a, const int32_t* batch_ids, 
   return cudaGetLastError();
 }
 
-// cls 0: N_b^j <= kSmallNb, 8 warps, two CTAs per SM; cls 1: N_b^j <= kMaxNb, 16 warps; tiles of 32 points
+// cls 0: N_b^j <= kSmallNb, tiles of 64 points; cls 1: N_b^j <= kMaxNb, tiles of 32 points; 16 warps, one CTA per SM
 cudaError_t launch_batch(int cls, bool gga, const BatchArgs& a, const int32_t* batch_ids, int nbatches, size_t smem,
                          cudaStream_t st) {
   if (nbatches <= 0) return cudaSuccess;
-#ifdef XC_HIOCC
-  if (cls == 0) return gga ? launch_batch_t<512, 32, true, 2, 2, 2>(a, batch_ids, nbatches, smem, st)
-                           : launch_batch_t<512, 32, false, 2, 2, 2>(a, batch_ids, nbatches, smem, st);
-#else
-  if (cls == 0) return gga ? launch_batch_t<256, 32, true, 4, 4, 2>(a, batch_ids, nbatches, smem, st)
-                           : launch_batch_t<256, 32, false, 4, 4, 2>(a, batch_ids, nbatches, smem, st);
-#endif
+  if (cls == 0) return gga ? launch_batch_t<512, 64, true, 4, 2, 1>(a, batch_ids, nbatches, smem, st)
+                           : launch_batch_t<512, 64, false, 4, 2, 1>(a, batch_ids, nbatches, smem, st);
   return gga ? launch_batch_t<512, 32, true, 3, 5, 1>(a, batch_ids, nbatches, smem, st)
              : launch_batch_t<512, 32, false, 3, 5, 1>(a, batch_ids, nbatches, smem, st);
 }

@@ -406,8 +406,9 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     if (b.nb == 0) continue;  // nothing to integrate: rho = 0 on every point
     int npr = 0;
     for (int k = 0; k < b.ns; ++k) npr += hp.shells[hp.bshells[b.sh_off + k]].nprim;
-    size_t s64 = batch_smem_bytes(32, gga, b.nb, b.ns, npr, kBatchThreads / 2);
-    if (b.nb <= kSmallNb && s64 <= kSmemLimit / 2 - 2048) {
+    // class 0: 64-point tiles, 16 warps, one CTA per SM; class 1 (N_b^j > kSmallNb or a 64-point tile does not fit): 32-point tiles
+    size_t s64 = batch_smem_bytes(64, gga, b.nb, b.ns, npr, kBatchThreads);
+    if (b.nb <= kSmallNb && s64 <= kSmemLimit - 1024) {
       hp.smem_small = std::max(hp.smem_small, s64);
       hp.ids_small.push_back((int32_t)j);
     } else {
