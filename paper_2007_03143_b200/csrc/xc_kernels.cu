@@ -470,6 +470,7 @@ __device__ __forceinline__ double ssf_dist(SsfCtx& s, int c0) {
 }
 
 // P_B = prod_C s(mu_BC).  bb = list position of B (warp-uniform, -1: not in the list), rB = r_B.
+// (Bx, By, Bz) is only read for bb < 0; a list atom's coordinates are fetched where the table does not reach.
 __device__ __forceinline__ double ssf_cell_product(SsfCtx& s, int bb, double Bx, double By, double Bz, double rB) {
   const unsigned FULL = 0xffffffffu;
   const double kappa = (1.0 + 0.64) / (1.0 - 0.64);
@@ -492,6 +493,7 @@ __device__ __forceinline__ double ssf_cell_product(SsfCtx& s, int bb, double Bx,
     for (int o = 16; o >= 1; o >>= 1) part *= __shfl_xor_sync(FULL, part, o);
     return part * 2.0;
   }
+  if (bb >= 0) ssf_atom(s, bb, Bx, By, Bz);
   for (int ch = 0; ch < nscan; ++ch) {
     const int c0 = ch << 5, c = c0 + s.lane;
     const double rC = ssf_dist(s, c0);
@@ -598,6 +600,7 @@ __global__ void __launch_bounds__(kSsfThreads, 2) k_weights_ssf(WeightArgs a, co
     tabB = tb;
     __syncthreads();
   }
+  const int tcols = tabB > 0 ? min((nC + 31) & ~31, kTabC) : 0;   // table columns that were built
 
   SsfCtx s;
   s.sX = sX; s.sY = sY; s.sZ = sZ; s.sId = sId; s.sTab = sTab; s.sDm = sDm; s.sRC = sRCall + warp * kRcap; s.a = &a; s.box = box;
@@ -648,29 +651,41 @@ __global__ void __launch_bounds__(kSsfThreads, 2) k_weights_ssf(WeightArgs a, co
         for (int b0 = 0; b0 < nown; b0 += 32) {
           const int bb = b0 + lane;
           const double rB = ssf_dist(s, b0);
-          double bx = 0.0, by = 0.0, bz = 0.0;
           bool cand = bb < nB && bb != ia && rB < own_lim;   // else r_B >= kappa r_min: P_B = 0 exactly
-          if (cand) ssf_atom(s, bb, bx, by, bz);
           // pre-filter: mu_BC >= a for one of the first kPre list atoms or the nearest atom  =>  P_B = 0
           const int npre = min(kPre, nC);
-          for (int k = 0; k < npre; ++k) {                   // positions < 32 of the row are always filled (scan 1)
-            const double u = rB - s.sRC[k];
-            const double ex = bx - sX[k], ey = by - sY[k], ez = bz - sZ[k];
-            if (k != bb && u > 0.0 && u * u >= (aa * aa) * (ex * ex + ey * ey + ez * ez)) cand = false;
-          }
-          if (im >= npre) {
-            const double u = rB - rmin;
-            const double ex = bx - mx, ey = by - my, ez = bz - mz;
-            if (im != bb && u > 0.0 && u * u >= (aa * aa) * (ex * ex + ey * ey + ez * ez)) cand = false;
+          if (tabB >= npre && b0 + 32 <= tcols) {
+            // 1 / (a R_Bk) = table entry (k, B): row k is warp-uniform, the lanes read consecutive columns;
+            // the entry (B, B) is 0, so k = B never fires
+            for (int k = 0; k < npre; ++k)                   // positions < 32 of the row are always filled (scan 1)
+              if ((rB - s.sRC[k]) * sTab[k * kTabC + bb] >= 1.0) cand = false;
+            if (im >= npre && __any_sync(FULL, cand)) {
+              double bx = 0.0, by = 0.0, bz = 0.0;
+              if (cand) ssf_atom(s, bb, bx, by, bz);
+              const double u = rB - rmin;
+              const double ex = bx - mx, ey = by - my, ez = bz - mz;
+              if (im != bb && u > 0.0 && u * u >= (aa * aa) * (ex * ex + ey * ey + ez * ez)) cand = false;
+            }
+          } else {
+            double bx = 0.0, by = 0.0, bz = 0.0;
+            if (cand) ssf_atom(s, bb, bx, by, bz);
+            for (int k = 0; k < npre; ++k) {
+              const double u = rB - s.sRC[k];
+              const double ex = bx - sX[k], ey = by - sY[k], ez = bz - sZ[k];
+              if (k != bb && u > 0.0 && u * u >= (aa * aa) * (ex * ex + ey * ey + ez * ez)) cand = false;
+            }
+            if (im >= npre) {
+              const double u = rB - rmin;
+              const double ex = bx - mx, ey = by - my, ez = bz - mz;
+              if (im != bb && u > 0.0 && u * u >= (aa * aa) * (ex * ex + ey * ey + ez * ez)) cand = false;
+            }
           }
           unsigned mask = __ballot_sync(FULL, cand);
           while (mask) {
             const int src = __ffs(mask) - 1;
             mask &= mask - 1;
             const int bs = b0 + src;
-            double Bx, By, Bz;
-            ssf_atom(s, bs, Bx, By, Bz);
-            sum += ssf_cell_product(s, bs, Bx, By, Bz, __shfl_sync(FULL, rB, src));
+            sum += ssf_cell_product(s, bs, 0.0, 0.0, 0.0, __shfl_sync(FULL, rB, src));
           }
         }
         result = a.wq[gi] * PA / sum;
