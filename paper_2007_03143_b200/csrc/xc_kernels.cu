@@ -494,7 +494,8 @@ __device__ __forceinline__ double ssf_cell_product(SsfCtx& s, int bb, double Bx,
     return part * 2.0;
   }
   if (bb >= 0) ssf_atom(s, bb, Bx, By, Bz);
-  for (int ch = 0; ch < nscan; ++ch) {
+  const int nrow = min(nscan, kRcap >> 5);                 // chunks served by the distance row
+  for (int ch = 0; ch < nrow; ++ch) {
     const int c0 = ch << 5, c = c0 + s.lane;
     const double rC = ssf_dist(s, c0);
     if (!__any_sync(FULL, rC < krB)) continue;             // 32 factors exactly 1
@@ -509,6 +510,28 @@ __device__ __forceinline__ double ssf_cell_product(SsfCtx& s, int bb, double Bx,
         const double ex = Bx - cx, ey = By - cy, ez = Bz - cz;
         zz = (rB - rC) * (rsqrt(ex * ex + ey * ey + ez * ez) * (1.0 / 0.64));   // mu_BC / a
       }
+    }
+    if (__any_sync(FULL, zz >= 1.0)) return 0.0;           // s = 0: P_B = 0
+    zz = zz < -1.0 ? -1.0 : zz;
+    part *= ssf_poly(zz);
+  }
+  // partners past the row: r_C and R_BC from one fetch of the coordinates
+  for (int ch = nrow; ch < nscan; ++ch) {
+    const int c0 = ch << 5, c = c0 + s.lane;
+    const bool valid = c < s.nC;
+    double cx = 0.0, cy = 0.0, cz = 0.0, rC = 1e300;
+    if (valid) {
+      ssf_atom(s, c, cx, cy, cz);
+      const double dx = s.x - cx, dy = s.y - cy, dz = s.z - cz;
+      rC = sqrt(dx * dx + dy * dy + dz * dz);
+    }
+    if (!__any_sync(FULL, rC < krB)) continue;             // 32 factors exactly 1
+    double zz = -1.0;                                      // factor exactly 1
+    if (tab && c0 < kTabC) {
+      zz = (rB - rC) * s.sTab[bb * kTabC + c];
+    } else if (valid && c != bb) {
+      const double ex = Bx - cx, ey = By - cy, ez = Bz - cz;
+      zz = (rB - rC) * (rsqrt(ex * ex + ey * ey + ez * ez) * (1.0 / 0.64));   // mu_BC / a
     }
     if (__any_sync(FULL, zz >= 1.0)) return 0.0;           // s = 0: P_B = 0
     zz = zz < -1.0 ? -1.0 : zz;
