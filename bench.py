@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- grid points/s of the full E_xc + V_xc + N_el build (fp64) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2] [--also c4,c5] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2] [--also c3,c4,c5,u2,g1] [--impl reference]
 
 A step = one pass of the whole hot path (weights -> density -> potential -> scatter/finalise) over one
 synthetic water-cluster workload (BASELINE.json:configs; generator: workloads/).  Prints ONE JSON line.
@@ -209,7 +209,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="c2")
-    ap.add_argument("--also", default="c3,c4,c5", help="comma list of extra workloads reported under other_workloads (or 'none')")
+    ap.add_argument("--also", default="c3,c4,c5,u2,g1", help="comma list of extra workloads reported under other_workloads (or 'none')")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

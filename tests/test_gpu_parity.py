@@ -208,9 +208,10 @@ def test_partition_kernel_vs_oracle(xc, orc, kind):
 
 
 # ---- full-size configs: sampled outputs + properties ---------------------------------------------
-@pytest.mark.parametrize("name", ["c4", "c5"])
+@pytest.mark.parametrize("name", ["c4", "c5", "u2", "g1"])
 def test_full_size_sampled(xc, orc, name):
-    """256- and 512-water PBE workloads in the launch configuration bench.py times.  The oracle cannot run
+    """256- and 512-water PBE workloads in the launch configuration bench.py times, plus the two SURVEY 8(f)
+    "next" workloads: u2 (64 waters on the UFG-shaped 99 x 590 grid) and g1 (irregular 410-water cluster).  The oracle cannot run
     them whole in seconds, so it computes (i) the weights, rho, grad rho and the per-batch E / N_el partial sums
     of sampled batches, and (ii) sampled V entries exactly: V[mu,nu] only receives contributions from batches
     whose S_j holds both shells, so evaluating that subset of batches gives the full entry.  Properties at any

@@ -52,6 +52,12 @@ CONFIGS = {
     "c3": Config("c3", (4, 4, 4), 320, 75, 302, 1, BASIS_SEED + 2),  # same geometry/basis/P as c2
     "c4": Config("c4", (8, 8, 4), 1280, 75, 302, 1, BASIS_SEED + 4),
     "c5": Config("c5", (8, 8, 8), 2560, 100, 302, 1, BASIS_SEED + 5),
+    # SURVEY.md section 8(f) item 2 ("next" workloads, not in BASELINE.json): u2 = the c2 cluster on a UFG-shaped
+    # 99 x 590 grid (Table 2); g1 = an irregular, surface-heavy cluster of 410 waters (1230 atoms,
+    # 10250 functions: the shape of the paper's Ubiquitin runs, Table 1) -- lattice (0, 0, n)
+    # means n molecules placed by random sequential addition in an ellipsoid
+    "u2": Config("u2", (4, 4, 4), 320, 99, 590, 1, BASIS_SEED + 2),
+    "g1": Config("g1", (0, 0, 410), 2050, 75, 302, 1, BASIS_SEED + 11),
     # small extra shapes for tests (not in BASELINE.json): 8 and 27 waters
     "w8": Config("w8", (2, 2, 2), 40, 50, 194, 1, BASIS_SEED + 8),
     "w27": Config("w27", (3, 3, 3), 135, 50, 194, 1, BASIS_SEED + 27),
@@ -117,6 +123,25 @@ def _geometry(rng, lattice):
     coords, zs = [], []
     if lattice == (1, 1, 1):
         return _MONOMER * ANGSTROM, _MONOMER_Z.copy()
+    if nx == 0:
+        # irregular cluster: nz molecules, O centres by random sequential addition (min O-O distance 2.6 A) in an
+        # ellipsoid with semi-axes (1.6, 1.0, 0.7) R sized for one molecule per (3.3 A)^3; random rotations
+        n = nz
+        axes = np.array([1.6, 1.0, 0.7]) * (n * 3.3 ** 3 / (4.0 / 3.0 * np.pi * 1.6 * 0.7)) ** (1.0 / 3.0)
+        centres = np.zeros((0, 3))
+        while len(centres) < n:
+            c = rng.uniform(-1.0, 1.0, size=3)
+            if c @ c > 1.0:
+                continue
+            c = c * axes
+            if len(centres) and np.min(np.sum((centres - c) ** 2, axis=1)) < 2.6 ** 2:
+                continue
+            centres = np.vstack([centres, c])
+        for c in centres:
+            R = _quat_to_rot(rng.standard_normal(4))
+            coords.append(_MONOMER @ R.T + c)
+            zs.append(_MONOMER_Z)
+        return np.concatenate(coords) * ANGSTROM, np.concatenate(zs)
     for i in range(nx):
         for j in range(ny):
             for k in range(nz):
@@ -250,7 +275,7 @@ def make_workload(name: str, with_P: bool = True, cache: bool = True) -> Workloa
     if not with_P:
         return w
     key = hashlib.sha1(("v1|%d|%s|%d|%d" % (cfg.geom_seed, cfg.lattice, cfg.n_occ, BASIS_SEED)).encode()).hexdigest()[:16]
-    path = os.path.join(_cache_dir(), "P_%s_%s.npy" % (cfg.name if cfg.name != "c3" else "c2", key))
+    path = os.path.join(_cache_dir(), "P_%s_%s.npy" % (cfg.name if cfg.name not in ("c3", "u2") else "c2", key))
     if cache and os.path.exists(path):
         P = np.load(path)
         if P.shape == (nb, nb):
