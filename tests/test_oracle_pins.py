@@ -468,3 +468,21 @@ def test_workload_generator_shapes():
     assert w2.n_basis == 1600 and len(w2.atoms_Z) == 192
     a, b = make_workload("c1"), make_workload("c1", cache=False)
     assert np.array_equal(a.P, b.P) and np.allclose(a.P, a.P.T)
+
+
+def test_next_workload_shapes():
+    """SURVEY 8(f) item 2 workloads: u2 = the c2 cluster on a 99 x 590 grid (Table 2, PAPER.md:L302: 99 * 590 = 58410 per atom);
+    g1 = irregular 410-water cluster (1230 atoms, 10250 functions), seeded and reproducible, O-O distances >= 2.6 A."""
+    u2, c2 = make_workload("u2", with_P=False), make_workload("c2", with_P=False)
+    assert np.array_equal(u2.atoms_xyz, c2.atoms_xyz) and np.array_equal(u2.exps, c2.exps)
+    assert (u2.n_rad, u2.n_ang) == (99, 590) and u2.n_rad * u2.n_ang == 58410 and u2.functional == 1
+    g1, g1b = make_workload("g1", with_P=False), make_workload("g1", with_P=False)
+    assert np.array_equal(g1.atoms_xyz, g1b.atoms_xyz)
+    assert len(g1.atoms_Z) == 1230 and g1.n_basis == 10250 and list(g1.atoms_Z[:3]) == [8, 1, 1]
+    O = g1.atoms_xyz[::3]
+    d2 = np.sum((O[:, None, :] - O[None, :, :]) ** 2, axis=2) + 1e9 * np.eye(len(O))
+    assert np.sqrt(d2.min()) >= 2.6 * 1.8897261246257702 - 1e-9
+    # O-H bond lengths are the monomer's
+    assert np.allclose(np.linalg.norm(g1.atoms_xyz[1::3] - O, axis=1), np.linalg.norm(c2.atoms_xyz[1] - c2.atoms_xyz[0]))
+    ext = O.max(0) - O.min(0)
+    assert ext[0] > 1.8 * ext[2]          # elongated: not a cube
