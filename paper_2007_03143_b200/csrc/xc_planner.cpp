@@ -178,13 +178,11 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
   const double* coord[3] = {cx.data(), cy.data(), cz.data()};
   std::vector<Leaf> leaves;
   {
-    std::vector<Leaf> stack;
-    stack.push_back({0, npts});
-    // depth-first, left part first => spatially coherent output order
-    while (!stack.empty()) {
-      Leaf cur = stack.back(); stack.pop_back();
+    // one bisection step: splits `cur` at the median of its longest axis (left part first => depth-first output order
+    // is spatially coherent); returns false if the range is a leaf
+    auto split = [&](const Leaf& cur, Leaf& left, Leaf& right) {
       int64_t n = cur.end - cur.begin;
-      if (n <= maxp) { leaves.push_back(cur); continue; }
+      if (n <= maxp) return false;
       double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
       for (int64_t k = cur.begin; k < cur.end; ++k)
         for (int p = 0; p < 3; ++p) { double v = coord[p][idx[k]]; lo[p] = std::min(lo[p], v); hi[p] = std::max(hi[p], v); }
@@ -195,9 +193,46 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
       const double* c = coord[ax];
       std::nth_element(idx.begin() + cur.begin, idx.begin() + cur.begin + half, idx.begin() + cur.end,
                        [c](int64_t a, int64_t b) { return c[a] < c[b] || (c[a] == c[b] && a < b); });
-      stack.push_back({cur.begin + half, cur.end});
-      stack.push_back({cur.begin, cur.begin + half});
+      left = {cur.begin, cur.begin + half};
+      right = {cur.begin + half, cur.end};
+      return true;
+    };
+    auto subtree = [&](Leaf root, std::vector<Leaf>& out) {   // depth-first, left part first
+      std::vector<Leaf> stack{root};
+      while (!stack.empty()) {
+        Leaf cur = stack.back(); stack.pop_back();
+        Leaf l, r;
+        if (!split(cur, l, r)) { out.push_back(cur); continue; }
+        stack.push_back(r);
+        stack.push_back(l);
+      }
+    };
+    // the first levels breadth-first (kept in left-to-right order), then the subtrees in parallel; the ranges are
+    // disjoint slices of idx, and the leaves are concatenated in subtree order: the plan does not depend on the
+    // number of threads
+    std::vector<Leaf> front{{0, npts}};
+    for (int level = 0; level < 7; ++level) {
+      std::vector<Leaf> next(2 * front.size());
+      std::vector<char> isleaf(front.size(), 0);
+#pragma omp parallel for schedule(dynamic, 1)
+      for (int64_t k = 0; k < (int64_t)front.size(); ++k) {
+        Leaf l, r;
+        if (front[k].end - front[k].begin <= 16 * (int64_t)maxp || !split(front[k], l, r)) { isleaf[k] = 1; continue; }
+        next[2 * k] = l; next[2 * k + 1] = r;
+      }
+      std::vector<Leaf> merged;
+      bool any = false;
+      for (size_t k = 0; k < front.size(); ++k) {
+        if (isleaf[k]) merged.push_back(front[k]);
+        else { merged.push_back(next[2 * k]); merged.push_back(next[2 * k + 1]); any = true; }
+      }
+      front.swap(merged);
+      if (!any) break;
     }
+    std::vector<std::vector<Leaf>> parts(front.size());
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t k = 0; k < (int64_t)front.size(); ++k) subtree(front[k], parts[k]);
+    for (auto& v : parts) leaves.insert(leaves.end(), v.begin(), v.end());
   }
 
   // ---- per-batch shell screening (Alg. 1 on the tight bounding box), with re-splitting of batches whose

@@ -109,3 +109,20 @@ def test_bench_reference_arm_and_gloo_two_ranks():
                          capture_output=True, text=True, timeout=600, env=env)
     assert out.returncode == 0, out.stderr[-2000:]
     assert "gloo ok 2" in out.stdout
+
+
+def test_plan_does_not_depend_on_thread_count():
+    """The planner bisects subtrees in parallel (OpenMP); the plan must be the same for any number of threads."""
+    code = ("import hashlib, sys; sys.path.insert(0, %r)\n"
+            "import paper_2007_03143_b200 as xc\n"
+            "from workloads import make_workload\n"
+            "w = make_workload('w27', with_P=False)\n"
+            "p = xc.Plan.from_workload(w, spec=xc.grid_spec(w.n_rad, w.n_ang, 1), device=-1).export()\n"
+            "print(hashlib.sha1(p.orig.tobytes() + p.batch_off.tobytes() + p.shell_off.tobytes() + p.shells.tobytes()).hexdigest())\n"
+            % ROOT)
+    digests = []
+    for n in ("1", "3", "8"):
+        env = dict(os.environ, OMP_NUM_THREADS=n)
+        out = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, check=True).stdout.strip()
+        digests.append(out)
+    assert len(set(digests)) == 1 and len(digests[0]) == 40
