@@ -325,6 +325,26 @@ def main():
             "plan": {"seconds": res["plan_seconds"], "algorithmic_flops": res["flops"], "sum_nb_nq": stats["sum_nb_nq"],
                      "sum_nb2": stats["sum_nb2"], "nq_hist": res["nq_hist"], "nb_hist": res["nb_hist"], "kind": "global k-d bisection"},
             "E_xc": res["E_xc"], "N_el": res["N_el"], "N_el_rel_err_vs_trPS": res["N_el_rel_err_vs_trPS"]}
+    # reading A1: the timed path is SSF (the paper's choice); the Becke-1988 partition (no compact support,
+    # O(N_A^2) pair terms per point) is timed beside it on the headline workload, same build otherwise
+    if world == 1:
+        try:
+            import torch
+            bplan = xc.Plan.from_workload(w, spec=xc.grid_spec(w.n_rad, w.n_ang, w.functional, partition=1), device=local_rank)
+            Pd = torch.from_numpy(w.P).cuda()
+            Vd = torch.empty_like(Pd)
+            bplan.eval(Pd, Vd)
+            tb = []
+            for _ in range(3):
+                bplan.eval(Pd, Vd)
+                tb.append(bplan.timings())
+            line["becke88"] = {"workload": args.workload, "ms_per_step": statistics.median(t["total_ms"] for t in tb),
+                               "weights_ms": statistics.median(t["weights_ms"] for t in tb),
+                               "points_per_s": res["n_points"] / (statistics.median(t["total_ms"] for t in tb) * 1e-3)}
+            bplan.close()
+            del Pd, Vd
+        except Exception as exc:
+            line["becke88"] = {"error": repr(exc)[:200]}
     if not args.no_cpu_baseline:
         cb = oracle_sample(w, args.workload)
         line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample", "seconds")}
