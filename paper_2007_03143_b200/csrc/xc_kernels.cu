@@ -344,7 +344,39 @@ __global__ void __launch_bounds__(kWeightThreads) k_weights_batched(WeightArgs a
       __syncwarp();
       double sum = 0.0, PA = 0.0;
       const int nsteps = (nC + 31) >> 5;
-      for (int bb = 0; bb < nB; ++bb) {
+      // Becke-88: the parent first (always in full), then the owners nearest to the batch first.  An owner's product is
+      // abandoned as soon as one lane's partial product (an upper bound of P_B: every factor is <= 1) is below 2^-60 of
+      // the sum so far: adding such a term would not change the fp64 sum, so w is bit-identical to the full
+      // O(N_A^2) evaluation in this order.  (SSF gains nothing from this: its factors are exactly 0 or not small.)
+      int ia = -1;
+      if (PART == 1) {
+        for (int c0 = 0; c0 < nC && ia < 0; c0 += 32) {
+          const unsigned m = __ballot_sync(FULL, c0 + lane < nC && sAt[c0 + lane] == A);
+          if (m) ia = c0 + __ffs(m) - 1;
+        }
+      }
+      unsigned premask = 0xffffffffu;
+      for (int ib = (PART == 1 ? -1 : 0); ib < nB; ++ib) {
+        if (PART == 1 && ib >= 0 && (ib & 31) == 0) {
+          // 32 owners at a time, one per lane: the product of the factors against the 8 atoms nearest to the batch is an
+          // upper bound of P_B; below 2^-60 of the sum so far (which only grows) the owner cannot change the sum
+          const int ob = ib + lane;
+          bool keep = ob < nB;
+          if (keep && ob != ia) {
+            const double rO = sD[ob];
+            const double* iRo = a.invR + (size_t)sAt[ob] * a.natoms;
+            double bound = 1.0;
+            const int npre = min(8, nC);
+            for (int k = 0; k < npre; ++k)
+              if (k != ob) bound *= s_becke((rO - sD[k]) * __ldg(iRo + sAt[k]));
+            keep = !(bound < sum * 8.673617379884035e-19);
+          }
+          premask = __ballot_sync(FULL, keep);
+        }
+        const int bb = ib < 0 ? ia : ib;
+        if (PART == 1 && (bb < 0 || (ib >= 0 && bb == ia))) continue;
+        if (PART == 1 && ib >= 0 && !((premask >> (ib & 31)) & 1u)) continue;
+        const double thresh = (PART == 1 && ib >= 0) ? sum * 8.673617379884035e-19 : 0.0;   // 2^-60
         const double rB = sD[bb];
         if (PART == 0 && rB >= kappa * dmin && rB > dmin) continue;           // P_B = 0 exactly
         const int Bid = sAt[bb];
@@ -363,7 +395,16 @@ __global__ void __launch_bounds__(kWeightThreads) k_weights_batched(WeightArgs a
             else if (rC < kappa * rB) part *= s_ssf((rB - rC) * __ldg(iR + sAt[c]));  // else the factor is exactly 1
           }
           if (PART == 0 && (k & 3) == 3 && !__any_sync(FULL, part != 0.0)) break;
+          if (PART == 1 && thresh > 0.0) {                                       // negligible owner?
+            double q = part;                       // after the nearest 32 / 64 partners: the product over all lanes
+            if (k < 2) {
+#pragma unroll
+              for (int o = 16; o >= 1; o >>= 1) q *= __shfl_xor_sync(FULL, q, o);
+            }
+            if (__any_sync(FULL, q < thresh)) { part = -1.0; break; }
+          }
         }
+        if (PART == 1 && part < 0.0) continue;                                  // warp-uniform
 #pragma unroll
         for (int o = 16; o >= 1; o >>= 1) part *= __shfl_xor_sync(FULL, part, o);
         PB *= part;

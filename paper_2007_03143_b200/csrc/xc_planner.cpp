@@ -341,7 +341,6 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
       std::vector<std::pair<double, int32_t>> cand;
 #pragma omp for schedule(dynamic, 64)
       for (int64_t j = 0; j < (int64_t)leaves.size(); ++j) {
-        if (!ssf) continue;  // Becke-88 has no compact support: one shared list of all atoms (below)
         Box b;
         for (int p = 0; p < 3; ++p) { b.lo[p] = 1e300; b.hi[p] = -1e300; }
         for (int64_t k = leaves[j].begin; k < leaves[j].end; ++k)
@@ -353,7 +352,9 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
           U = std::min(U, std::sqrt(d2));
         }
         for (int p = 0; p < 3; ++p) { hp.wbox[6 * j + p] = b.lo[p]; hp.wbox[6 * j + 3 + p] = b.hi[p]; }
-        const double rB = kappa * U * (1.0 + 1e-12) + 1e-12, rC = kappa * rB * (1.0 + 1e-12) + 1e-12;
+        // Becke-88 has no compact support: every atom is an owner and a partner; the list is still sorted by distance to
+        // the box (nearest first), which is what lets the kernel stop an owner's product once it is negligible
+        const double rB = ssf ? kappa * U * (1.0 + 1e-12) + 1e-12 : 1e300, rC = ssf ? kappa * rB * (1.0 + 1e-12) + 1e-12 : 1e300;
         cand.clear();
         for (int a = 0; a < natoms; ++a) {
           double d2 = 0.0;
@@ -391,7 +392,6 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
   hp.batches.resize(nbatch);
   int64_t sh_off = 0, f_off = 0, ppk = 0;
   hp.watoms.clear(); hp.wbatch_small.clear(); hp.wbatch_large.clear(); hp.w_max_small = hp.w_max_large = 0;
-  if (spec->partition != 0) { hp.watoms.resize(natoms); std::iota(hp.watoms.begin(), hp.watoms.end(), 0); }
   for (int64_t j = 0; j < nbatch; ++j) {
     BatchRec& b = hp.batches[j];
     b.pt_off = (int32_t)leaves[j].begin; b.nq = (int32_t)(leaves[j].end - leaves[j].begin);
@@ -399,12 +399,8 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     b.f_off = (int32_t)f_off; b.nb = nbs[j];
     b.ppk_off = ppk;
     ppk += round_up(b.nb, 4) * round_up(b.nb, 8);
-    if (spec->partition == 0) {
-      b.wa_off = (int64_t)hp.watoms.size(); b.wa_nB = wnB[j]; b.wa_nC = (int32_t)wlists[j].size();
-      hp.watoms.insert(hp.watoms.end(), wlists[j].begin(), wlists[j].end());
-    } else {
-      b.wa_off = 0; b.wa_nB = natoms; b.wa_nC = natoms;
-    }
+    b.wa_off = (int64_t)hp.watoms.size(); b.wa_nB = wnB[j]; b.wa_nC = (int32_t)wlists[j].size();
+    hp.watoms.insert(hp.watoms.end(), wlists[j].begin(), wlists[j].end());
     {
       int len = b.wa_nC;
       if (len <= kWeightSmallList) { hp.wbatch_small.push_back((int32_t)j); hp.w_max_small = std::max(hp.w_max_small, len); }

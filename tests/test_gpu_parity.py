@@ -62,6 +62,32 @@ def test_w8_becke_partition(xc, orc):
     plan.close()
 
 
+def test_w27_becke_partition(xc, orc):
+    _, plan, _, _ = _full_parity(orc, "w27", 1, partition=1)
+    plan.close()
+
+
+def test_c2_becke_weights_sampled(xc, orc):
+    """Becke-88 weights at 192 atoms: the kernel stops an owner's cell product once an upper bound of it is below 2^-60
+    of the running sum (bit-identical fp64 sum); the oracle evaluates the full O(N_A^2) products on sampled batches."""
+    import torch
+    w = make_workload("c2")
+    plan = xc.Plan.from_workload(w, spec=xc.grid_spec(w.n_rad, w.n_ang, 0, partition=1))
+    P = torch.from_numpy(w.P).cuda()
+    E, N, V = plan.eval(P)
+    assert abs(N - 2.0 * w.n_occ) / (2.0 * w.n_occ) < 2e-4
+    d = plan.diagnostics()
+    ex = plan.export()
+    rng = np.random.default_rng(5)
+    sub = np.sort(rng.choice(plan.n_batches, 40, replace=False))
+    pidx = np.concatenate([np.arange(ex.batch_off[j], ex.batch_off[j + 1]) for j in sub])
+    ref = orc.partition_weights(w.atoms_xyz, ex.pts[pidx], ex.wq[pidx], ex.parent[pidx], 1, False)
+    assert np.max(np.abs(d["w"][pidx] - ref)) <= 1e-13 * np.max(ex.wq[pidx])
+    E2, N2, V2 = plan.eval(P)
+    assert E2 == E and N2 == N and torch.equal(V, V2)     # bit-identical repeat
+    plan.close()
+
+
 def test_w27_pbe(xc, orc):
     _, plan, _, _ = _full_parity(orc, "w27", 1)
     plan.close()
