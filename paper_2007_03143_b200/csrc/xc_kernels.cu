@@ -512,7 +512,11 @@ __device__ __forceinline__ double ssf_dist(SsfCtx& s, int c0) {
 
 // P_B = prod_C s(mu_BC).  bb = list position of B (warp-uniform, -1: not in the list), rB = r_B.
 // (Bx, By, Bz) is only read for bb < 0; a list atom's coordinates are fetched where the table does not reach.
-__device__ __forceinline__ double ssf_cell_product(SsfCtx& s, int bb, double Bx, double By, double Bz, double rB) {
+// thresh: an owner other than the parent is abandoned (returns 0) as soon as the product over the partners visited so far --
+// an upper bound of P_B, every factor being <= 1 -- is below thresh = 2^-61 of the running sum of the owners before it:
+// adding such a P_B would not change the fp64 sum, so w stays bit-identical.  The bound is formed (one butterfly) after
+// 2, 4, 8, ... visited chunks of the long-list path only; the short-list path is too cheap to pay for it.
+__device__ __forceinline__ double ssf_cell_product(SsfCtx& s, int bb, double Bx, double By, double Bz, double rB, double thresh) {
   const unsigned FULL = 0xffffffffu;
   const double kappa = (1.0 + 0.64) / (1.0 - 0.64);
   const double krB = kappa * rB;
@@ -535,6 +539,14 @@ __device__ __forceinline__ double ssf_cell_product(SsfCtx& s, int bb, double Bx,
     return part * 2.0;
   }
   if (bb >= 0) ssf_atom(s, bb, Bx, By, Bz);
+  int nvis = 0;                                            // chunks that contributed factors
+  auto negligible = [&]() {
+    if (!(thresh > 0.0) || nvis < 2 || (nvis & (nvis - 1))) return false;
+    double q = part;
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) q *= __shfl_xor_sync(FULL, q, o);
+    return q < thresh;                                     // same value in every lane
+  };
   const int nrow = min(nscan, kRcap >> 5);                 // chunks served by the distance row
   for (int ch = 0; ch < nrow; ++ch) {
     const int c0 = ch << 5, c = c0 + s.lane;
@@ -555,6 +567,8 @@ __device__ __forceinline__ double ssf_cell_product(SsfCtx& s, int bb, double Bx,
     if (__any_sync(FULL, zz >= 1.0)) return 0.0;           // s = 0: P_B = 0
     zz = zz < -1.0 ? -1.0 : zz;
     part *= ssf_poly(zz);
+    ++nvis;
+    if (negligible()) return 0.0;
   }
   // partners past the row: r_C and R_BC from one fetch of the coordinates
   for (int ch = nrow; ch < nscan; ++ch) {
@@ -577,6 +591,8 @@ __device__ __forceinline__ double ssf_cell_product(SsfCtx& s, int bb, double Bx,
     if (__any_sync(FULL, zz >= 1.0)) return 0.0;           // s = 0: P_B = 0
     zz = zz < -1.0 ? -1.0 : zz;
     part *= ssf_poly(zz);
+    ++nvis;
+    if (negligible()) return 0.0;
   }
 #pragma unroll
   for (int o = 16; o >= 1; o >>= 1) part *= __shfl_xor_sync(FULL, part, o);
@@ -705,7 +721,7 @@ __global__ void __launch_bounds__(kSsfThreads, 2) k_weights_ssf(WeightArgs a, co
         const unsigned m = __ballot_sync(FULL, c < nC && (c < lcap ? sId[c] : a.watoms[b.wa_off + c]) == A);
         if (m) ia = c0 + __ffs(m) - 1;
       }
-      const double PA = ssf_cell_product(s, ia, Ax, Ay, Az, rA);
+      const double PA = ssf_cell_product(s, ia, Ax, Ay, Az, rA, 0.0);
       if (PA != 0.0) {
         // ---- 3. the other owners ----
         double sum = PA;
@@ -749,7 +765,7 @@ __global__ void __launch_bounds__(kSsfThreads, 2) k_weights_ssf(WeightArgs a, co
             const int src = __ffs(mask) - 1;
             mask &= mask - 1;
             const int bs = b0 + src;
-            sum += ssf_cell_product(s, bs, 0.0, 0.0, 0.0, __shfl_sync(FULL, rB, src));
+            sum += ssf_cell_product(s, bs, 0.0, 0.0, 0.0, __shfl_sync(FULL, rB, src), sum * 4.3368086899420177e-19);   // 2^-61
           }
         }
         result = a.wq[gi] * PA / sum;
