@@ -347,7 +347,7 @@ __global__ void __launch_bounds__(kWeightThreads) k_weights_batched(WeightArgs a
       // Becke-88: the parent first (always in full), then the owners nearest to the batch first.  An owner's product is
       // abandoned as soon as one lane's partial product (an upper bound of P_B: every factor is <= 1) is below 2^-60 of
       // the sum so far: adding such a term would not change the fp64 sum, so w is bit-identical to the full
-      // O(N_A^2) evaluation in this order.  (SSF gains nothing from this: its factors are exactly 0 or not small.)
+      // O(N_A^2) evaluation in this order.  (k_weights_ssf applies the same rule on its long-list path.)
       int ia = -1;
       if (PART == 1) {
         for (int c0 = 0; c0 < nC && ia < 0; c0 += 32) {
