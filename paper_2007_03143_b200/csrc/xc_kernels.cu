@@ -917,6 +917,31 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
   double *sE = sPt + 8 * T, *sN = sPt + 9 * T;
   double *sA = sPt + 10 * T, *sG0 = sPt + 11 * T, *sG1 = sPt + 12 * T, *sG2 = sPt + 13 * T;
 
+  // ---- points with w_i = 0 exactly (SSF zeroes ~10-20 % of them) add exact zeros to E, N_el and V^j: the tiles walk
+  //      over the ordered list of the others (rho / grad rho of the skipped points are not evaluated) ----
+  __shared__ short sLive[kBatchThreads];
+  __shared__ int sLiveCnt[NT / 32];
+  int nqe;
+  {
+    const bool live = tid < b.nq && a.w[(int64_t)b.pt_off + tid] != 0.0;   // N_q^j <= 512 = NT
+    const unsigned lm = __ballot_sync(0xffffffffu, live);
+    if (lane == 0) sLiveCnt[warp] = __popc(lm);
+    __syncthreads();
+    int off = 0;
+    nqe = 0;
+#pragma unroll
+    for (int k = 0; k < NT / 32; ++k) {
+      if (k < warp) off += sLiveCnt[k];
+      nqe += sLiveCnt[k];
+    }
+    if (live) sLive[off + __popc(lm & ((1u << lane) - 1u))] = (short)tid;
+    __syncthreads();
+    if (nqe == 0) {                              // block-uniform
+      if (tid == 0) { a.Epart[bidx] = 0.0; a.Npart[bidx] = 0.0; }
+      return;
+    }
+  }
+
   // ---- per batch: metadata, zero padding rows, V^j block assignment ----
   {
     const int32_t* fidx = a.bfidx + b.f_off;
@@ -937,9 +962,9 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
     }
     for (int k = tid; k < 64; k += NT) sExpT[k] = kExp2Tab[k];
     if (tid < T) {                               // points of the first tile
-      const int64_t gi = (int64_t)b.pt_off + min(tid, b.nq - 1);
+      const int64_t gi = (int64_t)b.pt_off + sLive[min(tid, nqe - 1)];
       sPt[tid] = a.px[gi]; sPt[T + tid] = a.py[gi]; sPt[2 * T + tid] = a.pz[gi];
-      sPt[3 * T + tid] = tid < b.nq ? a.w[gi] : 0.0;
+      sPt[3 * T + tid] = tid < nqe ? a.w[gi] : 0.0;
     }
     __syncthreads();
     // collocation order (shells with the most primitives first, dealt round-robin to the warps) and the
@@ -978,8 +1003,8 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
   double Eacc = 0.0, Nacc = 0.0;
   PH_DECL
   PH(0);
-  for (int t0 = 0, it = 0; t0 < b.nq; t0 += T, ++it) {
-    const int npt = min(T, b.nq - t0);         // valid points in this tile
+  for (int t0 = 0, it = 0; t0 < nqe; t0 += T, ++it) {
+    const int npt = min(T, nqe - t0);          // valid points in this tile
     const double* sx = sPt + (size_t)(it & 1) * 4 * T;   // this tile's points (written one tile ahead)
     const double *sy = sx + T, *sz = sx + 2 * T, *sw = sx + 3 * T;
     __syncthreads();                           // previous tile's readers of sPhi / sZ are done; tables / points visible
@@ -1118,9 +1143,9 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
 
     // ---- 3. functional (Eq. (19)), E and N_el partials (Eq. (16)); the warps after the first T threads fetch
     //         the next tile's points into the other buffer ----
-    if (tid >= T && tid < 2 * T && t0 + T < b.nq) {
-      const int li = tid - T, nn = min(T, b.nq - t0 - T);
-      const int64_t gi = (int64_t)b.pt_off + t0 + T + min(li, nn - 1);
+    if (tid >= T && tid < 2 * T && t0 + T < nqe) {
+      const int li = tid - T, nn = min(T, nqe - t0 - T);
+      const int64_t gi = (int64_t)b.pt_off + sLive[t0 + T + min(li, nn - 1)];
       double* nx = sPt + (size_t)((it + 1) & 1) * 4 * T;
       nx[li] = a.px[gi]; nx[T + li] = a.py[gi]; nx[2 * T + li] = a.pz[gi];
       nx[3 * T + li] = li < nn ? a.w[gi] : 0.0;
@@ -1144,7 +1169,7 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
       const double gs = 2.0 * wi * vs;
       sG0[tid] = gs * gx; sG1[tid] = gs * gy; sG2[tid] = gs * gz;
       if (tid < npt && a.rho_out) {
-        const int64_t gi = (int64_t)b.pt_off + t0 + tid;
+        const int64_t gi = (int64_t)b.pt_off + sLive[t0 + tid];
         a.rho_out[gi] = rho;
         if (a.grho_out) { a.grho_out[3 * gi] = gx; a.grho_out[3 * gi + 1] = gy; a.grho_out[3 * gi + 2] = gz; }
       }

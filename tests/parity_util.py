@@ -43,5 +43,7 @@ def report(g, r, wts=None):
     if wts is not None and g.get("w") is not None:
         out["dw"] = float(np.max(np.abs(g["w"] - wts)) / np.max(np.abs(wts)))
     if g.get("rho") is not None and r.rho is not None:
-        out["drho"] = float(np.max(np.abs(g["rho"] - r.rho)) / np.max(np.abs(r.rho)))
+        # the library does not evaluate rho at points whose weight is exactly 0 (they cannot contribute)
+        m = (g["w"] != 0.0) if g.get("w") is not None else np.ones(len(r.rho), bool)
+        out["drho"] = float(np.max(np.abs(g["rho"][m] - r.rho[m])) / np.max(np.abs(r.rho)))
     return out
