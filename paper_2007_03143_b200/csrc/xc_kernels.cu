@@ -515,7 +515,7 @@ __device__ __forceinline__ double ssf_dist(SsfCtx& s, int c0) {
 // thresh: an owner other than the parent is abandoned (returns 0) as soon as the product over the partners visited so far --
 // an upper bound of P_B, every factor being <= 1 -- is below thresh = 2^-61 of the running sum of the owners before it:
 // adding such a P_B would not change the fp64 sum, so w stays bit-identical.  The bound is formed (one integer warp reduction) after
-// 2, 4, 8, ... visited chunks of the long-list path only; the short-list path is too cheap to pay for it.
+// every visited chunk of the long-list path only; the short-list path is too cheap to pay for it.
 __device__ __forceinline__ double ssf_cell_product(SsfCtx& s, int bb, double Bx, double By, double Bz, double rB, double thresh) {
   const unsigned FULL = 0xffffffffu;
   const double kappa = (1.0 + 0.64) / (1.0 - 0.64);
@@ -541,7 +541,7 @@ __device__ __forceinline__ double ssf_cell_product(SsfCtx& s, int bb, double Bx,
   if (bb >= 0) ssf_atom(s, bb, Bx, By, Bz);
   int nvis = 0;                                            // chunks that contributed factors
   auto negligible = [&]() {
-    if (!(thresh > 0.0) || nvis < 2 || (nvis & (nvis - 1))) return false;
+    if (!(thresh > 0.0)) return false;
     // log2 of the product over the 32 lanes, bounded from ABOVE in fixed point with 10 fractional bits, by one integer
     // warp reduction: for x = m 2^e, m in [1, 2):  e + (m - 1) <= log2 x <= e + (m - 1) + 0.0861.  The high word >> 10 is
     // (e + 1023) 2^10 + the top 10 mantissa bits (truncated: + 1).  The bound is within 2^2.8 of the product; thresh is
