@@ -396,12 +396,9 @@ __global__ void __launch_bounds__(kWeightThreads) k_weights_batched(WeightArgs a
           }
           if (PART == 0 && (k & 3) == 3 && !__any_sync(FULL, part != 0.0)) break;
           if (PART == 1 && thresh > 0.0) {                                       // negligible owner?
-            double q = part;                       // after the nearest 32 / 64 partners: the product over all lanes
-            if (k < 2) {
-#pragma unroll
-              for (int o = 16; o >= 1; o >>= 1) q *= __shfl_xor_sync(FULL, q, o);
-            }
-            if (__any_sync(FULL, q < thresh)) { part = -1.0; break; }
+            // log2 of the product over the lanes bounded from above by one integer warp reduction (see ssf_cell_product)
+            const int ub = __reduce_add_sync(FULL, __double2hiint(part) >> 10) - 32 * (1023 << 10) + 32 * (1 + 89);
+            if (ub < (__double2hiint(thresh) >> 10) - (1023 << 10)) { part = -1.0; break; }
           }
         }
         if (PART == 1 && part < 0.0) continue;                                  // warp-uniform
