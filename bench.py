@@ -155,8 +155,11 @@ def run_workload(name, steps, warmup, functional=None, do_e2e=True, device=0, sa
     # flop count used for every TFLOP/s and roofline figure is the smaller one, 4 (N_b^j)^2 x (live points of batch j)
     wd = plan.diagnostics(want_points=True)["w"]
     live = np.add.reduceat((wd != 0.0).astype(np.int64), ex.batch_off[:-1]) if len(nq) else np.zeros(0, np.int64)
-    res["flops_all_points"] = float(plan.algorithmic_flops)
-    res["flops"] = float(np.sum(4.0 * nbj.astype(np.float64) ** 2 * live))
+    # GGA: X GEMM 2 N_b^2 + V^j (SYR2K triangle) 2 N_b^2 per point; LDA: X over the lower triangle of P^j N_b^2 + V^j (SYRK
+    # triangle) N_b^2 per point
+    per_pt = 4.0 if fn == 1 else 2.0
+    res["flops_all_points"] = float(plan.algorithmic_flops) * per_pt / 4.0
+    res["flops"] = float(np.sum(per_pt * nbj.astype(np.float64) ** 2 * live))
     res["live_point_fraction"] = float(live.sum() / max(1, plan.n_points))
     res["fp64_tflops"] = res["flops"] / (ms * 1e-3) * 1e-12
     res["fp64_frac"] = res["fp64_tflops"] / FP64_PEAK_TFLOPS
@@ -297,8 +300,8 @@ def main():
         except Exception:
             traffic = {}
     # k_xc_batch, bound = FP64 tensor/FMA pipe.  Algorithmic flops of the dense contractions:
-    # X GEMM 2 (N_b^j)^2 N_q^j + V^j 2 (N_b^j)^2 N_q^j (GGA, SYR2K triangle) or (N_b^j)^2 N_q^j (LDA, SYRK triangle)
-    contraction_flops = res["flops"] * (1.0 if gga else 0.75)
+    # GGA 4 (N_b^j)^2, LDA 2 (N_b^j)^2 per point with w != 0 (run_workload)
+    contraction_flops = res["flops"]
     fp64_src = ("FP64 pipe measured live in this run by xc_measure_fp64_peak: DMMA %.2f, DFMA %.2f TFLOP/s "
                 "(nominal %.1f = 148 SM x 64 FMA/clk x 2 x 1.965 GHz)" % (dmma_tf, dfma_tf, FP64_NOMINAL_TFLOPS))
     roofs = {

@@ -243,8 +243,8 @@ int xc_eval(xc_plan* p, const double* dP, int64_t ldp, double* dV, int64_t ldv, 
   ba.Epart = p->d_Epart; ba.Npart = p->d_Npart; ba.vhi = p->d_vhi; ba.vlo = p->d_vlo; ba.nbasis = hp.nbasis;
   ba.rho_tol = hp.spec.rho_tol;
   // P^j pack (Alg. 4 l.4.2), then the fused batch kernel (l.4.3-4.10); large N_b^j first
-  if (!hp.ids_large.empty()) { CU(launch_pack(ba, p->d_ids_large, (int)hp.ids_large.size(), st)); ++launches; }
-  if (!hp.ids_small.empty()) { CU(launch_pack(ba, p->d_ids_small, (int)hp.ids_small.size(), st)); ++launches; }
+  if (!hp.ids_large.empty()) { CU(launch_pack(ba, p->d_ids_large, (int)hp.ids_large.size(), !gga, st)); ++launches; }
+  if (!hp.ids_small.empty()) { CU(launch_pack(ba, p->d_ids_small, (int)hp.ids_small.size(), !gga, st)); ++launches; }
   CU(cudaEventRecord(p->ev[ie++], st));
   if (!hp.ids_large.empty()) { CU(launch_batch(1, gga, ba, p->d_ids_large, (int)hp.ids_large.size(), hp.smem_large, st)); ++launches; }
   if (!hp.ids_small.empty()) { CU(launch_batch(0, gga, ba, p->d_ids_small, (int)hp.ids_small.size(), hp.smem_small, st)); ++launches; }

@@ -783,7 +783,9 @@ __global__ void __launch_bounds__(kSsfThreads, 2) k_weights_ssf(WeightArgs a, co
 // contiguous doubles, lane (g4 = lane >> 2, t4 = lane & 3) holding P[nu = 4 ks + t4][mu = 8 nt + g4];
 // zero padded to nb4 x nb8.  One warp-wide 256-byte load per fragment in the batch kernel, no index math there.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_pack_P(BatchArgs a, const int32_t* __restrict__ batch_ids) {
+// tri (LDA): rho = phi^T P phi = 2 phi^T L phi with L = strict lower triangle of P^j + half its diagonal, so only
+// L is packed (entries nu > mu are zero) and the X GEMM skips the k-steps above the diagonal.
+__global__ void __launch_bounds__(256) k_pack_P(BatchArgs a, const int32_t* __restrict__ batch_ids, int tri) {
   const BatchRec b = a.batches[batch_ids[blockIdx.x]];
   const int nb = b.nb, ntile = (nb + 7) >> 3, nks = (nb + 3) >> 2;
   const int32_t* fidx = a.bfidx + b.f_off;
@@ -795,6 +797,7 @@ __global__ void __launch_bounds__(256) k_pack_P(BatchArgs a, const int32_t* __re
     const int nu = 4 * ks + (lane & 3), mu = 8 * nt + (lane >> 2);
     double v = 0.0;
     if (nu < nb && mu < nb) v = __ldg(a.P + (size_t)fidx[mu] * a.ldp + fidx[nu]);   // P symmetric: row mu is read along nu
+    if (tri) v = nu < mu ? v : (nu == mu ? 0.5 * v : 0.0);
     out[e] = v;
   }
 }
@@ -878,6 +881,50 @@ __device__ __forceinline__ void xgemm_tile(double (&C)[2][NTW][2], const double*
       dmma884(C[1][v][0], C[1][v][1], A1, Bc[v]);
     }
   }
+}
+
+// LDA: X' = L Phi (k_pack_P, tri).  mu-tile mt only has non-zero fragments for the k-steps ks < 2 mt + 2, so the tiles of
+// a warp (mt0, mt0 + WM, ...) drop in one after the other: k-steps [lim_{v-1}, lim_v) run the tiles v .. NV-1, each range
+// with its own fully unrolled loop (no predicated-off DMMA).
+template <int V0, int NV, int NTW, int BS>
+__device__ __forceinline__ void xgemm_seg(double (&C)[2][NTW][2], const double*& Ap, const double*& Bp, int ks_lo, int ks_hi,
+                                          int astep, int bstep) {
+  if (ks_lo >= ks_hi) return;
+  double Bn[NV];
+#pragma unroll
+  for (int v = V0; v < NV; ++v) Bn[v] = __ldg(Bp + v * BS);
+  for (int ks = ks_lo; ks < ks_hi; ++ks) {
+    const double A0 = Ap[0], A1 = Ap[8];
+    double Bc[NV];
+#pragma unroll
+    for (int v = V0; v < NV; ++v) Bc[v] = Bn[v];
+    Ap += astep;
+    Bp += bstep;
+    if (ks + kPfDist < ks_hi) {
+#pragma unroll
+      for (int v = V0; v < NV; ++v) asm volatile("prefetch.global.L1 [%0];" ::"l"(Bp + (size_t)(kPfDist - 1) * bstep + v * BS));
+    }
+    if (ks + 1 < ks_hi) {
+#pragma unroll
+      for (int v = V0; v < NV; ++v) Bn[v] = __ldg(Bp + v * BS);
+    }
+#pragma unroll
+    for (int v = V0; v < NV; ++v) {
+      dmma884(C[0][v][0], C[0][v][1], A0, Bc[v]);
+      dmma884(C[1][v][0], C[1][v][1], A1, Bc[v]);
+    }
+  }
+}
+template <int NV, int NTW, int BS>
+__device__ __forceinline__ void xgemm_tri(double (&C)[2][NTW][2], const double* Ap, const double* Bp, int nks, int mt0, int wmstep,
+                                          int astep, int bstep) {
+  int lim[4];
+#pragma unroll
+  for (int v = 0; v < 4; ++v) lim[v] = v < NV ? min(nks, 2 * (mt0 + v * wmstep) + 2) : nks;
+  xgemm_seg<0, NV, NTW, BS>(C, Ap, Bp, 0, lim[0], astep, bstep);
+  if (NV > 1) xgemm_seg<(NV > 1 ? 1 : 0), NV, NTW, BS>(C, Ap, Bp, lim[0], lim[1], astep, bstep);
+  if (NV > 2) xgemm_seg<(NV > 2 ? 2 : 0), NV, NTW, BS>(C, Ap, Bp, lim[1], lim[2], astep, bstep);
+  if (NV > 3) xgemm_seg<(NV > 3 ? 3 : 0), NV, NTW, BS>(C, Ap, Bp, lim[2], lim[3], astep, bstep);
 }
 
 template <int NT, int T>
@@ -1059,12 +1106,22 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
       // number of mu-tiles of this warp (warp-uniform): one fully unrolled loop per count, so that no DMMA is
       // ever issued predicated-off (a predicated-off DMMA still takes its slot in the FP64 tensor pipe)
       const int nv = wm < ntile ? min(NTW, (ntile - wm + Cfg::WM - 1) / Cfg::WM) : 0;
-      switch (nv) {
-        case 1: xgemm_tile<1, NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
-        case 2: xgemm_tile<(NTW >= 2 ? 2 : 1), NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
-        case 3: xgemm_tile<(NTW >= 3 ? 3 : 1), NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
-        case 4: xgemm_tile<(NTW >= 4 ? 4 : 1), NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
-        default: break;
+      if (GGA) {
+        switch (nv) {
+          case 1: xgemm_tile<1, NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
+          case 2: xgemm_tile<(NTW >= 2 ? 2 : 1), NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
+          case 3: xgemm_tile<(NTW >= 3 ? 3 : 1), NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
+          case 4: xgemm_tile<(NTW >= 4 ? 4 : 1), NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
+          default: break;
+        }
+      } else {                                 // LDA: lower triangle only, rho = 2 Phi . (L Phi)
+        switch (nv) {
+          case 1: xgemm_tri<1, NTW, Cfg::WM * 32>(C, Ap, Bp, nks, wm, Cfg::WM, 4 * LD, ntile * 32); break;
+          case 2: xgemm_tri<(NTW >= 2 ? 2 : 1), NTW, Cfg::WM * 32>(C, Ap, Bp, nks, wm, Cfg::WM, 4 * LD, ntile * 32); break;
+          case 3: xgemm_tri<(NTW >= 3 ? 3 : 1), NTW, Cfg::WM * 32>(C, Ap, Bp, nks, wm, Cfg::WM, 4 * LD, ntile * 32); break;
+          case 4: xgemm_tri<(NTW >= 4 ? 4 : 1), NTW, Cfg::WM * 32>(C, Ap, Bp, nks, wm, Cfg::WM, 4 * LD, ntile * 32); break;
+          default: break;
+        }
       }
       if (GGA) {
         // X^T -> shared memory (the Z buffer, [mu][i]); rows >= nb receive exact zeros (zero padding of the packed P^j)
@@ -1161,6 +1218,7 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
           gz += sRed[(size_t)(q * 4 + 3) * T + tid];
         }
       }
+      if (!GGA) rho *= 2.0;                      // LDA: the X GEMM ran over the lower triangle of P^j (half the diagonal)
       gx *= 2.0; gy *= 2.0; gz *= 2.0;
       const double sigma = gx * gx + gy * gy + gz * gz;
       const double wi = sw[tid];
@@ -1365,9 +1423,9 @@ cudaError_t launch_functional(int kind, int64_t n, const double* rho, const doub
   return cudaGetLastError();
 }
 
-cudaError_t launch_pack(const BatchArgs& a, const int32_t* batch_ids, int nbatches, cudaStream_t st) {
+cudaError_t launch_pack(const BatchArgs& a, const int32_t* batch_ids, int nbatches, bool tri, cudaStream_t st) {
   if (nbatches <= 0) return cudaSuccess;
-  k_pack_P<<<nbatches, 256, 0, st>>>(a, batch_ids);
+  k_pack_P<<<nbatches, 256, 0, st>>>(a, batch_ids, tri ? 1 : 0);
   return cudaGetLastError();
 }
 

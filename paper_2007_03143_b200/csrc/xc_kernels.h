@@ -43,7 +43,7 @@ cudaError_t launch_weights_batched(int partition, const WeightArgs& a, const int
                                    int max_list, cudaStream_t st);
 cudaError_t launch_functional(int kind, int64_t n, const double* rho, const double* sigma, double rho_tol, double* f,
                               double* vr, double* vs, cudaStream_t st);
-cudaError_t launch_pack(const BatchArgs& a, const int32_t* batch_ids, int nbatches, cudaStream_t st);
+cudaError_t launch_pack(const BatchArgs& a, const int32_t* batch_ids, int nbatches, bool tri, cudaStream_t st);
 cudaError_t launch_batch(int cls, bool gga, const BatchArgs& a, const int32_t* batch_ids, int nbatches, size_t smem,
                          cudaStream_t st);
 cudaError_t launch_finalize(int nbasis, const unsigned long long* vhi, const unsigned long long* vlo, double* V,
