@@ -224,6 +224,7 @@ def main():
     ap.add_argument("--also", default="c3,c4,c5,u2,g1", help="comma list of extra workloads reported under other_workloads (or 'none')")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-becke", action="store_true", help="skip the Becke-1988 side measurement")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -340,7 +341,7 @@ def main():
             "E_xc": res["E_xc"], "N_el": res["N_el"], "N_el_rel_err_vs_trPS": res["N_el_rel_err_vs_trPS"]}
     # reading A1: the timed path is SSF (the paper's choice); the Becke-1988 partition (no compact support,
     # O(N_A^2) pair terms per point) is timed beside it on the headline workload, same build otherwise
-    if world == 1:
+    if world == 1 and not args.no_becke:
         try:
             import torch
             bplan = xc.Plan.from_workload(w, spec=xc.grid_spec(w.n_rad, w.n_ang, w.functional, partition=1), device=local_rank)

@@ -59,6 +59,10 @@ typedef struct {
   double  rho_tol;        /* points with rho <= rho_tol contribute nothing (1e-15, reading A12) */
 } xc_grid_spec;
 
+/* flags of xc_eval / xc_eval_host */
+#define XC_EVAL_REUSE_WEIGHTS 1   /* reuse the partition weights of the previous xc_eval on this plan (skip step (a); reading A16) */
+#define XC_EVAL_DIAG          2   /* also store rho and grad rho of every point for xc_eval_diagnostics (parity tests; costs 32 B/point) */
+
 typedef struct xc_plan xc_plan;   /* opaque: owns host + device copies of grid, batches, basis, workspaces */
 
 /* Step (b) of the hot path + all uploads: builds the atom-centred grid (O1-O3), batches the points into
@@ -91,8 +95,13 @@ int xc_plan_export(const xc_plan* plan, double* pts, double* wq, int32_t* parent
  *   dV [device] n_basis x n_basis, leading dimension ldv >= n_basis: OVERWRITTEN (Alg. 2 l.2.4),
  *      both triangles written, exactly symmetric, bit-identical from run to run.
  *   E_xc, N_el [host] scalars, valid when the call returns (the call synchronises the stream once, at the end).
- *   flags: bit 0 = reuse the partition weights of the previous xc_eval on this plan (skip step (a);
- *          "cached-weights build", reading A16); 0 = full build. */
+ *   flags: XC_EVAL_REUSE_WEIGHTS ("cached-weights build", reading A16), XC_EVAL_DIAG; 0 = full build, nothing but the
+ *          three outputs is produced.
+ * The increments of V are summed in 96-bit fixed point whose exponent adapts to the build (the plan remembers it): if a
+ * build's increments do not fit the remembered exponent, steps (c)-(g) are repeated once.  A non-finite value in P (or
+ * produced on the way) is never dropped: E_xc, N_el and all of V come back NaN and the call returns XC_EINVAL.
+ * A plan is not re-entrant: it owns the workspaces of its builds, so two xc_eval calls on ONE plan must not overlap
+ * (different plans may run concurrently).  The caller's current CUDA device is left unchanged. */
 int xc_eval(xc_plan* plan, const double* dP, int64_t ldp, double* dV, int64_t ldv,
             double* E_xc, double* N_el, int32_t flags, void* cuda_stream);
 
@@ -101,7 +110,8 @@ int xc_eval_host(xc_plan* plan, const double* hP, int64_t ldp, double* hV, int64
                  double* E_xc, double* N_el, int32_t flags);
 
 /* Diagnostics of the last xc_eval on this plan, for parity tests at full size.  All [host], may be NULL:
- *   w n_points final partition weights (plan order);  rho n_points;  grad_rho 3*n_points (zeros for LDA);
+ *   w n_points final partition weights (plan order);  rho n_points;  grad_rho 3*n_points (zeros for LDA) -- these two
+ *   only if that xc_eval ran with XC_EVAL_DIAG (else XC_EINVAL), and only at points with w != 0;
  *   E_batch, N_batch n_batches: per-batch partial sums of w f and w rho. */
 int xc_eval_diagnostics(xc_plan* plan, double* w, double* rho, double* grad_rho, double* E_batch, double* N_batch);
 

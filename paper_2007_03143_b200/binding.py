@@ -13,6 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libxc_b200.so")
 
 XC_OK, XC_EINVAL, XC_EUNSUPPORTED, XC_ENOMEM, XC_ECUDA = 0, -1, -2, -3, -4
+XC_EVAL_REUSE_WEIGHTS, XC_EVAL_DIAG = 1, 2
 
 
 class XcAtom(C.Structure):
@@ -169,8 +170,9 @@ class Plan:
                                    shells.ctypes.data_as(C.POINTER(C.c_int32))))
         return PlanExport(pts, wq, parent, orig, boff, soff, shells)
 
-    def eval(self, P, V=None, reuse_weights=False, stream=None):
-        """P, V: torch CUDA float64 tensors (n_basis x n_basis). Returns (E_xc, N_el, V)."""
+    def eval(self, P, V=None, reuse_weights=False, stream=None, diag=False):
+        """P, V: torch CUDA float64 tensors (n_basis x n_basis). Returns (E_xc, N_el, V).
+        diag: also keep rho / grad rho of every point for diagnostics() (XC_EVAL_DIAG)."""
         import torch
         assert P.is_cuda and P.dtype == torch.float64 and P.dim() == 2 and P.stride(1) == 1
         if V is None:
@@ -178,7 +180,8 @@ class Plan:
         assert V.is_cuda and V.dtype == torch.float64 and V.stride(1) == 1
         E, N = C.c_double(), C.c_double()
         _check(_lib.xc_eval(self._h, C.c_void_p(P.data_ptr()), P.stride(0), C.c_void_p(V.data_ptr()), V.stride(0),
-                            C.byref(E), C.byref(N), 1 if reuse_weights else 0, _stream_ptr(stream)))
+                            C.byref(E), C.byref(N), (XC_EVAL_REUSE_WEIGHTS if reuse_weights else 0) | (XC_EVAL_DIAG if diag else 0),
+                            _stream_ptr(stream)))
         return E.value, N.value, V
 
     def eval_host(self, P, V=None, reuse_weights=False):
@@ -191,11 +194,12 @@ class Plan:
         _check(_lib.xc_eval_host(self._h, Pp, ldp, Vp, ldv, C.byref(E), C.byref(N), 1 if reuse_weights else 0))
         return E.value, N.value, V
 
-    def diagnostics(self, want_points=True):
+    def diagnostics(self, want_points=True, want_rho=False):
+        """w (want_points), rho / grad_rho (want_rho: the last eval must have run with diag=True), per-batch E / N_el partials."""
         n, nb = self.n_points, self.n_batches
         w = np.empty(n) if want_points else None
-        rho = np.empty(n) if want_points else None
-        gr = np.empty((n, 3)) if want_points else None
+        rho = np.empty(n) if want_rho else None
+        gr = np.empty((n, 3)) if want_rho else None
         Eb, Nb = np.empty(nb), np.empty(nb)
         _check(_lib.xc_eval_diagnostics(self._h, _dp(w), _dp(rho), _dp(gr), _dp(Eb), _dp(Nb)))
         return dict(w=w, rho=rho, grad_rho=gr, E_batch=Eb, N_batch=Nb)

@@ -5,6 +5,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -28,6 +29,15 @@ int cuda_fail(cudaError_t e, const char* what) {
     if (_e != cudaSuccess) return cuda_fail(_e, #call);  \
   } while (0)
 
+// XC_DEBUG_SYNC=1 in the environment: synchronise after every kernel of xc_eval and name the one that failed
+bool debug_sync() { static const bool on = std::getenv("XC_DEBUG_SYNC") != nullptr; return on; }
+#define CUK(call, st)                                                  \
+  do {                                                                 \
+    cudaError_t _e = (call);                                           \
+    if (_e == cudaSuccess && debug_sync()) _e = cudaStreamSynchronize(st); \
+    if (_e != cudaSuccess) return cuda_fail(_e, #call);                \
+  } while (0)
+
 template <class T>
 int upload(T** dptr, const std::vector<T>& h) {
   *dptr = nullptr;
@@ -49,15 +59,16 @@ struct xc_plan {
   double *d_exps = nullptr, *d_coefs = nullptr;
   BatchRec* d_batches = nullptr;
   int32_t *d_bshells = nullptr, *d_bsfoff = nullptr, *d_bfidx = nullptr, *d_bfinfo = nullptr;
-  double *d_wbox = nullptr;
-  double2* d_pairtab = nullptr;
+  double* d_wbox = nullptr;
   int32_t *d_watoms = nullptr, *d_wsmall = nullptr, *d_wlarge = nullptr;
   int32_t *d_ids_small = nullptr, *d_ids_large = nullptr;
   double* d_ppk = nullptr;
   unsigned long long *d_vhi = nullptr, *d_vlo = nullptr;
-  double *d_Epart = nullptr, *d_Npart = nullptr, *d_result = nullptr;
-  double *d_rho = nullptr, *d_grho = nullptr;
-  double* h_result = nullptr;  // pinned
+  double *d_Epart = nullptr, *d_Npart = nullptr, *d_result = nullptr;   // d_result: E, N_el, then the two flag words of the accumulator
+  double *d_rho = nullptr, *d_grho = nullptr;   // diagnostics, allocated on first use (XC_EVAL_DIAG)
+  bool diag_valid = false;
+  double* h_result = nullptr;  // pinned, 4 doubles
+  int vexp = 0;                // exponent of the fixed-point V accumulator: resolution 2^(vexp - 64), range 2^(vexp + 31)
   double *d_Ptmp = nullptr, *d_Vtmp = nullptr;  // for xc_eval_host
   bool weights_valid = false;
   std::vector<cudaEvent_t> ev;
@@ -65,32 +76,38 @@ struct xc_plan {
   int launches = 0;
 };
 
+struct DeviceGuard {   // the entry points leave the caller's current device as they found it
+  int prev = -1;
+  explicit DeviceGuard(int dev) { if (cudaGetDevice(&prev) != cudaSuccess) prev = -1; if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
 static void free_plan(xc_plan* p) {
   if (!p) return;
   if (p->device < 0) { delete p; return; }
-  cudaSetDevice(p->device);
+  DeviceGuard guard(p->device);
   void* ptrs[] = {p->d_px, p->d_py, p->d_pz, p->d_wq, p->d_w, p->d_parent, p->d_atoms, p->d_invR, p->d_rnn, p->d_shells,
                   p->d_exps, p->d_coefs, p->d_batches, p->d_bshells, p->d_bsfoff, p->d_bfidx, p->d_bfinfo, p->d_ids_small,
                   p->d_ids_large, p->d_ppk, p->d_vhi, p->d_vlo, p->d_Epart, p->d_Npart, p->d_result,
-                  p->d_rho, p->d_grho, p->d_Ptmp, p->d_Vtmp, p->d_watoms, p->d_wsmall, p->d_wlarge, p->d_pairtab, p->d_wbox};
+                  p->d_rho, p->d_grho, p->d_Ptmp, p->d_Vtmp, p->d_watoms, p->d_wsmall, p->d_wlarge, p->d_wbox};
   for (void* q : ptrs) if (q) cudaFree(q);
   if (p->h_result) cudaFreeHost(p->h_result);
   for (cudaEvent_t e : p->ev) cudaEventDestroy(e);
   delete p;
 }
 
-static void atom_tables(const std::vector<double>& atoms, int natoms, std::vector<double>& invR, std::vector<double>& rnn) {
-  invR.assign((size_t)natoms * natoms, 0.0);
-  rnn.assign(natoms, 1e300);
+// [natoms][natoms] table 1 / R_BC, 0 on the diagonal (Becke-88 kernel)
+static void pair_table(const std::vector<double>& atoms, int natoms, std::vector<double>& inv) {
+  inv.assign((size_t)natoms * natoms, 0.0);
+#pragma omp parallel for schedule(static)
   for (int a = 0; a < natoms; ++a)
     for (int b = 0; b < natoms; ++b) {
       if (a == b) continue;
       double dx = atoms[3 * a] - atoms[3 * b], dy = atoms[3 * a + 1] - atoms[3 * b + 1], dz = atoms[3 * a + 2] - atoms[3 * b + 2];
-      double r = std::sqrt(dx * dx + dy * dy + dz * dz);
-      invR[(size_t)a * natoms + b] = 1.0 / r;
-      rnn[a] = std::min(rnn[a], r);
+      inv[(size_t)a * natoms + b] = 1.0 / std::sqrt(dx * dx + dy * dy + dz * dz);
     }
 }
+
 
 extern "C" {
 
@@ -121,8 +138,10 @@ int xc_plan_create(const xc_atom* atoms, int32_t natoms, const xc_shell* shells,
   p->device = device;
   std::string err;
   int rc;
+  std::vector<double> ptab;   // 1 / R_BC (Becke-88 only: the SSF kernel forms its pair terms per tile)
   try {
     rc = build_host_plan(atoms, natoms, shells, nshells, exps, coefs, nprim_total, spec, p->hp, err);
+    if (rc == XC_OK && device != -1 && p->hp.spec.partition == 1) pair_table(p->hp.atoms, p->hp.natoms, ptab);
   } catch (const std::bad_alloc&) {
     rc = XC_ENOMEM; err = "host allocation failed in planner";
   }
@@ -130,17 +149,11 @@ int xc_plan_create(const xc_atom* atoms, int32_t natoms, const xc_shell* shells,
   HostPlan& hp = p->hp;
   if (device == -1) { *out = p; return XC_OK; }   // host-only plan: info / stats / export only
   auto bail = [&](int code) { free_plan(p); return code; };
-  if (cudaSetDevice(device) != cudaSuccess) return bail(fail(XC_ECUDA, "cudaSetDevice failed"));
-  std::vector<double> invR, rnn;
-  atom_tables(hp.atoms, hp.natoms, invR, rnn);
+  DeviceGuard guard(device);
 #define UP(d, h) do { int _r = upload(&p->d, h); if (_r != XC_OK) return bail(_r); } while (0)
   UP(d_px, hp.px); UP(d_py, hp.py); UP(d_pz, hp.pz); UP(d_wq, hp.wq); UP(d_parent, hp.parent);
-  UP(d_atoms, hp.atoms); UP(d_invR, invR); UP(d_rnn, rnn);
-  if (hp.spec.partition == 0) {   // SSF pair table: a R_BC, 1 / (a R_BC)
-    std::vector<double2> tab(invR.size());
-    for (size_t k = 0; k < invR.size(); ++k) tab[k] = invR[k] > 0.0 ? make_double2(0.64 / invR[k], invR[k] / 0.64) : make_double2(0.0, 0.0);
-    UP(d_pairtab, tab);
-  }
+  UP(d_atoms, hp.atoms);
+  UP(d_invR, ptab);
   UP(d_shells, hp.shells); UP(d_exps, hp.exps); UP(d_coefs, hp.coefs);
   UP(d_batches, hp.batches); UP(d_bshells, hp.bshells); UP(d_bsfoff, hp.bsfoff); UP(d_bfidx, hp.bfidx); UP(d_bfinfo, hp.bfinfo);
   UP(d_wbox, hp.wbox);
@@ -151,12 +164,14 @@ int xc_plan_create(const xc_atom* atoms, int32_t natoms, const xc_shell* shells,
   size_t nb2 = (size_t)hp.nbasis * hp.nbasis;
 #define AL(d, bytes) do { cudaError_t _e = cudaMalloc((void**)&p->d, std::max<size_t>((bytes), 8)); if (_e != cudaSuccess) return bail(cuda_fail(_e, "cudaMalloc " #d)); } while (0)
   AL(d_w, hp.npts * 8); AL(d_ppk, (size_t)hp.ppk_doubles * 8);
-  AL(d_vhi, nb2 * 8); AL(d_vlo, nb2 * 8); AL(d_Epart, nitems * 8); AL(d_Npart, nitems * 8); AL(d_result, 16);
-  AL(d_rho, hp.npts * 8); AL(d_grho, hp.npts * 24);
+  AL(d_vhi, nb2 * 8); AL(d_vlo, nb2 * 8); AL(d_Epart, nitems * 8); AL(d_Npart, nitems * 8); AL(d_result, 32);
 #undef AL
+  // SSF: the points the weights kernel never visits (w = w^q exactly) get their weight once, here
+  if (cudaMemcpy(p->d_w, p->d_wq, std::max<size_t>(hp.npts * 8, 8), cudaMemcpyDeviceToDevice) != cudaSuccess)
+    return bail(fail(XC_ECUDA, "cudaMemcpy failed"));
   if (cudaMemset(p->d_Epart, 0, std::max<size_t>(nitems * 8, 8)) != cudaSuccess || cudaMemset(p->d_Npart, 0, std::max<size_t>(nitems * 8, 8)) != cudaSuccess)
     return bail(fail(XC_ECUDA, "cudaMemset failed"));   // batches without functions never write their partials
-  if (cudaMallocHost((void**)&p->h_result, 16) != cudaSuccess) return bail(fail(XC_ENOMEM, "cudaMallocHost failed"));
+  if (cudaMallocHost((void**)&p->h_result, 32) != cudaSuccess) return bail(fail(XC_ENOMEM, "cudaMallocHost failed"));
   p->ev.resize(5);
   for (auto& e : p->ev)
     if (cudaEventCreate(&e) != cudaSuccess) return bail(fail(XC_ECUDA, "cudaEventCreate failed"));
@@ -209,59 +224,91 @@ int xc_eval(xc_plan* p, const double* dP, int64_t ldp, double* dV, int64_t ldv, 
   HostPlan& hp = p->hp;
   if (ldp < hp.nbasis || ldv < hp.nbasis) return fail(XC_EINVAL, "leading dimension smaller than n_basis");
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  CU(cudaSetDevice(p->device));
+  DeviceGuard guard(p->device);
   const bool gga = hp.spec.functional == 1;
+  const bool diag = (flags & XC_EVAL_DIAG) != 0;
   int launches = 0;
   size_t ie = 0;
+  if (diag && !p->d_rho) {
+    CU(cudaMalloc((void**)&p->d_rho, std::max<size_t>(hp.npts * 8, 8)));
+    CU(cudaMalloc((void**)&p->d_grho, std::max<size_t>(hp.npts * 24, 8)));
+  }
   CU(cudaEventRecord(p->ev[ie++], st));
-  if (!(flags & 1) || !p->weights_valid) {
+  if (!(flags & XC_EVAL_REUSE_WEIGHTS) || !p->weights_valid) {
     WeightArgs wa;
-    wa.batches = p->d_batches; wa.watoms = p->d_watoms; wa.atoms = p->d_atoms; wa.invR = p->d_invR; wa.rnn = p->d_rnn;
-    wa.pairtab = p->d_pairtab; wa.wbox = p->d_wbox; wa.natoms = hp.natoms; wa.px = p->d_px; wa.py = p->d_py; wa.pz = p->d_pz; wa.wq = p->d_wq; wa.parent = p->d_parent; wa.w = p->d_w;
-    if (!hp.wbatch_large.empty()) {   // long lists first: they are the long pole
-      CU(launch_weights_batched(hp.spec.partition, wa, p->d_wlarge, (int)hp.wbatch_large.size(), hp.w_warps_large, hp.w_max_large, st));
-      ++launches;
-    }
-    if (!hp.wbatch_small.empty()) {
-      CU(launch_weights_batched(hp.spec.partition, wa, p->d_wsmall, (int)hp.wbatch_small.size(), 8, hp.w_max_small, st));
+    wa.batches = p->d_batches; wa.watoms = p->d_watoms; wa.atoms = p->d_atoms; wa.invR = p->d_invR;
+    wa.wbox = p->d_wbox; wa.natoms = hp.natoms; wa.px = p->d_px; wa.py = p->d_py; wa.pz = p->d_pz; wa.wq = p->d_wq; wa.parent = p->d_parent; wa.w = p->d_w;
+    if (hp.spec.partition == 0) {                          // long lists first: they are the long pole
+      if (!hp.wbatch_large.empty()) { CUK(launch_weights_ssf(wa, p->d_wlarge, (int)hp.wbatch_large.size(), hp.w_max_large, st), st); ++launches; }
+      if (!hp.wbatch_small.empty()) { CUK(launch_weights_ssf(wa, p->d_wsmall, (int)hp.wbatch_small.size(), hp.w_max_small, st), st); ++launches; }
+    } else if (!hp.batches.empty()) {
+      CUK(launch_weights_becke(wa, nullptr, (int)hp.batches.size(), hp.w_warps, hp.w_max_list, st), st);
       ++launches;
     }
     p->weights_valid = true;
   }
   CU(cudaEventRecord(p->ev[ie++], st));
   size_t nb2 = (size_t)hp.nbasis * hp.nbasis;
-  CU(cudaMemsetAsync(p->d_vhi, 0, nb2 * 8, st));
-  CU(cudaMemsetAsync(p->d_vlo, 0, nb2 * 8, st));
-  CU(cudaMemsetAsync(p->d_rho, 0, hp.npts * 8, st));
-  CU(cudaMemsetAsync(p->d_grho, 0, hp.npts * 24, st));
   BatchArgs ba;
   ba.batches = p->d_batches; ba.bshells = p->d_bshells; ba.bsfoff = p->d_bsfoff; ba.bfidx = p->d_bfidx; ba.bfinfo = p->d_bfinfo;
   ba.shells = p->d_shells; ba.exps = p->d_exps; ba.coefs = p->d_coefs;
   ba.px = p->d_px; ba.py = p->d_py; ba.pz = p->d_pz; ba.w = p->d_w;
   ba.P = dP; ba.ldp = ldp; ba.ppk = p->d_ppk;
-  ba.rho_out = p->d_rho; ba.grho_out = gga ? p->d_grho : nullptr;
+  ba.rho_out = diag ? p->d_rho : nullptr; ba.grho_out = (diag && gga) ? p->d_grho : nullptr;
   ba.Epart = p->d_Epart; ba.Npart = p->d_Npart; ba.vhi = p->d_vhi; ba.vlo = p->d_vlo; ba.nbasis = hp.nbasis;
   ba.rho_tol = hp.spec.rho_tol;
+  ba.vflags = (unsigned*)(p->d_result + 2);
+  if (diag) {
+    CU(cudaMemsetAsync(p->d_rho, 0, hp.npts * 8, st));
+    CU(cudaMemsetAsync(p->d_grho, 0, hp.npts * 24, st));
+  }
+  p->diag_valid = diag;
   // P^j pack (Alg. 4 l.4.2), then the fused batch kernel (l.4.3-4.10); large N_b^j first
-  if (!hp.ids_large.empty()) { CU(launch_pack(ba, p->d_ids_large, (int)hp.ids_large.size(), !gga, st)); ++launches; }
-  if (!hp.ids_small.empty()) { CU(launch_pack(ba, p->d_ids_small, (int)hp.ids_small.size(), !gga, st)); ++launches; }
-  CU(cudaEventRecord(p->ev[ie++], st));
-  if (!hp.ids_large.empty()) { CU(launch_batch(1, gga, ba, p->d_ids_large, (int)hp.ids_large.size(), hp.smem_large, st)); ++launches; }
-  if (!hp.ids_small.empty()) { CU(launch_batch(0, gga, ba, p->d_ids_small, (int)hp.ids_small.size(), hp.smem_small, st)); ++launches; }
-  CU(cudaEventRecord(p->ev[ie++], st));
-  CU(launch_finalize(hp.nbasis, p->d_vhi, p->d_vlo, dV, ldv, st));
-  CU(launch_reduce((int64_t)hp.batches.size(), p->d_Epart, p->d_Npart, p->d_result, st));
-  launches += 2;
-  CU(cudaMemcpyAsync(p->h_result, p->d_result, 16, cudaMemcpyDeviceToHost, st));
-  CU(cudaEventRecord(p->ev[ie++], st));
-  CU(cudaStreamSynchronize(st));
+  if (!hp.ids_large.empty()) { CUK(launch_pack(ba, p->d_ids_large, (int)hp.ids_large.size(), !gga, st), st); ++launches; }
+  if (!hp.ids_small.empty()) { CUK(launch_pack(ba, p->d_ids_small, (int)hp.ids_small.size(), !gga, st), st); ++launches; }
+  // The increments of V go to a fixed-point accumulator with resolution 2^(vexp - 64) and range 2^(vexp + 31).  The batch
+  // kernel reports the largest |increment| and whether one was not finite; if the exponent the plan remembers from its last
+  // build does not suit this P (first build with unusually scaled inputs), steps (c)-(g) are repeated once with the right one.
+  for (int attempt = 0;; ++attempt) {
+    ba.vexp = p->vexp;
+    CU(cudaMemsetAsync(p->d_vhi, 0, nb2 * 8, st));
+    CU(cudaMemsetAsync(p->d_vlo, 0, nb2 * 8, st));
+    CU(cudaMemsetAsync(p->d_result + 2, 0, 16, st));
+    if (attempt == 0) CU(cudaEventRecord(p->ev[ie++], st));
+    if (!hp.ids_large.empty()) { CUK(launch_batch(1, gga, ba, p->d_ids_large, (int)hp.ids_large.size(), hp.smem_large, st), st); ++launches; }
+    if (!hp.ids_small.empty()) { CUK(launch_batch(0, gga, ba, p->d_ids_small, (int)hp.ids_small.size(), hp.smem_small, st), st); ++launches; }
+    if (attempt == 0) CU(cudaEventRecord(p->ev[ie++], st));
+    CUK(launch_reduce((int64_t)hp.batches.size(), p->d_Epart, p->d_Npart, p->d_result, st), st);
+    CUK(launch_finalize(hp.nbasis, p->d_vhi, p->d_vlo, dV, ldv, p->vexp, false, st), st);   // speculative: almost always the last word
+    launches += 2;
+    CU(cudaMemcpyAsync(p->h_result, p->d_result, 32, cudaMemcpyDeviceToHost, st));
+    if (attempt == 0) CU(cudaEventRecord(p->ev[ie++], st));
+    CU(cudaStreamSynchronize(st));
+    unsigned vf[4];
+    std::memcpy(vf, p->h_result + 2, 16);
+    const bool poison = vf[1] != 0;
+    if (poison) {
+      CUK(launch_finalize(hp.nbasis, p->d_vhi, p->d_vlo, dV, ldv, p->vexp, true, st), st);
+      CU(cudaStreamSynchronize(st));
+      *E_xc = *N_el = std::nan("");
+      return fail(XC_EINVAL, "non-finite value met while accumulating V (NaN or Inf in P, or overflow); V is filled with NaN");
+    }
+    // vf[0] = high word of the largest |increment| (0: every increment was 0); e = its binary exponent
+    const int e = vf[0] ? (int)(vf[0] >> 20) - 1023 : p->vexp;
+    const bool fits = p->vexp >= e - 10 && p->vexp <= e + 14;
+    if (fits || attempt == 1) {
+      if (!fits) return fail(XC_EUNSUPPORTED, "V increments span more than the fixed-point accumulator covers");
+      break;
+    }
+    p->vexp = e - 8;
+  }
   *E_xc = p->h_result[0];
   *N_el = p->h_result[1];
   // stage timings
   float t;
   p->ms[0] = p->ms[1] = p->ms[2] = p->ms[3] = p->ms[4] = 0.f;
   CU(cudaEventElapsedTime(&t, p->ev[0], p->ev[1])); p->ms[0] = t;
-  CU(cudaEventElapsedTime(&t, p->ev[1], p->ev[2])); p->ms[1] = t;   // includes the memsets
+  CU(cudaEventElapsedTime(&t, p->ev[1], p->ev[2])); p->ms[1] = t;   // includes zeroing the accumulators
   CU(cudaEventElapsedTime(&t, p->ev[2], p->ev[3])); p->ms[2] = t;
   CU(cudaEventElapsedTime(&t, p->ev[3], p->ev[4])); p->ms[3] = t;
   CU(cudaEventElapsedTime(&t, p->ev[0], p->ev[4])); p->ms[4] = t;
@@ -274,7 +321,7 @@ int xc_eval_host(xc_plan* p, const double* hP, int64_t ldp, double* hV, int64_t 
   if (p->device < 0) return fail(XC_ECUDA, "host-only plan (device = -1): no CUDA device bound, and there is no CPU fallback");
   const int n = p->hp.nbasis;
   if (ldp < n || ldv < n) return fail(XC_EINVAL, "leading dimension smaller than n_basis");
-  CU(cudaSetDevice(p->device));
+  DeviceGuard guard(p->device);
   size_t bytes = (size_t)n * n * 8;
   if (!p->d_Ptmp) CU(cudaMalloc((void**)&p->d_Ptmp, bytes));
   if (!p->d_Vtmp) CU(cudaMalloc((void**)&p->d_Vtmp, bytes));
@@ -289,7 +336,8 @@ int xc_eval_diagnostics(xc_plan* p, double* w, double* rho, double* grad_rho, do
   if (!p) return fail(XC_EINVAL, "plan is null");
   if (p->device < 0) return fail(XC_ECUDA, "host-only plan (device = -1)");
   const HostPlan& hp = p->hp;
-  CU(cudaSetDevice(p->device));
+  if ((rho || grad_rho) && !p->diag_valid) return fail(XC_EINVAL, "rho / grad_rho need the last xc_eval to have run with XC_EVAL_DIAG");
+  DeviceGuard guard(p->device);
   CU(cudaDeviceSynchronize());
   if (w) CU(cudaMemcpy(w, p->d_w, hp.npts * 8, cudaMemcpyDeviceToHost));
   if (rho) CU(cudaMemcpy(rho, p->d_rho, hp.npts * 8, cudaMemcpyDeviceToHost));
@@ -330,20 +378,87 @@ int xc_partition_weights(const xc_atom* atoms, int32_t natoms, int32_t partition
   if (!atoms || natoms < 1 || npts < 0 || (npts && (!dx || !dy || !dz || !dwq || !dparent || !dw_out)))
     return fail(XC_EINVAL, "bad argument");
   if (partition < 0 || partition > 1) return fail(XC_EINVAL, "bad partition enum");
-  std::vector<double> a(3 * (size_t)natoms), invR, rnn;
-  for (int i = 0; i < natoms; ++i) { a[3 * i] = atoms[i].x; a[3 * i + 1] = atoms[i].y; a[3 * i + 2] = atoms[i].z; }
-  atom_tables(a, natoms, invR, rnn);
-  double *da = nullptr, *di = nullptr, *dr = nullptr;
-  int rc = upload(&da, a);
-  if (rc == XC_OK) rc = upload(&di, invR);
-  if (rc == XC_OK) rc = upload(&dr, rnn);
+  if (npts >= ((int64_t)1 << 31)) return fail(XC_EUNSUPPORTED, "more than 2^31 points");
+  if (npts == 0) return XC_OK;
+  // The kernels of xc_eval on an ad-hoc plan: pseudo-batches of 512 consecutive points, each with the bounding box of its
+  // points and its own atom list (exact SSF support / every atom for Becke-88, sorted by distance to the box), no point
+  // pre-classified as trivial.
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int64_t nbatch = (npts + 511) / 512;
+  std::vector<double> a, ptab, box, hx, hy, hz;
+  std::vector<int32_t> watoms, ids_small, ids_large;
+  std::vector<BatchRec> recs;
+  int nwarps = 8, max_small = 0, max_large = 0, max_list = 0;
+  try {
+    a.resize(3 * (size_t)natoms);
+    for (int i = 0; i < natoms; ++i) {
+      a[3 * i] = atoms[i].x; a[3 * i + 1] = atoms[i].y; a[3 * i + 2] = atoms[i].z;
+      if (!std::isfinite(atoms[i].x) || !std::isfinite(atoms[i].y) || !std::isfinite(atoms[i].z)) return fail(XC_EINVAL, "non-finite atom coordinate");
+    }
+    for (int i = 0; i < natoms; ++i)
+      for (int j = 0; j < i; ++j)
+        if (a[3 * i] == a[3 * j] && a[3 * i + 1] == a[3 * j + 1] && a[3 * i + 2] == a[3 * j + 2]) return fail(XC_EINVAL, "two atoms coincide");
+    if (partition == 1) pair_table(a, natoms, ptab);
+    hx.resize(npts); hy.resize(npts); hz.resize(npts);
+    CU(cudaStreamSynchronize(st));
+    CU(cudaMemcpy(hx.data(), dx, npts * 8, cudaMemcpyDeviceToHost));
+    CU(cudaMemcpy(hy.data(), dy, npts * 8, cudaMemcpyDeviceToHost));
+    CU(cudaMemcpy(hz.data(), dz, npts * 8, cudaMemcpyDeviceToHost));
+    recs.resize((size_t)nbatch);
+    box.assign(6 * (size_t)nbatch, 0.0);
+    std::vector<int32_t> lst;
+    for (int64_t j = 0; j < nbatch; ++j) {
+      BatchRec& b = recs[(size_t)j];
+      std::memset(&b, 0, sizeof(b));
+      b.pt_off = (int32_t)(j * 512); b.nq = (int32_t)std::min<int64_t>(512, npts - j * 512);
+      double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+      for (int64_t k = b.pt_off; k < (int64_t)b.pt_off + b.nq; ++k) {
+        if (!std::isfinite(hx[k]) || !std::isfinite(hy[k]) || !std::isfinite(hz[k])) return fail(XC_EINVAL, "non-finite point coordinate");
+        lo[0] = std::min(lo[0], hx[k]); hi[0] = std::max(hi[0], hx[k]);
+        lo[1] = std::min(lo[1], hy[k]); hi[1] = std::max(hi[1], hy[k]);
+        lo[2] = std::min(lo[2], hz[k]); hi[2] = std::max(hi[2], hz[k]);
+      }
+      for (int q = 0; q < 3; ++q) { box[6 * j + q] = lo[q]; box[6 * j + 3 + q] = hi[q]; }
+      int nB = 0;
+      weight_atom_list(a.data(), natoms, lo, hi, partition == 0, lst, nB);
+      b.wa_off = (int64_t)watoms.size(); b.wa_nB = nB; b.wa_nC = (int32_t)lst.size();
+      watoms.insert(watoms.end(), lst.begin(), lst.end());
+      max_list = std::max(max_list, (int)lst.size());
+      if ((int)lst.size() <= kWeightSmallList) { ids_small.push_back((int32_t)j); max_small = std::max(max_small, (int)lst.size()); }
+      else { ids_large.push_back((int32_t)j); max_large = std::max(max_large, (int)lst.size()); }
+    }
+    if (partition == 1) {
+      while (nwarps > 1 && weights_smem_bytes(max_list, nwarps) > kSmemLimit) nwarps >>= 1;
+      if (weights_smem_bytes(max_list, nwarps) > kSmemLimit) return fail(XC_EUNSUPPORTED, "too many atoms for the Becke-88 weights kernel");
+    }
+  } catch (const std::bad_alloc&) {
+    return fail(XC_ENOMEM, "host allocation failed");
+  }
+  double *da = nullptr, *dt = nullptr, *dbox = nullptr;
+  int32_t *dl = nullptr, *dsm = nullptr, *dlg = nullptr;
+  BatchRec* db = nullptr;
+  int rc = upload(&da, a);
+  if (rc == XC_OK) rc = upload(&dt, ptab);
+  if (rc == XC_OK) rc = upload(&dbox, box);
+  if (rc == XC_OK) rc = upload(&dl, watoms);
+  if (rc == XC_OK) rc = upload(&db, recs);
+  if (rc == XC_OK) rc = upload(&dsm, ids_small);
+  if (rc == XC_OK) rc = upload(&dlg, ids_large);
   if (rc == XC_OK) {
-    cudaError_t e = launch_weights(partition, natoms, da, di, dr, npts, dx, dy, dz, dwq, dparent, dw_out, st);
+    WeightArgs wa;
+    wa.batches = db; wa.watoms = dl; wa.atoms = da; wa.invR = dt; wa.wbox = dbox; wa.natoms = natoms;
+    wa.px = dx; wa.py = dy; wa.pz = dz; wa.wq = dwq; wa.parent = dparent; wa.w = dw_out;
+    cudaError_t e = cudaSuccess;
+    if (partition == 0) {
+      if (!ids_large.empty()) e = launch_weights_ssf(wa, dlg, (int)ids_large.size(), max_large, st);
+      if (e == cudaSuccess && !ids_small.empty()) e = launch_weights_ssf(wa, dsm, (int)ids_small.size(), max_small, st);
+    } else {
+      e = launch_weights_becke(wa, nullptr, (int)nbatch, nwarps, max_list, st);
+    }
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) rc = cuda_fail(e, "xc_partition_weights");
   }
-  cudaFree(da); cudaFree(di); cudaFree(dr);
+  cudaFree(da); cudaFree(dt); cudaFree(dbox); cudaFree(dl); cudaFree(db); cudaFree(dsm); cudaFree(dlg);
   return rc;
 }
 

@@ -15,8 +15,8 @@ constexpr int kBatchThreads = 512;  // 16 warps per batch CTA
 constexpr int kSmallNb = 112;   // N_b^j limit of the 64-point-tile instantiation (<= 28 lower-triangle 16x16 blocks = 2 per warp of 16)
 constexpr int kMaxNb = 192;     // N_b^j limit of the batch kernel (<= 78 blocks = 5 per warp); the planner splits larger batches
 constexpr size_t kSmemLimit = 227 * 1024;
-constexpr int kWeightSmallList = 192; // atom-list length that separates the two launches of the weights kernel
-constexpr int kWeightThreads = 256;
+constexpr int kWeightThreads = 256;  // Becke-88 weights kernel: 8 warps per batch CTA
+constexpr int kWeightSmallList = 192; // SSF weights kernel: atom-list length that separates its two launches
 
 struct ShellRec {      // 48 bytes
   double x, y, z;      // centre
@@ -31,7 +31,10 @@ struct BatchRec {      // one quadrature batch B_j with its shell list S_j (PAPE
   int64_t ppk_off;             // offset (doubles) of this batch's packed P^j (nb4 x nb8, DMMA fragment order)
   int64_t wa_off;              // offset into the weight-kernel atom lists
   int32_t wa_nB, wa_nC;        // atoms that can own weight here / atoms that can appear in a cell product
+  int32_t ntriv, _pad;         // SSF: the first ntriv points of the batch have w = w^q exactly (r_A < (1-a)/2 R_nn(A))
 };
+
+
 
 inline int ncart(int L) { return (L + 1) * (L + 2) / 2; }
 inline int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
@@ -39,6 +42,8 @@ inline int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
 // shared-memory footprint of the batch kernel for a batch (bytes); T = points per tile
 size_t batch_smem_bytes(int T, bool gga, int nb, int ns, int npr, int nthreads);   // npr: primitives of the batch's shells
 size_t weights_smem_bytes(int nC, int warps);
+// atom list of the weights kernels for the box [lo, hi] of points: owners = out[0 .. nB), partners = all of out (sorted by distance to the box)
+void weight_atom_list(const double* atoms, int natoms, const double lo[3], const double hi[3], bool ssf, std::vector<int32_t>& out, int& nB);
 
 struct HostPlan {
   int natoms = 0, nshells = 0, nbasis = 0, nprim = 0;
@@ -57,8 +62,10 @@ struct HostPlan {
   std::vector<int32_t> bfinfo;         // per local function: (local shell slot << 8) | (l<<4 | m<<2 | n)
   std::vector<int32_t> watoms;         // concatenated per-batch atom lists of the weights kernel (sorted by distance to the batch box)
   std::vector<double> wbox;            // [nbatch][6] tight bounding boxes
-  std::vector<int32_t> wbatch_small, wbatch_large;  // batch ids by list length (two launches)
-  int w_max_small = 0, w_max_large = 0, w_warps_large = 8;
+  std::vector<int32_t> wbatch_small, wbatch_large;  // SSF weights kernel: batches with non-trivial points, by list length (two launches)
+  int w_max_small = 0, w_max_large = 0;
+  std::vector<double> rnn;             // nearest-neighbour distance of every atom
+  int w_max_list = 0, w_warps = 8;     // Becke-88 weights kernel: longest atom list, warps per CTA that fit in shared memory
   std::vector<int32_t> ids_small, ids_large;  // batch-kernel work lists (N_b^j <= kSmallNb / the others), heaviest first
   int64_t ppk_doubles = 0;              // size of the packed-P^j buffer
   double sum_nbnq = 0, sum_nb2 = 0, flops = 0;

@@ -20,7 +20,9 @@ struct BatchArgs {
   double* ppk;                         // packed P^j of every batch (DMMA B-fragment order)
   double* rho_out; double* grho_out;   // optional diagnostics (may be null)
   double* Epart; double* Npart;        // one partial per batch
-  unsigned long long* vhi; unsigned long long* vlo;   // fixed-point V accumulator (lower triangle)
+  unsigned long long* vhi; unsigned long long* vlo;   // fixed-point V accumulator (lower triangle), value = (hi 2^32 + lo) 2^(vexp - 64)
+  int vexp;
+  unsigned* vflags;                    // [0] high word of the largest |increment| of V, [1] != 0: a non-finite increment was met
   int nbasis;
   double rho_tol;
 };
@@ -28,26 +30,25 @@ struct BatchArgs {
 struct WeightArgs {
   const BatchRec* batches;
   const int32_t* watoms;
-  const double* atoms; const double* invR; const double* rnn;
-  const double2* pairtab;  // [natoms][natoms]: a R_BC, 1 / (a R_BC)  (a = 0.64, SSF)
-  const double* wbox;   // [nbatch][6] tight bounding boxes (lo xyz, hi xyz)
+  const double* atoms;
+  const double* invR;    // [natoms][natoms] 1 / R_BC (Becke-88), 0 on the diagonal
+  const double* wbox;    // [nbatch][6] tight bounding boxes (lo xyz, hi xyz)
   int natoms;
   const double* px; const double* py; const double* pz; const double* wq; const int32_t* parent;
   double* w;
 };
 
-cudaError_t launch_weights(int partition, int natoms, const double* atoms, const double* invR, const double* rnn,
-                           int64_t npts, const double* px, const double* py, const double* pz, const double* wq,
-                           const int32_t* parent, double* w, cudaStream_t st);
-cudaError_t launch_weights_batched(int partition, const WeightArgs& a, const int32_t* batch_ids, int nbatches, int nwarps,
-                                   int max_list, cudaStream_t st);
+// SSF: one CTA per batch, one warp per non-trivial point; max_list = longest atom list among the batches launched
+cudaError_t launch_weights_ssf(const WeightArgs& a, const int32_t* batch_ids, int nbatches, int max_list, cudaStream_t st);
+// Becke-88: one CTA per batch (batch_ids may be null: batch = block index)
+cudaError_t launch_weights_becke(const WeightArgs& a, const int32_t* batch_ids, int nbatches, int nwarps, int max_list, cudaStream_t st);
 cudaError_t launch_functional(int kind, int64_t n, const double* rho, const double* sigma, double rho_tol, double* f,
                               double* vr, double* vs, cudaStream_t st);
 cudaError_t launch_pack(const BatchArgs& a, const int32_t* batch_ids, int nbatches, bool tri, cudaStream_t st);
 cudaError_t launch_batch(int cls, bool gga, const BatchArgs& a, const int32_t* batch_ids, int nbatches, size_t smem,
                          cudaStream_t st);
 cudaError_t launch_finalize(int nbasis, const unsigned long long* vhi, const unsigned long long* vlo, double* V,
-                            int64_t ldv, cudaStream_t st);
+                            int64_t ldv, int vexp, bool poison, cudaStream_t st);
 cudaError_t launch_reduce(int64_t n, const double* ep, const double* np, double* out, cudaStream_t st);
 
 }  // namespace xcb

@@ -112,6 +112,38 @@ size_t batch_smem_bytes(int T, bool gga, int nb, int ns, int npr, int nthreads) 
 
 size_t weights_smem_bytes(int nC, int warps) { return (size_t)nC * (24 + 4) + (size_t)warps * nC * 8 + 64; }
 
+// Atom list of the weights kernels for a box of points (step (a)), exact SSF compact support, sorted by
+// distance to the box.  U = min_C dmax(C, box) bounds r_min of every point of the box from above.  An atom B can own weight
+// at some point only if r_B < kappa r_min <= kappa U, and a factor s(mu_BC) differs from 1 only if r_C < kappa r_B < kappa^2 U.
+// With dmin(., box) <= r_. the lists {dmin < kappa U} (owners: the first nB) and {dmin < kappa^2 U} (partners: all) are
+// supersets.  Becke-88 has no compact support: every atom is an owner and a partner; the order (nearest first) is what
+// lets that kernel stop an owner's product once it is negligible.
+void weight_atom_list(const double* atoms, int natoms, const double lo[3], const double hi[3], bool ssf, std::vector<int32_t>& out, int& nB) {
+  const double a_ssf = 0.64, kappa = (1.0 + a_ssf) / (1.0 - a_ssf);
+  double U = 1e300;
+  for (int a = 0; a < natoms; ++a) {
+    double d2 = 0.0;
+    for (int p = 0; p < 3; ++p) { double t = std::max(std::fabs(atoms[3 * a + p] - lo[p]), std::fabs(atoms[3 * a + p] - hi[p])); d2 += t * t; }
+    U = std::min(U, std::sqrt(d2));
+  }
+  const double rB = ssf ? kappa * U * (1.0 + 1e-12) + 1e-12 : 1e300, rC = ssf ? kappa * rB * (1.0 + 1e-12) + 1e-12 : 1e300;
+  std::vector<std::pair<double, int32_t>> cand;
+  for (int a = 0; a < natoms; ++a) {
+    double d2 = 0.0;
+    for (int p = 0; p < 3; ++p) {
+      double c = atoms[3 * a + p];
+      double t = c < lo[p] ? lo[p] - c : (c > hi[p] ? c - hi[p] : 0.0);
+      d2 += t * t;
+    }
+    double d = std::sqrt(d2);
+    if (d <= rC) cand.push_back({d, a});
+  }
+  std::sort(cand.begin(), cand.end());
+  out.resize(cand.size());
+  nB = 0;
+  for (size_t k = 0; k < cand.size(); ++k) { out[k] = cand[k].second; if (cand[k].first <= rB) nB = (int)k + 1; }
+}
+
 int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, int nshells, const double* exps,
                     const double* coefs, int nprim_total, const xc_grid_spec* spec, HostPlan& hp, std::string& err) {
   if (!atoms || !shells || !exps || !coefs || !spec) { err = "null argument"; return XC_EINVAL; }
@@ -125,6 +157,25 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
   hp.natoms = natoms; hp.nshells = nshells; hp.nprim = nprim_total; hp.spec = *spec;
   hp.atoms.resize(3 * (size_t)natoms);
   for (int a = 0; a < natoms; ++a) { hp.atoms[3 * a] = atoms[a].x; hp.atoms[3 * a + 1] = atoms[a].y; hp.atoms[3 * a + 2] = atoms[a].z; }
+  for (double v : hp.atoms)
+    if (!std::isfinite(v)) { err = "non-finite atom coordinate"; return XC_EINVAL; }
+  // nearest-neighbour distances (SSF "trivial point" rule); coincident centres make mu_BC undefined
+  hp.rnn.assign(natoms, 1e300);
+  {
+    bool coincident = false;
+#pragma omp parallel for schedule(static) reduction(|| : coincident)
+    for (int a = 0; a < natoms; ++a) {
+      double m = 1e300;
+      for (int b = 0; b < natoms; ++b) {
+        if (b == a) continue;
+        const double dx = hp.atoms[3 * a] - hp.atoms[3 * b], dy = hp.atoms[3 * a + 1] - hp.atoms[3 * b + 1], dz = hp.atoms[3 * a + 2] - hp.atoms[3 * b + 2];
+        m = std::min(m, std::sqrt(dx * dx + dy * dy + dz * dz));
+      }
+      hp.rnn[a] = m;
+      if (!(m > 1e-8)) coincident = true;
+    }
+    if (coincident) { err = "two atoms coincide (R_AB < 1e-8 bohr)"; return XC_EINVAL; }
+  }
   hp.exps.assign(exps, exps + nprim_total);
   hp.coefs.assign(coefs, coefs + nprim_total);
   for (int k = 0; k < nprim_total; ++k)
@@ -326,6 +377,24 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     }
   }
 
+  // ---- SSF: points with r_A < (1-a)/2 R_nn(A) have w = w^q exactly (every mu_AC <= -a).  They come first in their
+  //      batch (each group keeps its Morton order); the weights kernel only visits the others ----
+  std::vector<int32_t> ntriv(leaves.size(), 0);
+  if (spec->partition == 0) {
+    const double lim = 0.5 * (1.0 - 0.64);
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t j = 0; j < (int64_t)leaves.size(); ++j) {
+      auto trivial = [&](int64_t p) {
+        if (natoms == 1) return true;
+        const int a = (int)(p / per_atom);
+        const double dx = cx[p] - hp.atoms[3 * a], dy = cy[p] - hp.atoms[3 * a + 1], dz = cz[p] - hp.atoms[3 * a + 2];
+        return std::sqrt(dx * dx + dy * dy + dz * dz) < lim * hp.rnn[a];
+      };
+      auto mid = std::stable_partition(idx.begin() + leaves[j].begin, idx.begin() + leaves[j].end, trivial);
+      ntriv[j] = (int32_t)(mid - (idx.begin() + leaves[j].begin));
+    }
+  }
+
   // ---- atom lists of the weights kernel (step (a)), exact SSF compact support ----
   // U = min_C dmax(C, box) bounds r_min of every point of the batch from above.  An atom B can own weight at some
   // point only if r_B < kappa r_min <= kappa U, and a factor s(mu_BC) differs from 1 only if r_C < kappa r_B < kappa^2 U.
@@ -333,46 +402,13 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
   hp.wbox.assign(6 * leaves.size(), 0.0);
   std::vector<std::vector<int32_t>> wlists(leaves.size());
   std::vector<int> wnB(leaves.size(), 0);
-  {
-    const double a_ssf = 0.64, kappa = (1.0 + a_ssf) / (1.0 - a_ssf);
-    const bool ssf = spec->partition == 0;
-#pragma omp parallel
-    {
-      std::vector<std::pair<double, int32_t>> cand;
-#pragma omp for schedule(dynamic, 64)
-      for (int64_t j = 0; j < (int64_t)leaves.size(); ++j) {
-        Box b;
-        for (int p = 0; p < 3; ++p) { b.lo[p] = 1e300; b.hi[p] = -1e300; }
-        for (int64_t k = leaves[j].begin; k < leaves[j].end; ++k)
-          for (int p = 0; p < 3; ++p) { double v = coord[p][idx[k]]; b.lo[p] = std::min(b.lo[p], v); b.hi[p] = std::max(b.hi[p], v); }
-        double U = 1e300;
-        for (int a = 0; a < natoms; ++a) {
-          double d2 = 0.0;
-          for (int p = 0; p < 3; ++p) { double t = std::max(std::fabs(hp.atoms[3 * a + p] - b.lo[p]), std::fabs(hp.atoms[3 * a + p] - b.hi[p])); d2 += t * t; }
-          U = std::min(U, std::sqrt(d2));
-        }
-        for (int p = 0; p < 3; ++p) { hp.wbox[6 * j + p] = b.lo[p]; hp.wbox[6 * j + 3 + p] = b.hi[p]; }
-        // Becke-88 has no compact support: every atom is an owner and a partner; the list is still sorted by distance to
-        // the box (nearest first), which is what lets the kernel stop an owner's product once it is negligible
-        const double rB = ssf ? kappa * U * (1.0 + 1e-12) + 1e-12 : 1e300, rC = ssf ? kappa * rB * (1.0 + 1e-12) + 1e-12 : 1e300;
-        cand.clear();
-        for (int a = 0; a < natoms; ++a) {
-          double d2 = 0.0;
-          for (int p = 0; p < 3; ++p) {
-            double c = hp.atoms[3 * a + p];
-            double t = c < b.lo[p] ? b.lo[p] - c : (c > b.hi[p] ? c - b.hi[p] : 0.0);
-            d2 += t * t;
-          }
-          double d = std::sqrt(d2);
-          if (d <= rC) cand.push_back({d, a});
-        }
-        std::sort(cand.begin(), cand.end());
-        wlists[j].resize(cand.size());
-        int nB = 0;
-        for (size_t k = 0; k < cand.size(); ++k) { wlists[j][k] = cand[k].second; if (cand[k].first <= rB) nB = (int)k + 1; }
-        wnB[j] = nB;
-      }
-    }
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t j = 0; j < (int64_t)leaves.size(); ++j) {
+    double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+    for (int64_t k = leaves[j].begin; k < leaves[j].end; ++k)
+      for (int p = 0; p < 3; ++p) { double v = coord[p][idx[k]]; lo[p] = std::min(lo[p], v); hi[p] = std::max(hi[p], v); }
+    for (int p = 0; p < 3; ++p) { hp.wbox[6 * j + p] = lo[p]; hp.wbox[6 * j + 3 + p] = hi[p]; }
+    weight_atom_list(hp.atoms.data(), natoms, lo, hi, spec->partition == 0, wlists[j], wnB[j]);
   }
 
   // ---- permuted point arrays ----
@@ -391,7 +427,7 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
   const int64_t nbatch = (int64_t)leaves.size();
   hp.batches.resize(nbatch);
   int64_t sh_off = 0, f_off = 0, ppk = 0;
-  hp.watoms.clear(); hp.wbatch_small.clear(); hp.wbatch_large.clear(); hp.w_max_small = hp.w_max_large = 0;
+  hp.watoms.clear(); hp.wbatch_small.clear(); hp.wbatch_large.clear(); hp.w_max_small = hp.w_max_large = hp.w_max_list = 0;
   for (int64_t j = 0; j < nbatch; ++j) {
     BatchRec& b = hp.batches[j];
     b.pt_off = (int32_t)leaves[j].begin; b.nq = (int32_t)(leaves[j].end - leaves[j].begin);
@@ -401,8 +437,10 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     ppk += round_up(b.nb, 4) * round_up(b.nb, 8);
     b.wa_off = (int64_t)hp.watoms.size(); b.wa_nB = wnB[j]; b.wa_nC = (int32_t)wlists[j].size();
     hp.watoms.insert(hp.watoms.end(), wlists[j].begin(), wlists[j].end());
-    {
-      int len = b.wa_nC;
+    hp.w_max_list = std::max(hp.w_max_list, (int)b.wa_nC);
+    b.ntriv = ntriv[j]; b._pad = 0;
+    if (spec->partition == 0 && b.ntriv < b.nq) {          // SSF: batches whose points are all trivial need no kernel
+      const int len = b.wa_nC;
       if (len <= kWeightSmallList) { hp.wbatch_small.push_back((int32_t)j); hp.w_max_small = std::max(hp.w_max_small, len); }
       else { hp.wbatch_large.push_back((int32_t)j); hp.w_max_large = std::max(hp.w_max_large, len); }
     }
@@ -453,9 +491,9 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
   std::stable_sort(hp.ids_large.begin(), hp.ids_large.end(), [&](int32_t x, int32_t y) { return cost(x) > cost(y); });
   // Becke-88 weights launch: warps per CTA such that the per-warp distance rows fit in shared memory
   // (the SSF kernel has a fixed footprint and reads list entries beyond its cache from global memory)
-  hp.w_warps_large = 8;
-  while (spec->partition != 0 && hp.w_warps_large > 1 && weights_smem_bytes(hp.w_max_large, hp.w_warps_large) > kSmemLimit) hp.w_warps_large >>= 1;
-  if (spec->partition != 0 && weights_smem_bytes(hp.w_max_large, hp.w_warps_large) > kSmemLimit) {
+  hp.w_warps = 8;
+  while (spec->partition != 0 && hp.w_warps > 1 && weights_smem_bytes(hp.w_max_list, hp.w_warps) > kSmemLimit) hp.w_warps >>= 1;
+  if (spec->partition != 0 && weights_smem_bytes(hp.w_max_list, hp.w_warps) > kSmemLimit) {
     err = "too many atoms for the Becke-88 weights kernel"; return XC_EUNSUPPORTED;
   }
   return XC_OK;

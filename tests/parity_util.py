@@ -21,9 +21,9 @@ def run_gpu(w, functional=None, P=None, want_points=True, **spec_kw):
     spec = xc.grid_spec(w.n_rad, w.n_ang, fn, **spec_kw)
     plan = xc.Plan.from_workload(w, spec=spec)
     Pd = torch.from_numpy(np.ascontiguousarray(w.P if P is None else P)).cuda()
-    E, N, V = plan.eval(Pd)
+    E, N, V = plan.eval(Pd, diag=want_points)
     torch.cuda.synchronize()
-    diag = plan.diagnostics(want_points=want_points)
+    diag = plan.diagnostics(want_points=want_points, want_rho=want_points)
     return plan, dict(E=E, N=N, V=V.cpu().numpy(), **diag)
 
 

@@ -247,11 +247,11 @@ def test_full_size_sampled(xc, orc, name):
     w = make_workload(name)
     plan = xc.Plan.from_workload(w)
     P = torch.from_numpy(w.P).cuda()
-    E, N, V = plan.eval(P)
+    E, N, V = plan.eval(P, diag=True)
     Vh = V.cpu().numpy()
     assert np.array_equal(Vh, Vh.T)
     assert abs(N - 2.0 * w.n_occ) / (2.0 * w.n_occ) < 2e-4
-    d = plan.diagnostics()
+    d = plan.diagnostics(want_rho=True)
     assert N == pytest.approx(float(np.sum(d["N_batch"])), rel=1e-12) and E == pytest.approx(float(np.sum(d["E_batch"])), rel=1e-12)
     ex = plan.export()
     op = oracle_plan(orc, ex)
