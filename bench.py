@@ -1,10 +1,13 @@
 #!/usr/bin/env python
 """bench.py -- grid points/s of the full E_xc + V_xc + N_el build (fp64) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2] [--also c3,c4,c5,u2,g1] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c5] [--also c4,c3,c2,c1,u2,g1] [--impl reference]
 
 A step = one pass of the whole hot path (weights -> density -> potential -> scatter/finalise) over one
 synthetic water-cluster workload (BASELINE.json:configs; generator: workloads/).  Prints ONE JSON line.
+The headline workload is c5 (512 waters, 12800 functions, 46.4 M points, PBE): the largest single-GPU
+configuration BASELINE.json names; c4 (256 waters) is measured beside it with the same detail (e2e, both
+rooflines, clocks, plan seconds); the other workloads are short side entries.
 N > 1 (torchrun): the path is not sharded ("replicas only"): every rank runs the same build on
 its own GPU, value = N * points / max-over-ranks device time, scaling = "weak".
 """
@@ -23,7 +26,18 @@ sys.path.insert(0, ROOT)
 METRIC = "grid points/s for full E_xc+V_xc build (fp64, 1 B200); % of FP64 roofline"
 UNIT = "grid points/s"
 FP64_NOMINAL_TFLOPS = 37.2   # 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (datasheet-level; the live measurement below is what is used)
-FP64_PEAK_TFLOPS = FP64_NOMINAL_TFLOPS   # replaced by the live measurement in main()
+FLOP_PER_PAIR = 15.0         # "(a): plain FP64 ALU ...; ~15 flop per evaluated pair; report pairs/point"
+
+DESCR = {
+    "c1": "c1: water monomer, 3 atoms, 25 basis functions, 50x194 grid",
+    "c2": "c2: 64-water cluster, 192 atoms, 1600 basis functions, 75x302 grid",
+    "c3": "c3: 64-water cluster, 192 atoms, 1600 basis functions, 75x302 grid",
+    "c4": "c4: 256-water cluster, 768 atoms, 6400 basis functions, 75x302 grid",
+    "c5": "c5: 512-water cluster, 1536 atoms, 12800 basis functions, 100x302 grid",
+    "u2": "u2: 64-water cluster on a UFG-shaped 99x590 grid (SURVEY 8(f))",
+    "s2": "s2: 64-water cluster on an SFG-shaped 175x974 grid (SURVEY 8(f))",
+    "g1": "g1: irregular 410-water cluster, 1230 atoms, 10250 basis functions, 75x302 grid (SURVEY 8(f))",
+}
 
 
 def _peaks():
@@ -33,6 +47,16 @@ def _peaks():
             d = json.load(fh)
         return float(d.get("hbm_gbs", 6650.0)), "measured"
     return 6650.0, "fallback"
+
+
+def _ncu_traffic(workload, kernel):
+    """dram bytes per launch of `kernel` from the committed ncu --set full capture of this round (profiles/), or None."""
+    p = os.path.join(ROOT, "profiles", "r02_ncu_traffic.json")
+    try:
+        with open(p) as fh:
+            return json.load(fh).get(workload, {}).get(kernel)
+    except Exception:
+        return None
 
 
 class ClockSampler:
@@ -90,7 +114,16 @@ def _hist(a):
     return {"mean": float(a.mean()), "p50": float(np.percentile(a, 50)), "p95": float(np.percentile(a, 95)), "max": float(a.max())}
 
 
-def run_workload(name, steps, warmup, functional=None, do_e2e=True, device=0, sampler=None):
+def config_of(name, w, world):
+    """The workload as named in the JSON line: derived from the workload alone, so both arms print the same dict."""
+    fn = "PBE" if w.functional == 1 else "Slater+VWN5"
+    return {"workload": "%s, %s, SSF partition" % (DESCR.get(name, name), fn), "workload_id": name, "functional": fn,
+            "n_points": int(len(w.atoms_Z)) * w.n_rad * w.n_ang, "n_basis": int(w.n_basis), "n_atoms": int(len(w.atoms_Z)),
+            "partition": "SSF", "parallelism": "replicas only" if world > 1 else "single GPU",
+            "l2": "flushed between timed iterations (256 MB fill)", "seed": 200703143}
+
+
+def run_workload(name, steps, warmup, peaks, do_e2e=True, device=0, sampler=None):
     """Times `steps` full builds of workload `name` on the current GPU. Returns a dict of measurements."""
     import numpy as np
     import torch
@@ -99,7 +132,7 @@ def run_workload(name, steps, warmup, functional=None, do_e2e=True, device=0, sa
     from workloads import make_workload
 
     w = make_workload(name)
-    fn = w.functional if functional is None else functional
+    fn = w.functional
     t0 = time.perf_counter()
     plan = xc.Plan.from_workload(w, spec=xc.grid_spec(w.n_rad, w.n_ang, fn), device=device)
     plan_s = time.perf_counter() - t0
@@ -136,14 +169,16 @@ def run_workload(name, steps, warmup, functional=None, do_e2e=True, device=0, sa
         flush.fill_(1.0)
         plan.eval(P, V, reuse_weights=True)
         t_c.append(plan.timings()["total_ms"])
+    # one extra, untimed build that counts the pair factors step (a) evaluates (roofline of the weights kernel)
+    plan.eval(P, V, count_pairs=True)
+    pairs, nontrivial = plan.counters()
+    stats = plan.stats()
     res = dict(workload=name, functional="PBE" if fn == 1 else "Slater+VWN5", n_points=plan.n_points, n_basis=plan.n_basis,
                n_atoms=int(len(w.atoms_Z)), n_batches=plan.n_batches, ms_per_step=ms, stage_ms=stage, launches=launches,
                E_xc=E, N_el=N, N_el_rel_err_vs_trPS=abs(N - 2.0 * w.n_occ) / (2.0 * w.n_occ), plan_seconds=plan_s,
-               cached_weights_ms=float(np.median(t_c)), flops=plan.algorithmic_flops, stats=plan.stats())
+               cached_weights_ms=float(np.median(t_c)), stats=stats, clocks=ctx.summary())
     res["points_per_s"] = plan.n_points / (ms * 1e-3)
     res["builds_per_s"] = 1e3 / ms
-    res["fp64_tflops"] = plan.algorithmic_flops / (ms * 1e-3) * 1e-12
-    res["fp64_frac"] = res["fp64_tflops"] / FP64_PEAK_TFLOPS
     ex = plan.export()
     nq = np.diff(ex.batch_off)
     foff = (np.asarray(w.shell_L, np.int64) + 1) * (np.asarray(w.shell_L, np.int64) + 2) // 2
@@ -162,7 +197,22 @@ def run_workload(name, steps, warmup, functional=None, do_e2e=True, device=0, sa
     res["flops"] = float(np.sum(per_pt * nbj.astype(np.float64) ** 2 * live))
     res["live_point_fraction"] = float(live.sum() / max(1, plan.n_points))
     res["fp64_tflops"] = res["flops"] / (ms * 1e-3) * 1e-12
-    res["fp64_frac"] = res["fp64_tflops"] / FP64_PEAK_TFLOPS
+    res["fp64_frac"] = res["fp64_tflops"] / peaks["fp64"]
+    # rooflines of the two kernels that make up a build
+    res["roofline_batch"] = {
+        "kernel": "k_xc_batch", "bound": "tensor", "achieved": res["flops"] / (stage["batch_ms"] * 1e-3) * 1e-12, "peak": peaks["fp64"],
+        "unit": "TFLOP/s", "peak_source": peaks["fp64_src"], "traffic": _ncu_traffic(name, "k_xc_batch"),
+        "ms_per_build": stage["batch_ms"], "algorithmic_flops": res["flops"]}
+    res["roofline_batch"]["frac"] = res["roofline_batch"]["achieved"] / peaks["fp64"]
+    # step (a): plain FP64 ALU work, FLOP_PER_PAIR flop per evaluated pair factor (counted on the device), against the measured DFMA rate
+    wflops = FLOP_PER_PAIR * max(pairs, 0)
+    res["roofline_weights"] = {
+        "kernel": "k_weights_ssf", "bound": "alu", "achieved": wflops / max(stage["weights_ms"], 1e-9) * 1e-9, "peak": peaks["dfma"],
+        "unit": "TFLOP/s", "peak_source": peaks["dfma_src"], "traffic": _ncu_traffic(name, "k_weights_ssf"),
+        "ms_per_build": stage["weights_ms"], "pairs_evaluated": pairs, "nontrivial_points": nontrivial,
+        "pairs_per_nontrivial_point": pairs / max(1, nontrivial), "pairs_per_point": pairs / max(1, plan.n_points),
+        "flop_per_pair": FLOP_PER_PAIR}
+    res["roofline_weights"]["frac"] = res["roofline_weights"]["achieved"] / peaks["dfma"]
     if do_e2e:
         # end to end through the C ABI with HOST buffers (pinned): H2D of P and D2H of V inside the timed region
         Ph = torch.from_numpy(w.P).pin_memory()
@@ -215,16 +265,21 @@ def oracle_sample(w, name, target_seconds=15.0, stride=None, fn=None):
                        % (len(atoms), na, stride, len(pts), plan.n_batches, name), E_sample=r.E_xc)
 
 
+SIDE_KEYS = ("workload", "functional", "n_points", "n_basis", "n_batches", "ms_per_step", "points_per_s", "builds_per_s", "fp64_tflops",
+             "fp64_frac", "live_point_fraction", "stage_ms", "cached_weights_ms", "N_el_rel_err_vs_trPS", "nb_hist", "nq_hist",
+             "plan_seconds", "clocks", "roofline_batch", "roofline_weights")
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="c2")
-    ap.add_argument("--also", default="c3,c4,c5,u2,g1", help="comma list of extra workloads reported under other_workloads (or 'none')")
+    ap.add_argument("--workload", default="c5")
+    ap.add_argument("--also", default="c4,c3,c2,c1,u2,g1", help="comma list of extra workloads reported under other_workloads (or 'none')")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-becke", action="store_true", help="skip the Becke-1988 side measurement")
+    ap.add_argument("--no-becke", action="store_true", help="skip the Becke-1988 side measurement (on c2)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -240,15 +295,14 @@ def main():
         w = make_workload(args.workload)
         times, last = [], None
         for k in range(args.warmup + args.steps):
-            last = oracle_sample(w, args.workload, target_seconds=6.0)
+            last = oracle_sample(w, args.workload, target_seconds=4.0)
             if k >= args.warmup:
                 times.append(last["seconds"])
         npts_sample = last["value"] * last["seconds"]
         val = npts_sample / statistics.mean(times)
         line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": statistics.mean(times) * 1e3, "higher_is_better": True, "scaling": "weak",
-                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                "config": {"workload": args.workload, "functional": "PBE" if w.functional == 1 else "Slater+VWN5"},
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_of(args.workload, w, world),
                 "cpu_baseline": {"value": val, "unit": UNIT, "cores": last["cores"], "kind": "oracle", "sample": last["sample"]},
                 "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
         print(json.dumps(line))
@@ -263,15 +317,16 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
         dist.barrier()
     torch.cuda.synchronize()
-    # FP64 roofline denominator, measured live on this GPU (MEASURED_PEAKS.json has no FP64 entry): register-resident
+    # FP64 roofline denominators, measured live on this GPU (MEASURED_PEAKS.json has no FP64 entry): register-resident
     # DMMA (mma.sync m8n8k4 f64) and DFMA chains through the C ABI, burst figure (kernel timed alone)
     import paper_2007_03143_b200 as xc
     dmma_tf, dmma_mhz = xc.measure_fp64_peak(1, local_rank, 5)
     dfma_tf, _ = xc.measure_fp64_peak(0, local_rank, 5)
-    global FP64_PEAK_TFLOPS
-    FP64_PEAK_TFLOPS = max(dmma_tf, dfma_tf)
+    how = ("measured live in this run by xc_measure_fp64_peak: DMMA %.2f, DFMA %.2f TFLOP/s (nominal %.1f = 148 SM x 64 FMA/clk x 2 x "
+           "1.965 GHz)" % (dmma_tf, dfma_tf, FP64_NOMINAL_TFLOPS))
+    peaks = {"fp64": max(dmma_tf, dfma_tf), "fp64_src": "FP64 tensor/FMA pipe " + how, "dfma": dfma_tf, "dfma_src": "FP64 ALU (DFMA) " + how}
     sampler = ClockSampler(local_rank)
-    res, w = run_workload(args.workload, args.steps, warmup, device=local_rank, sampler=sampler)
+    res, w = run_workload(args.workload, args.steps, warmup, peaks, device=local_rank, sampler=sampler)
     ms = res["ms_per_step"]
     if world > 1:
         t = torch.tensor([ms], dtype=torch.float64, device="cuda")
@@ -287,74 +342,43 @@ def main():
         return
     hbm_peak, hbm_src = _peaks()
     value = world * res["n_points"] / (ms * 1e-3)
-    # dominant kernel by device time; its roofline
     st = res["stage_ms"]
     stats = res["stats"]
-    gga = w.functional == 1
-    dom = max(("weights_ms", "batch_ms"), key=lambda k: st[k])
-    traffic = {}
-    tpath = os.path.join(ROOT, "profiles", "traffic_bytes.txt")   # dram bytes per build from the committed ncu --set full captures
-    if os.path.exists(tpath):
-        try:
-            with open(tpath) as fh:
-                traffic = json.load(fh).get(args.workload, {})
-        except Exception:
-            traffic = {}
-    # k_xc_batch, bound = FP64 tensor/FMA pipe.  Algorithmic flops of the dense contractions:
-    # GGA 4 (N_b^j)^2, LDA 2 (N_b^j)^2 per point with w != 0 (run_workload)
-    contraction_flops = res["flops"]
-    fp64_src = ("FP64 pipe measured live in this run by xc_measure_fp64_peak: DMMA %.2f, DFMA %.2f TFLOP/s "
-                "(nominal %.1f = 148 SM x 64 FMA/clk x 2 x 1.965 GHz)" % (dmma_tf, dfma_tf, FP64_NOMINAL_TFLOPS))
-    roofs = {
-        "batch_ms": {"kernel": "k_xc_batch", "bound": "tensor", "achieved": contraction_flops / (st["batch_ms"] * 1e-3) * 1e-12,
-                     "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "peak_source": fp64_src},
-        # step (a) is plain FP64 ALU work bound by instruction issue (profiles/); its algorithmic HBM traffic is
-        # 44 B/point (x, y, z, w^q, parent in; w out), reported against the HBM peak to show it is not memory bound
-        "weights_ms": {"kernel": "k_weights_ssf", "bound": "hbm", "achieved": 44.0 * res["n_points"] / (st["weights_ms"] * 1e-3) * 1e-9,
-                       "peak": hbm_peak, "unit": "GB/s", "peak_source": "MEASURED_PEAKS.json hbm_gbs (%s)" % hbm_src},
-    }
-    for key, r in roofs.items():
-        r["frac"] = r["achieved"] / r["peak"]
-        r["traffic"] = traffic.get(key)
-        r["ms_per_build"] = st[key]
-    roof = roofs[dom]
-    other = roofs["weights_ms" if dom == "batch_ms" else "batch_ms"]
+    # the kernel that takes most of the build comes first; both are reported
+    dom, other = ("roofline_weights", "roofline_batch") if st["weights_ms"] >= st["batch_ms"] else ("roofline_batch", "roofline_weights")
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warmup,
             "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic",
-            "config": {"workload": "%s: 64-water cluster, 192 atoms, 1600 basis functions, 75x302 grid, %s" %
-                                   (args.workload, res["functional"]) if args.workload in ("c2", "c3") else args.workload,
-                       "workload_id": args.workload, "functional": res["functional"], "n_points": res["n_points"],
-                       "n_basis": res["n_basis"], "n_atoms": res["n_atoms"], "n_batches": res["n_batches"],
-                       "partition": "SSF", "parallelism": "replicas only" if world > 1 else "single GPU",
-                       "l2": "flushed between timed iterations (256 MB fill)", "seed": 200703143},
-            "clocks": sampler.summary(), "e2e": {k: res["e2e"][k] for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step")},
-            "gpu_launches": res["launches"], "roofline": roof, "roofline_second_kernel": other,
+            "data": "synthetic", "config": config_of(args.workload, w, world),
+            "clocks": res["clocks"], "e2e": {k: res["e2e"][k] for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step")},
+            "gpu_launches": res["launches"], "roofline": res[dom], "roofline_second_kernel": res[other],
             "builds_per_s": world * 1e3 / ms, "fp64_tflops": res["flops"] / (ms * 1e-3) * 1e-12,
-            "fp64_roofline_frac": res["flops"] / (ms * 1e-3) * 1e-12 / FP64_PEAK_TFLOPS,
+            "fp64_roofline_frac": res["flops"] / (ms * 1e-3) * 1e-12 / peaks["fp64"],
             "fp64_peak": {"dmma_tflops": dmma_tf, "dfma_tflops": dfma_tf, "implied_sm_mhz": dmma_mhz, "how": "xc_measure_fp64_peak, best of 5"},
+            "hbm_peak": {"gbs": hbm_peak, "source": "MEASURED_PEAKS.json hbm_gbs (%s)" % hbm_src,
+                         "note": "neither kernel is HBM-bound: see roofline.traffic / profiles/ for the measured DRAM bytes"},
             "stage_ms": st, "cached_weights_ms": res["cached_weights_ms"],
             "cached_weights_points_per_s": res["n_points"] / (res["cached_weights_ms"] * 1e-3),
-            "plan": {"seconds": res["plan_seconds"], "algorithmic_flops": res["flops"], "algorithmic_flops_all_points": res["flops_all_points"],
+            "plan": {"seconds": res["plan_seconds"], "n_batches": res["n_batches"], "algorithmic_flops": res["flops"],
+                     "algorithmic_flops_all_points": res["flops_all_points"],
                      "live_point_fraction": res["live_point_fraction"], "sum_nb_nq": stats["sum_nb_nq"],
                      "sum_nb2": stats["sum_nb2"], "nq_hist": res["nq_hist"], "nb_hist": res["nb_hist"], "kind": "global k-d bisection"},
             "E_xc": res["E_xc"], "N_el": res["N_el"], "N_el_rel_err_vs_trPS": res["N_el_rel_err_vs_trPS"]}
     # reading A1: the timed path is SSF (the paper's choice); the Becke-1988 partition (no compact support,
-    # O(N_A^2) pair terms per point) is timed beside it on the headline workload, same build otherwise
+    # O(N_A^2) pair terms per point: 13 s per build at c5) is timed beside it on c2, same build otherwise
     if world == 1 and not args.no_becke:
         try:
-            import torch
-            bplan = xc.Plan.from_workload(w, spec=xc.grid_spec(w.n_rad, w.n_ang, w.functional, partition=1), device=local_rank)
-            Pd = torch.from_numpy(w.P).cuda()
+            wb = make_workload("c2")
+            bplan = xc.Plan.from_workload(wb, spec=xc.grid_spec(wb.n_rad, wb.n_ang, wb.functional, partition=1), device=local_rank)
+            Pd = torch.from_numpy(wb.P).cuda()
             Vd = torch.empty_like(Pd)
             bplan.eval(Pd, Vd)
             tb = []
             for _ in range(3):
                 bplan.eval(Pd, Vd)
                 tb.append(bplan.timings())
-            line["becke88"] = {"workload": args.workload, "ms_per_step": statistics.median(t["total_ms"] for t in tb),
+            line["becke88"] = {"workload": "c2", "ms_per_step": statistics.median(t["total_ms"] for t in tb),
                                "weights_ms": statistics.median(t["weights_ms"] for t in tb),
-                               "points_per_s": res["n_points"] / (statistics.median(t["total_ms"] for t in tb) * 1e-3)}
+                               "points_per_s": bplan.n_points / (statistics.median(t["total_ms"] for t in tb) * 1e-3)}
             bplan.close()
             del Pd, Vd
         except Exception as exc:
@@ -368,10 +392,12 @@ def main():
             if nm == args.workload:
                 continue
             try:
-                r2, _ = run_workload(nm, max(3, min(args.steps, 5)), 3, do_e2e=False, device=local_rank, sampler=ClockSampler(local_rank))
-                others.append({k: r2[k] for k in ("workload", "functional", "n_points", "n_basis", "n_batches", "ms_per_step",
-                                                  "points_per_s", "builds_per_s", "fp64_tflops", "fp64_frac", "live_point_fraction", "stage_ms",
-                                                  "cached_weights_ms", "N_el_rel_err_vs_trPS", "nb_hist", "nq_hist")})
+                first_class = nm in ("c4", "c5")
+                r2, _ = run_workload(nm, max(3, min(args.steps, 10 if first_class else 5)), 3, peaks, do_e2e=first_class, device=local_rank)
+                o = {k: r2[k] for k in SIDE_KEYS}
+                if first_class:
+                    o["e2e"] = {k: r2["e2e"][k] for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step")}
+                others.append(o)
             except Exception as exc:  # an extra workload must never cost the headline line
                 others.append({"workload": nm, "error": repr(exc)[:200]})
     line["other_workloads"] = others

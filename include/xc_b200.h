@@ -62,6 +62,7 @@ typedef struct {
 /* flags of xc_eval / xc_eval_host */
 #define XC_EVAL_REUSE_WEIGHTS 1   /* reuse the partition weights of the previous xc_eval on this plan (skip step (a); reading A16) */
 #define XC_EVAL_DIAG          2   /* also store rho and grad rho of every point for xc_eval_diagnostics (parity tests; costs 32 B/point) */
+#define XC_EVAL_COUNT_PAIRS   4   /* count the pair factors s(mu_BC) step (a) evaluates (SSF), for xc_eval_counters; perturbs the timing slightly */
 
 typedef struct xc_plan xc_plan;   /* opaque: owns host + device copies of grid, batches, basis, workspaces */
 
@@ -120,6 +121,12 @@ int xc_eval_diagnostics(xc_plan* plan, double* w, double* rho, double* grad_rho,
  * ms[3] finalise, ms[4] total.
  * launches: number of kernel launches of that xc_eval. */
 int xc_eval_timings(const xc_plan* plan, float ms[5], int32_t* launches);
+
+/* Work counters for the roofline of step (a) ("plain FP64 ALU ... report pairs/point"): ssf_pairs = pair
+ * factors s(mu_BC) evaluated (lane slots of the 32-wide chunks) by the last xc_eval that ran step (a) with
+ * XC_EVAL_COUNT_PAIRS, -1 if there was none; nontrivial_points = points of the plan the SSF kernel visits (the others have
+ * w = w^q exactly, Eq. (9) with every mu_AC <= -a).  Either pointer may be NULL. */
+int xc_eval_counters(const xc_plan* plan, int64_t* ssf_pairs, int64_t* nontrivial_points);
 
 /* Algorithmic sizes of the plan used by the roofline report: [0] sum_j N_b^j N_q^j (function-points),
  * [1] sum_j (N_b^j)^2, [2] sum_j 4 (N_b^j)^2 N_q^j, [3] max N_b^j, [4] mean N_q^j, [5] bytes of the packed-P^j buffer,

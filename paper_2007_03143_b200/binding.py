@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libxc_b200.so")
 
 XC_OK, XC_EINVAL, XC_EUNSUPPORTED, XC_ENOMEM, XC_ECUDA = 0, -1, -2, -3, -4
-XC_EVAL_REUSE_WEIGHTS, XC_EVAL_DIAG = 1, 2
+XC_EVAL_REUSE_WEIGHTS, XC_EVAL_DIAG, XC_EVAL_COUNT_PAIRS = 1, 2, 4
 
 
 class XcAtom(C.Structure):
@@ -59,6 +59,7 @@ def _load():
     lib.xc_eval_host.argtypes = [vp, vp, C.c_int64, vp, C.c_int64, dp, dp, C.c_int32]
     lib.xc_eval_diagnostics.argtypes = [vp, dp, dp, dp, dp, dp]
     lib.xc_eval_timings.argtypes = [vp, C.POINTER(C.c_float), ip]
+    lib.xc_eval_counters.argtypes = [vp, lp, lp]
     lib.xc_plan_destroy.argtypes = [vp]
     lib.xc_integrate.argtypes = [C.POINTER(XcAtom), C.c_int32, C.POINTER(XcShell), C.c_int32, dp, dp, C.c_int32,
                                  C.POINTER(XcGridSpec), C.c_int32, vp, C.c_int64, vp, C.c_int64, dp, dp, vp]
@@ -71,7 +72,7 @@ def _load():
 
 
 EXPORTED = ["xc_plan_create", "xc_plan_info", "xc_plan_export", "xc_eval", "xc_eval_host", "xc_eval_diagnostics",
-            "xc_eval_timings", "xc_plan_stats", "xc_plan_destroy", "xc_integrate", "xc_partition_weights",
+            "xc_eval_timings", "xc_eval_counters", "xc_plan_stats", "xc_plan_destroy", "xc_integrate", "xc_partition_weights",
             "xc_functional", "xc_measure_fp64_peak", "xc_strerror", "xc_last_error"]
 
 _lib = _load()
@@ -170,7 +171,7 @@ class Plan:
                                    shells.ctypes.data_as(C.POINTER(C.c_int32))))
         return PlanExport(pts, wq, parent, orig, boff, soff, shells)
 
-    def eval(self, P, V=None, reuse_weights=False, stream=None, diag=False):
+    def eval(self, P, V=None, reuse_weights=False, stream=None, diag=False, count_pairs=False):
         """P, V: torch CUDA float64 tensors (n_basis x n_basis). Returns (E_xc, N_el, V).
         diag: also keep rho / grad rho of every point for diagnostics() (XC_EVAL_DIAG)."""
         import torch
@@ -180,7 +181,7 @@ class Plan:
         assert V.is_cuda and V.dtype == torch.float64 and V.stride(1) == 1
         E, N = C.c_double(), C.c_double()
         _check(_lib.xc_eval(self._h, C.c_void_p(P.data_ptr()), P.stride(0), C.c_void_p(V.data_ptr()), V.stride(0),
-                            C.byref(E), C.byref(N), (XC_EVAL_REUSE_WEIGHTS if reuse_weights else 0) | (XC_EVAL_DIAG if diag else 0),
+                            C.byref(E), C.byref(N), (XC_EVAL_REUSE_WEIGHTS if reuse_weights else 0) | (XC_EVAL_DIAG if diag else 0) | (XC_EVAL_COUNT_PAIRS if count_pairs else 0),
                             _stream_ptr(stream)))
         return E.value, N.value, V
 
@@ -203,6 +204,12 @@ class Plan:
         Eb, Nb = np.empty(nb), np.empty(nb)
         _check(_lib.xc_eval_diagnostics(self._h, _dp(w), _dp(rho), _dp(gr), _dp(Eb), _dp(Nb)))
         return dict(w=w, rho=rho, grad_rho=gr, E_batch=Eb, N_batch=Nb)
+
+    def counters(self):
+        """(pair factors evaluated by step (a) in the last eval(count_pairs=True), points the SSF kernel visits)."""
+        a, b = C.c_int64(), C.c_int64()
+        _check(_lib.xc_eval_counters(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
 
     def timings(self):
         ms = (C.c_float * 5)()

@@ -68,6 +68,8 @@ struct xc_plan {
   double *d_rho = nullptr, *d_grho = nullptr;   // diagnostics, allocated on first use (XC_EVAL_DIAG)
   bool diag_valid = false;
   double* h_result = nullptr;  // pinned, 4 doubles
+  unsigned long long* d_paircnt = nullptr;   // XC_EVAL_COUNT_PAIRS
+  long long ssf_pairs = -1;    // pair factors evaluated by the last counted build (-1: none)
   int vexp = 0;                // exponent of the fixed-point V accumulator: resolution 2^(vexp - 64), range 2^(vexp + 31)
   double *d_Ptmp = nullptr, *d_Vtmp = nullptr;  // for xc_eval_host
   bool weights_valid = false;
@@ -89,7 +91,7 @@ static void free_plan(xc_plan* p) {
   void* ptrs[] = {p->d_px, p->d_py, p->d_pz, p->d_wq, p->d_w, p->d_parent, p->d_atoms, p->d_invR, p->d_rnn, p->d_shells,
                   p->d_exps, p->d_coefs, p->d_batches, p->d_bshells, p->d_bsfoff, p->d_bfidx, p->d_bfinfo, p->d_ids_small,
                   p->d_ids_large, p->d_ppk, p->d_vhi, p->d_vlo, p->d_Epart, p->d_Npart, p->d_result,
-                  p->d_rho, p->d_grho, p->d_Ptmp, p->d_Vtmp, p->d_watoms, p->d_wsmall, p->d_wlarge, p->d_wbox};
+                  p->d_rho, p->d_grho, p->d_Ptmp, p->d_Vtmp, p->d_watoms, p->d_wsmall, p->d_wlarge, p->d_wbox, p->d_paircnt};
   for (void* q : ptrs) if (q) cudaFree(q);
   if (p->h_result) cudaFreeHost(p->h_result);
   for (cudaEvent_t e : p->ev) cudaEventDestroy(e);
@@ -237,6 +239,12 @@ int xc_eval(xc_plan* p, const double* dP, int64_t ldp, double* dV, int64_t ldv, 
   if (!(flags & XC_EVAL_REUSE_WEIGHTS) || !p->weights_valid) {
     WeightArgs wa;
     wa.batches = p->d_batches; wa.watoms = p->d_watoms; wa.atoms = p->d_atoms; wa.invR = p->d_invR;
+    wa.paircnt = nullptr;
+    if ((flags & XC_EVAL_COUNT_PAIRS) && hp.spec.partition == 0) {
+      if (!p->d_paircnt) CU(cudaMalloc((void**)&p->d_paircnt, 8));
+      CU(cudaMemsetAsync(p->d_paircnt, 0, 8, st));
+      wa.paircnt = p->d_paircnt;
+    }
     wa.wbox = p->d_wbox; wa.natoms = hp.natoms; wa.px = p->d_px; wa.py = p->d_py; wa.pz = p->d_pz; wa.wq = p->d_wq; wa.parent = p->d_parent; wa.w = p->d_w;
     if (hp.spec.partition == 0) {                          // long lists first: they are the long pole
       if (!hp.wbatch_large.empty()) { CUK(launch_weights_ssf(wa, p->d_wlarge, (int)hp.wbatch_large.size(), hp.w_max_large, st), st); ++launches; }
@@ -246,6 +254,13 @@ int xc_eval(xc_plan* p, const double* dP, int64_t ldp, double* dV, int64_t ldv, 
       ++launches;
     }
     p->weights_valid = true;
+    p->ssf_pairs = -1;
+    if (wa.paircnt) {
+      unsigned long long v = 0;
+      CU(cudaMemcpyAsync(&v, p->d_paircnt, 8, cudaMemcpyDeviceToHost, st));
+      CU(cudaStreamSynchronize(st));
+      p->ssf_pairs = (long long)v;
+    }
   }
   CU(cudaEventRecord(p->ev[ie++], st));
   size_t nb2 = (size_t)hp.nbasis * hp.nbasis;
@@ -354,6 +369,17 @@ int xc_eval_timings(const xc_plan* p, float ms[5], int32_t* launches) {
   return XC_OK;
 }
 
+int xc_eval_counters(const xc_plan* p, int64_t* ssf_pairs, int64_t* nontrivial_points) {
+  if (!p) return fail(XC_EINVAL, "plan is null");
+  if (ssf_pairs) *ssf_pairs = p->ssf_pairs;
+  if (nontrivial_points) {
+    int64_t n = 0;
+    for (const BatchRec& b : p->hp.batches) n += b.nq - b.ntriv;
+    *nontrivial_points = n;
+  }
+  return XC_OK;
+}
+
 int xc_plan_destroy(xc_plan* p) {
   free_plan(p);
   return XC_OK;
@@ -446,7 +472,7 @@ int xc_partition_weights(const xc_atom* atoms, int32_t natoms, int32_t partition
   if (rc == XC_OK) rc = upload(&dlg, ids_large);
   if (rc == XC_OK) {
     WeightArgs wa;
-    wa.batches = db; wa.watoms = dl; wa.atoms = da; wa.invR = dt; wa.wbox = dbox; wa.natoms = natoms;
+    wa.batches = db; wa.watoms = dl; wa.atoms = da; wa.invR = dt; wa.wbox = dbox; wa.natoms = natoms; wa.paircnt = nullptr;
     wa.px = dx; wa.py = dy; wa.pz = dz; wa.wq = dwq; wa.parent = dparent; wa.w = dw_out;
     cudaError_t e = cudaSuccess;
     if (partition == 0) {

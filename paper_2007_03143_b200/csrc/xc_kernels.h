@@ -36,6 +36,7 @@ struct WeightArgs {
   int natoms;
   const double* px; const double* py; const double* pz; const double* wq; const int32_t* parent;
   double* w;
+  unsigned long long* paircnt;   // null, or: counter of the pair factors s(mu_BC) the SSF kernel evaluated (XC_EVAL_COUNT_PAIRS)
 };
 
 // SSF: one CTA per batch, one warp per non-trivial point; max_list = longest atom list among the batches launched

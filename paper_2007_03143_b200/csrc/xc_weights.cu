@@ -54,6 +54,7 @@ struct SsfCtx {
   int nC, nch, lane, lcap, tabB;
   double x, y, z;
   int filled;     // list positions [0, filled) of sRC hold r_C of this point
+  int nfac;       // chunks of 32 factors evaluated for this point (only counted when WeightArgs::paircnt is set)
 };
 
 __device__ __forceinline__ double ssf_poly(double zz) {   // s(mu) for zz = mu / a in [-1, 1]; exactly 1 at -1, 0 at +1
@@ -130,6 +131,7 @@ __device__ __forceinline__ double ssf_cell_product(SsfCtx& s, int bb, double Bx,
       if (__any_sync(FULL, zz >= 1.0)) return 0.0;         // s = 0: P_B = 0
       zz = zz < -1.0 ? -1.0 : zz;
       part *= ssf_poly(zz);
+      ++s.nfac;
     }
 #pragma unroll
     for (int o = 16; o >= 1; o >>= 1) part *= __shfl_xor_sync(FULL, part, o);
@@ -169,6 +171,7 @@ __device__ __forceinline__ double ssf_cell_product(SsfCtx& s, int bb, double Bx,
     zz = zz < -1.0 ? -1.0 : zz;
     part *= ssf_poly(zz);
     ++nvis;
+    ++s.nfac;
     if (negligible()) return 0.0;
   }
   // partners past the row: r_C and R_BC from one fetch of the coordinates
@@ -193,6 +196,7 @@ __device__ __forceinline__ double ssf_cell_product(SsfCtx& s, int bb, double Bx,
     zz = zz < -1.0 ? -1.0 : zz;
     part *= ssf_poly(zz);
     ++nvis;
+    ++s.nfac;
     if (negligible()) return 0.0;
   }
 #pragma unroll
@@ -277,6 +281,7 @@ __global__ void __launch_bounds__(kSsfThreads, 2) k_weights_ssf(WeightArgs a, co
     const int64_t gi = (int64_t)b.pt_off + sList[n];
     s.x = a.px[gi]; s.y = a.py[gi]; s.z = a.pz[gi];
     s.filled = 0;
+    s.nfac = 0;
     const int A = a.parent[gi];
     __syncwarp();                                          // the previous point's readers of the row are done
     // ---- 1. nearest atom ----
@@ -359,7 +364,11 @@ __global__ void __launch_bounds__(kSsfThreads, 2) k_weights_ssf(WeightArgs a, co
         result = a.wq[gi] * PA / sum;
       }
     }
-    if (lane == 0) { a.w[gi] = result; n = atomicAdd(&sNext, 1); }
+    if (lane == 0) {
+      a.w[gi] = result;
+      n = atomicAdd(&sNext, 1);
+      if (a.paircnt) atomicAdd(a.paircnt, (unsigned long long)s.nfac * 32ull);   // profiling builds of bench.py only
+    }
     n = __shfl_sync(FULL, n, 0);
   }
 }

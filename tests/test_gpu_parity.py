@@ -235,11 +235,11 @@ def test_partition_kernel_vs_oracle(xc, orc, kind):
 
 
 # ---- full-size configs: sampled outputs + properties ---------------------------------------------
-@pytest.mark.parametrize("name", ["c4", "c5", "u2", "g1"])
+@pytest.mark.parametrize("name", ["c5", "u2", "s2", "g1"])
 def test_full_size_sampled(xc, orc, name):
-    """256- and 512-water PBE workloads in the launch configuration bench.py times, plus the two SURVEY 8(f)
-    "next" workloads: u2 (64 waters on the UFG-shaped 99 x 590 grid) and g1 (irregular 410-water cluster).  The oracle cannot run
-    them whole in seconds, so it computes (i) the weights, rho, grad rho and the per-batch E / N_el partial sums
+    """The 512-water PBE workload in the launch configuration bench.py times (sampled outputs plus properties; c4 and c5
+    are also compared in full by test_c4_full / test_c5_full), plus the SURVEY 8(f) "next" workloads: u2 / s2 (64 waters on the
+    UFG- / SFG-shaped 99 x 590 / 175 x 974 grids) and g1 (irregular 410-water cluster).  Here the oracle computes (i) the weights, rho, grad rho and the per-batch E / N_el partial sums
     of sampled batches, and (ii) sampled V entries exactly: V[mu,nu] only receives contributions from batches
     whose S_j holds both shells, so evaluating that subset of batches gives the full entry.  Properties at any
     size: V symmetric, N_el = tr(PS) within the grid error, bit-identical repeat."""
@@ -294,3 +294,129 @@ def test_full_size_sampled(xc, orc, name):
     E2, N2, V2 = plan.eval(P)
     assert E2 == E and N2 == N and bool((V2.cpu().numpy() == Vh).all())
     plan.close()
+
+
+# ---- full-size parity of every output on the 256- and 512-water configurations ------------------------
+def test_c4_full(xc, orc):
+    """256 waters, 6400 functions, 17.4 M points, PBE -- every output compared in full: the oracle runs Mode A over all
+    42 424 batches of the exported plan (about two minutes on 16 host cores)."""
+    _, plan, g, r = _full_parity(orc, "c4", 1)
+    assert abs(g["N"] - 2560.0) / 2560.0 < 2e-4
+    plan.close()
+
+
+def test_c5_full(xc, orc):
+    """512 waters, 12800 functions, 46.4 M points, PBE, the largest single-GPU configuration -- every output compared in
+    full: weights of all points, rho / grad rho where w != 0, per-batch and total E_xc / N_el, all 1.6e8 entries of V
+    (the oracle runs Mode A over all 131 072 batches of the exported plan: a few minutes on 16 host cores)."""
+    _, plan, g, r = _full_parity(orc, "c5", 1)
+    assert abs(g["N"] - 5120.0) / 5120.0 < 2e-4
+    plan.close()
+
+
+# ---- step (a): the long-list paths of the hot SSF kernel ------------------------------------------------
+@pytest.mark.parametrize("name", ["c4", "g1"])
+def test_ssf_long_lists_dense_cluster(xc, orc, name):
+    """768 / 1230 atoms on a 6 x 26 grid: every batch has an atom list longer than the kernel's distance row (256), so
+    every point takes the long-list path (lazily filled rows, partners past the row, the negligible-owner rule).  All
+    weights against the oracle's pruned evaluation (pinned against brute force on the CPU), a random 3000 against the
+    full O(N_A^2) products, and the sets of exact zeros and exact w^q."""
+    import torch
+    w = make_workload(name, with_P=False)
+    plan = xc.Plan.from_workload(w, spec=xc.grid_spec(6, 26, 0))
+    st = plan.stats()
+    assert st["w_partners_mean"] > 256
+    P = torch.eye(w.n_basis, dtype=torch.float64, device="cuda")
+    plan.eval(P)
+    got = plan.diagnostics()["w"]
+    ex = plan.export()
+    ref = orc.partition_weights(w.atoms_xyz, ex.pts, ex.wq, ex.parent, 0, True)
+    assert np.max(np.abs(got - ref)) <= 1e-13 * np.max(ex.wq)
+    # exact zeros on the same set, up to mu_BC within ~1e-4 of a: there s(mu) = 2.2 (1 - mu/a)^4 < 1e-16 is below the
+    # rounding error of the polynomial (1 - g loses it in the oracle's form, 1/2 - z q(z^2) in the kernel's), so one side
+    # may return exactly 0 and the other ~1e-17 (mpmath at three such points of g1: true s = 1.2e-17, 5.5e-18, 6.9e-19)
+    zm = (got == 0.0) != (ref == 0.0)
+    assert np.all(np.abs(got[zm] - ref[zm]) <= 1e-15 * ex.wq[zm]) and zm.sum() <= 1e-4 * len(got)
+    # w = w^q exactly on the same set, up to the last-bit rounding of w^q P_A / sum when P_A / sum is within an ulp of 1
+    mism = (got == ex.wq) != (ref == ex.wq)
+    assert np.all(np.abs(got[mism] - ref[mism]) <= 2.3e-16 * ex.wq[mism]) and mism.sum() <= 1e-3 * len(got)
+    sel = np.random.default_rng(8).choice(len(got), 3000, replace=False)
+    full = orc.partition_weights(w.atoms_xyz, ex.pts[sel], ex.wq[sel], ex.parent[sel], 0, False)
+    assert np.max(np.abs(got[sel] - full)) <= 1e-13 * np.max(ex.wq)
+    plan.close()
+
+
+def test_ssf_lists_beyond_the_shared_memory_cache(xc, orc):
+    """4752 atoms (1584 waters), points far outside the cluster included: atom lists longer than the kernel's shared-memory
+    atom cache (2112 atoms: coordinates fetched from global memory beyond it) and than its chunk table (4096 atoms).
+    Through xc_partition_weights, which runs the kernels of xc_eval on ad-hoc batches."""
+    import torch
+    w = make_workload("x15", with_P=False)
+    rng = np.random.default_rng(15)
+    n = 1536
+    par = rng.integers(0, len(w.atoms_xyz), n).astype(np.int32)
+    pts = w.atoms_xyz[par] + rng.normal(size=(n, 3)) * rng.choice([0.3, 2.0, 6.0, 40.0], size=(n, 1))
+    order = np.argsort(np.linalg.norm(pts - w.atoms_xyz.mean(0), axis=1))     # spatially coherent pseudo-batches of 512
+    pts, par = pts[order], par[order]
+    wq = rng.uniform(0.1, 2.0, n)
+    got = xc.partition_weights(w.atoms_xyz, torch.from_numpy(pts).cuda(), torch.from_numpy(wq).cuda(),
+                               torch.from_numpy(par).cuda(), 0).cpu().numpy()
+    ref = orc.partition_weights(w.atoms_xyz, pts, wq, par, 0, True)
+    assert np.max(np.abs(got - ref)) <= 1e-13 * np.max(wq)
+    assert np.array_equal(got == 0.0, ref == 0.0)
+    sel = rng.choice(n, 150, replace=False)
+    full = orc.partition_weights(w.atoms_xyz, pts[sel], wq[sel], par[sel], 0, False)
+    assert np.max(np.abs(got[sel] - full)) <= 1e-13 * np.max(wq)
+
+
+# ---- the fixed-point accumulator of V: scale, non-finite input ------------------------------------------
+@pytest.mark.parametrize("k", [20, -20])
+def test_v_scaled_by_powers_of_two(xc, k):
+    """phi -> 2^k phi (coefficients) and P -> 2^-2k P leave rho, E_xc, N_el unchanged bit for bit and scale V by exactly
+    2^2k: V = 2^40 V0 / 2^-40 V0.  The accumulator's exponent must follow (one repeated build), never wrap or lose bits."""
+    import torch
+    w = make_workload("w8")
+    plan0 = xc.Plan.from_workload(w)
+    E0, N0, V0 = plan0.eval(torch.from_numpy(w.P).cuda())
+    s_ = 2.0 ** k
+    plan = xc.Plan(w.atoms_xyz, w.atoms_Z, w.shell_atom, w.shell_L, w.shell_nprim, w.shell_prim_off, w.exps, w.coefs * s_,
+                   xc.grid_spec(w.n_rad, w.n_ang, w.functional))
+    P = torch.from_numpy(w.P / (s_ * s_)).cuda()
+    E, N, V = plan.eval(P)
+    assert E == E0 and N == N0
+    assert float((V / (s_ * s_) - V0).abs().max()) <= 1e-13 * float(V0.abs().max())
+    E2, N2, V2 = plan.eval(P)                                                  # the plan remembers the exponent
+    assert E2 == E and torch.equal(V, V2)
+    plan.close(); plan0.close()
+
+
+def test_non_finite_input_is_reported(xc):
+    import torch
+    w = make_workload("w8")
+    plan = xc.Plan.from_workload(w)
+    P = torch.from_numpy(w.P).cuda()
+    E0, N0, V0 = plan.eval(P)
+    for bad in (float("nan"), float("inf")):
+        Pb = P.clone()
+        Pb[3, 3] = bad
+        V = torch.zeros_like(P)
+        with pytest.raises(xc.XcError) as e:
+            plan.eval(Pb, V)
+        assert e.value.code == -1 and bool(torch.isnan(V).all())
+    E1, N1, V1 = plan.eval(P)                                                  # the plan is usable afterwards
+    assert E1 == E0 and torch.equal(V0, V1)
+    plan.close()
+
+
+def test_bad_geometry_is_rejected(xc):
+    w = make_workload("c1")
+    xyz = w.atoms_xyz.copy()
+    xyz[2] = xyz[1]
+    with pytest.raises(xc.XcError) as e:
+        xc.Plan(xyz, w.atoms_Z, w.shell_atom, w.shell_L, w.shell_nprim, w.shell_prim_off, w.exps, w.coefs, xc.grid_spec(10, 26, 0))
+    assert e.value.code == -1
+    xyz = w.atoms_xyz.copy()
+    xyz[0, 0] = np.nan
+    with pytest.raises(xc.XcError) as e:
+        xc.Plan(xyz, w.atoms_Z, w.shell_atom, w.shell_L, w.shell_nprim, w.shell_prim_off, w.exps, w.coefs, xc.grid_spec(10, 26, 0))
+    assert e.value.code == -1

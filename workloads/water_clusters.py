@@ -58,6 +58,11 @@ CONFIGS = {
     # means n molecules placed by random sequential addition in an ellipsoid
     "u2": Config("u2", (4, 4, 4), 320, 99, 590, 1, BASIS_SEED + 2),
     "g1": Config("g1", (0, 0, 410), 2050, 75, 302, 1, BASIS_SEED + 11),
+    # s2 = the c2 cluster on an SFG-shaped 175 x 974 grid (Table 2), PBE
+    "s2": Config("s2", (4, 4, 4), 320, 175, 974, 1, BASIS_SEED + 2),
+    # geometry-only shape for the weights kernels (never used with a density matrix): 1584 waters, 4752 atoms -- atom
+    # lists longer than the SSF kernel's shared-memory cache (2112) and chunk table (4096)
+    "x15": Config("x15", (12, 12, 11), 7920, 6, 26, 1, BASIS_SEED + 15),
     # small extra shapes for tests (not in BASELINE.json): 8 and 27 waters
     "w8": Config("w8", (2, 2, 2), 40, 50, 194, 1, BASIS_SEED + 8),
     "w27": Config("w27", (3, 3, 3), 135, 50, 194, 1, BASIS_SEED + 27),
@@ -275,7 +280,7 @@ def make_workload(name: str, with_P: bool = True, cache: bool = True) -> Workloa
     if not with_P:
         return w
     key = hashlib.sha1(("v1|%d|%s|%d|%d" % (cfg.geom_seed, cfg.lattice, cfg.n_occ, BASIS_SEED)).encode()).hexdigest()[:16]
-    path = os.path.join(_cache_dir(), "P_%s_%s.npy" % (cfg.name if cfg.name not in ("c3", "u2") else "c2", key))
+    path = os.path.join(_cache_dir(), "P_%s_%s.npy" % (cfg.name if cfg.name not in ("c3", "u2", "s2") else "c2", key))
     if cache and os.path.exists(path):
         P = np.load(path)
         if P.shape == (nb, nb):
