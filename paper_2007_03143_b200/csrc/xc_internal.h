@@ -16,7 +16,7 @@ constexpr int kSmallNb = 112;   // N_b^j limit of the 64-point-tile instantiatio
 constexpr int kMaxNb = 192;     // N_b^j limit of the batch kernel (<= 78 blocks = 5 per warp); the planner splits larger batches
 constexpr size_t kSmemLimit = 227 * 1024;
 constexpr int kWeightThreads = 256;  // Becke-88 weights kernel: 8 warps per batch CTA
-constexpr int kWeightSmallList = 192; // SSF weights kernel: atom-list length that separates its two launches
+constexpr int kWeightSmallList = 256; // SSF weights kernel: atom-list length that separates its two launches
 
 struct ShellRec {      // 48 bytes
   double x, y, z;      // centre
