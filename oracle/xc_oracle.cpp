@@ -13,7 +13,8 @@
 // Pins (tests/test_oracle_*.py, all -m "not gpu"): closed-form one-primitive Slater energy (P1),
 // sum w rho = tr(P S) (P2), V symmetric (P3), finite-difference dE/dP = V (P4), unscreened brute
 // force (P5), functional values vs 40-digit mpmath (P6), functional limits (P7), collocation vs
-// finite differences and closed-form overlaps (P8), plan validity (P9), translation invariance (P10).
+// finite differences and closed-form overlaps (P8), plan validity (P9), translation invariance (P10);
+// pure d shells (reading A19): typed values, orthonormality with s and p on a fine grid, Unsold's theorem, tr(PS), dE/dP = V.
 // Parity UNPINNED against the paper itself: the paper prints no E_xc / V_xc / N_el value.
 //
 // Build: g++ -O2 -fopenmp -shared -fPIC -o libxc_oracle.so xc_oracle.cpp   (oracle/build.py)
@@ -167,6 +168,12 @@ inline void eval_point(int kind, double rho, double sigma, double rho_tol, doubl
 }
 
 inline int ncart(int L) { return (L + 1) * (L + 2) / 2; }
+// Shell code (reading A19): low byte = angular momentum L; bit 8 (0x100) set = "pure" shell, whose functions are
+// the 2L+1 real solid harmonics instead of the (L+1)(L+2)/2 Cartesian monomials ("spherical Gaussian
+// functions"; L323 cc-pVDZ).  Only d shells change: a pure s or p shell has the same functions as the Cartesian one.
+inline int sh_L(int code) { return code & 0xff; }
+inline bool sh_pure(int code) { return (code & 0x100) != 0 && sh_L(code) == 2; }
+inline int nfun(int code) { return sh_pure(code) ? 5 : ncart(sh_L(code)); }
 
 // ---- partition cell functions ------------------------------------------------------------------
 // SSF (Stratmann-Scuseria-Frisch 1996), a = 0.64 (A1/A2): s = (1 - g)/2,
@@ -209,8 +216,9 @@ inline double ipow(double x, int n) {
   for (int k = 0; k < n; ++k) r *= x;
   return r;
 }
-inline void shell_at_point(int L, int nprim, const double* alpha, const double* d, const double* R, const double* r,
+inline void shell_at_point(int code, int nprim, const double* alpha, const double* d, const double* R, const double* r,
                            double* phi, double* grad) {
+  const int L = sh_L(code);
   double dx = r[0] - R[0], dy = r[1] - R[1], dz = r[2] - R[2];
   double r2 = dx * dx + dy * dy + dz * dz;
   double R0 = 0.0, R1 = 0.0;
@@ -233,6 +241,27 @@ inline void shell_at_point(int L, int nprim, const double* alpha, const double* 
       }
       ++c;
     }
+  if (sh_pure(code)) {
+    // Pure d shell (A19): the five real solid harmonics of degree 2, m = -2 .. 2, as combinations of the Cartesian
+    // functions xx, xy, xz, yy, yz, zz (which share one radial part whose xx component has unit norm, A6):
+    //   d(-2) = sqrt3 xy,  d(-1) = sqrt3 yz,  d(0) = zz - (xx + yy)/2,  d(+1) = sqrt3 xz,  d(+2) = (sqrt3/2)(xx - yy).
+    // Each has unit norm and they are mutually orthogonal (pinned by the overlap and Unsold tests).
+    const double s3 = std::sqrt(3.0);
+    const int nv = grad ? 4 : 1;
+    for (int v = 0; v < nv; ++v) {   // v = 0: values, 1..3: x, y, z derivatives (the transformation is linear)
+      double cart[6], pure[5];
+      for (int q = 0; q < 6; ++q) cart[q] = v == 0 ? phi[q] : grad[3 * q + v - 1];
+      pure[0] = s3 * cart[1];
+      pure[1] = s3 * cart[4];
+      pure[2] = cart[5] - 0.5 * (cart[0] + cart[3]);
+      pure[3] = s3 * cart[2];
+      pure[4] = 0.5 * s3 * (cart[0] - cart[3]);
+      for (int q = 0; q < 5; ++q) {
+        if (v == 0) phi[q] = pure[q];
+        else grad[3 * q + v - 1] = pure[q];
+      }
+    }
+  }
 }
 
 }  // namespace
@@ -571,7 +600,7 @@ int orc_collocation(int nsh, const int32_t* sh_list, const int32_t* shell_atom, 
                     const double* coefs, const double* xyz, int64_t npts, const double* pts, double* phi,
                     double* gx, double* gy, double* gz) {
   int nf = 0;
-  for (int k = 0; k < nsh; ++k) nf += ncart(shell_L[sh_list[k]]);
+  for (int k = 0; k < nsh; ++k) nf += nfun(shell_L[sh_list[k]]);
   for (int64_t i = 0; i < npts; ++i) {
     int f = 0;
     for (int k = 0; k < nsh; ++k) {
@@ -579,7 +608,7 @@ int orc_collocation(int nsh, const int32_t* sh_list, const int32_t* shell_atom, 
       double ph[6], gr[18];
       shell_at_point(shell_L[s], shell_nprim[s], exps + shell_prim_off[s], coefs + shell_prim_off[s],
                      xyz + 3 * shell_atom[s], pts + 3 * i, ph, gx ? gr : nullptr);
-      for (int c = 0; c < ncart(shell_L[s]); ++c, ++f) {
+      for (int c = 0; c < nfun(shell_L[s]); ++c, ++f) {
         phi[(size_t)f * npts + i] = ph[c];
         if (gx) {
           gx[(size_t)f * npts + i] = gr[3 * c + 0];
@@ -625,7 +654,7 @@ void orc_eval(int64_t nbatch, const int64_t* batch_off, const int64_t* shell_off
     // S_j function index list
     std::vector<int> fidx;
     for (int k = 0; k < ns; ++k)
-      for (int c = 0; c < ncart(shell_L[S[k]]); ++c) fidx.push_back(func_off[S[k]] + c);
+      for (int c = 0; c < nfun(shell_L[S[k]]); ++c) fidx.push_back(func_off[S[k]] + c);
     size_t nb = fidx.size();
     if (nb == 0 || nq == 0) continue;
     // O7: Phi^j (nb x nq) and gradients, Eq. (12a)
@@ -731,7 +760,7 @@ void orc_eval_unscreened(int64_t npts, const double* pts, const double* w, int n
       for (int s = 0; s < nshells; ++s) {
         shell_at_point(shell_L[s], shell_nprim[s], exps + shell_prim_off[s], coefs + shell_prim_off[s],
                        xyz + 3 * shell_atom[s], pts + 3 * i, &phi[f], &g[3 * f]);
-        f += ncart(shell_L[s]);
+        f += nfun(shell_L[s]);
       }
       double rho = 0.0, gr[3] = {0.0, 0.0, 0.0};
       for (int m = 0; m < nbasis; ++m) {
@@ -776,7 +805,7 @@ double orc_plan_flops(int64_t nbatch, const int64_t* batch_off, const int64_t* s
   double tot = 0.0;
   for (int64_t j = 0; j < nbatch; ++j) {
     double nb = 0.0;
-    for (int64_t k = shell_off[j]; k < shell_off[j + 1]; ++k) nb += ncart(shell_L[shells[k]]);
+    for (int64_t k = shell_off[j]; k < shell_off[j + 1]; ++k) nb += nfun(shell_L[shells[k]]);
     tot += 4.0 * nb * nb * (double)(batch_off[j + 1] - batch_off[j]);
   }
   return tot;

@@ -155,7 +155,7 @@ def collocation(sh_list, basis, xyz, pts, grad=True):
     sa, sL, sn, so, ex, co = _i32(sa), _i32(sL), _i32(sn), _i32(so), _f64(ex), _f64(co)
     sh_list = _i32(sh_list)
     xyz, pts = _f64(xyz), _f64(pts)
-    nf = int(sum((int(sL[s]) + 1) * (int(sL[s]) + 2) // 2 for s in sh_list))
+    nf = int(sum(_nfun(int(sL[s])) for s in sh_list))
     n = len(pts)
     phi = np.empty((nf, n))
     g = [np.empty((nf, n)) for _ in range(3)] if grad else [None] * 3
@@ -172,8 +172,14 @@ def functional(kind, rho, sigma=None, rho_tol=1e-15):
     return f, vr, vs
 
 
+def _nfun(code):
+    """Functions of a shell code (low byte L; bit 8: pure d shell = 5 functions): sizes the output arrays."""
+    L = code & 0xff
+    return 5 if (code & 0x100) and L == 2 else (L + 1) * (L + 2) // 2
+
+
 def _func_off(shell_L):
-    nc = (np.asarray(shell_L, np.int64) + 1) * (np.asarray(shell_L, np.int64) + 2) // 2
+    nc = np.array([_nfun(int(c)) for c in np.asarray(shell_L)], dtype=np.int64)
     return np.concatenate([[0], np.cumsum(nc)[:-1]]).astype(np.int32), int(nc.sum())
 
 

@@ -486,3 +486,97 @@ def test_next_workload_shapes():
     assert np.allclose(np.linalg.norm(g1.atoms_xyz[1::3] - O, axis=1), np.linalg.norm(c2.atoms_xyz[1] - c2.atoms_xyz[0]))
     ext = O.max(0) - O.min(0)
     assert ext[0] > 1.8 * ext[2]          # elongated: not a cube
+
+
+# ---- pure (real solid harmonic) d shells, SURVEY 8(f) item 4 (reading A19) -----------
+def _one_atom_pure_d(alpha=0.9):
+    # one centre: s, p and a pure d shell, one primitive each; the d radial part has unit norm on xx (A6)
+    from workloads import PURE
+    xyz = np.array([[0.2, -0.1, 0.3]])
+    ns = (2 * alpha / math.pi) ** 0.75
+    npp = ns * (4 * alpha) ** 0.5
+    nd = ns * (4 * alpha) / math.sqrt(3.0)
+    basis = (np.array([0, 0, 0], np.int32), np.array([0, 1, 2 | PURE], np.int32), np.array([1, 1, 1], np.int32),
+             np.array([0, 1, 2], np.int32), np.array([alpha, alpha, alpha]), np.array([ns, npp, nd]))
+    return xyz, basis
+
+
+def test_pure_d_explicit_values_and_gradient(orc):
+    """The five pure d functions typed out from the real solid harmonics of degree 2 (m = -2..2), and their gradients
+    against central finite differences."""
+    xyz, basis = _one_atom_pure_d()
+    pt = np.array([[1.0, 0.5, -0.75], [-0.4, 0.9, 0.2]])
+    sh = np.array([2], np.int32)
+    phi, gx, gy, gz = orc.collocation(sh, basis, xyz, pt)
+    assert phi.shape == (5, 2)
+    for i in range(2):
+        x, y, z = pt[i] - xyz[0]
+        R = basis[5][2] * math.exp(-basis[4][2] * (x * x + y * y + z * z))
+        s3 = math.sqrt(3.0)
+        expect = [s3 * x * y * R, s3 * y * z * R, (z * z - 0.5 * (x * x + y * y)) * R, s3 * x * z * R, 0.5 * s3 * (x * x - y * y) * R]
+        assert np.allclose(phi[:, i], expect, rtol=1e-14, atol=1e-300)
+    h = 1e-5
+    for c, g in enumerate((gx, gy, gz)):
+        d = np.zeros(3)
+        d[c] = h
+        fd = (orc.collocation(sh, basis, xyz, pt + d, grad=False) - orc.collocation(sh, basis, xyz, pt - d, grad=False)) / (2 * h)
+        assert np.max(np.abs(fd - g)) < 1e-8 * np.max(np.abs(g))
+
+
+def test_pure_d_orthonormal_and_orthogonal_to_s_and_p(orc):
+    """int phi_mu phi_nu over a fine one-centre grid: the 1 + 3 + 5 functions are orthonormal.  (A Cartesian zz overlaps
+    with s; the trace-free d(0) must not; wrong coefficients break the unit norms.)"""
+    xyz, basis = _one_atom_pure_d()
+    pts, wq, _ = orc.build_grid(xyz, 150, 1152, angular_kind=1)
+    phi = orc.collocation(np.array([0, 1, 2], np.int32), basis, xyz, pts, grad=False)
+    S = (phi * wq) @ phi.T
+    assert S.shape == (9, 9)
+    assert np.max(np.abs(S - np.eye(9))) < 1e-10
+
+
+def test_pure_d_unsold_theorem(orc):
+    """sum_m d_m(r)^2 depends on |r| only (Unsold): equal on random directions of one sphere; pins the relative
+    normalisation of the five components."""
+    xyz, basis = _one_atom_pure_d()
+    rng = np.random.default_rng(5)
+    u = rng.normal(size=(200, 3))
+    u /= np.linalg.norm(u, axis=1, keepdims=True)
+    for rad in (0.3, 1.7):
+        phi = orc.collocation(np.array([2], np.int32), basis, xyz, xyz + rad * u, grad=False)
+        tot = np.sum(phi * phi, axis=0)
+        assert np.max(np.abs(tot - tot[0])) < 1e-14 * tot[0]
+        # = (3/4) r^4 R(r)^2 ... checked against the closed form: sum_m d_m^2 = r^4 R^2 (x,y,z on the unit sphere)
+        R = basis[5][2] * math.exp(-basis[4][2] * rad * rad)
+        assert tot[0] == pytest.approx(rad ** 4 * R * R, rel=1e-13)
+
+
+def test_pure_d_workload_trace_and_finite_difference(orc):
+    """p1 (monomer, O d shell pure: 24 functions): closed-form S of the generator vs quadrature, tr(PS) = 10, N_el on
+    the product grid, V symmetric and V = dE/dP by central differences (PBE)."""
+    w = make_workload("p1")
+    assert w.n_basis == 24
+    S = overlap_matrix(w)
+    assert float(np.trace(w.P @ S)) == pytest.approx(10.0, abs=1e-11)
+    basis = _basis(w)
+    ptsO, wqO, _ = orc.build_grid(w.atoms_xyz[:1], 150, 1152, angular_kind=1)
+    shO = np.where(w.shell_atom == 0)[0].astype(np.int32)
+    phi = orc.collocation(shO, basis, w.atoms_xyz, ptsO, grad=False)
+    assert np.max(np.abs((phi * wqO) @ phi.T - S[:14, :14])) < 1e-10
+    pts, wq, par = orc.build_grid(w.atoms_xyz, 100, 1152, 1)
+    rc = orc.rcut(w.shell_nprim, w.shell_prim_off, w.exps)
+    plan = orc.plan_paper(w.atoms_xyz, pts, wq, par, w.shell_atom, rc)
+    wts = orc.partition_weights(w.atoms_xyz, plan.pts, plan.wq, plan.parent, 0, True)
+    r = orc.evaluate(plan, wts, basis, w.atoms_xyz, w.P, 1)
+    assert abs(r.N_el - 10.0) < 1e-5
+    vmax = np.max(np.abs(r.V))
+    assert np.max(np.abs(r.V - r.V.T)) <= 1e-15 * vmax
+    b = orc.evaluate_unscreened(plan.pts, wts, basis, w.atoms_xyz, w.P, 1)
+    assert np.max(np.abs(r.V - b.V)) <= 1e-10 * vmax and abs(r.E_xc - b.E_xc) <= 1e-11 * abs(b.E_xc)
+    h = 1e-4
+    for (m, n) in [(9, 9), (11, 13), (2, 10), (12, 20), (13, 13), (10, 23)]:   # 9..13 = the pure d functions of O
+        D = np.zeros_like(w.P)
+        D[m, n] = D[n, m] = 1.0
+        ep = orc.evaluate(plan, wts, basis, w.atoms_xyz, w.P + h * D, 1, want_V=False).E_xc
+        em = orc.evaluate(plan, wts, basis, w.atoms_xyz, w.P - h * D, 1, want_V=False).E_xc
+        expect = r.V[m, m] if m == n else 2.0 * r.V[m, n]
+        assert abs((ep - em) / (2 * h) - expect) < 1e-7 * vmax

@@ -35,6 +35,9 @@ O_EXP_RANGE = (0.2, 5000.0)
 H_EXP_RANGE = (0.1, 30.0)
 
 
+PURE = 0x100  # shell code bit: pure (real solid harmonic) shell; only changes d shells (5 functions instead of 6)
+
+
 @dataclasses.dataclass(frozen=True)
 class Config:
     name: str
@@ -44,6 +47,7 @@ class Config:
     n_ang: int
     functional: int  # 0 = LDA Slater+VWN5, 1 = GGA PBE
     geom_seed: int
+    pure_d: bool = False  # the O d shell as 5 pure functions (cc-pVDZ-style)
 
 
 CONFIGS = {
@@ -65,12 +69,23 @@ CONFIGS = {
     "x15": Config("x15", (12, 12, 11), 7920, 6, 26, 1, BASIS_SEED + 15),
     # small extra shapes for tests (not in BASELINE.json): 8 and 27 waters
     "w8": Config("w8", (2, 2, 2), 40, 50, 194, 1, BASIS_SEED + 8),
+    # pure (spherical) d shells on O: monomer, 8 and 27 waters; 14 functions per O
+    "p1": Config("p1", (1, 1, 1), 5, 50, 194, 1, BASIS_SEED + 1, True),
+    "p8": Config("p8", (2, 2, 2), 40, 50, 194, 1, BASIS_SEED + 8, True),
+    "p8l": Config("p8l", (2, 2, 2), 40, 50, 194, 0, BASIS_SEED + 8, True),
+    "p27": Config("p27", (3, 3, 3), 135, 50, 194, 1, BASIS_SEED + 27, True),
     "w27": Config("w27", (3, 3, 3), 135, 50, 194, 1, BASIS_SEED + 27),
 }
 
 
 def ncart(L: int) -> int:
     return (L + 1) * (L + 2) // 2
+
+
+def nfun(code: int) -> int:
+    """Functions of a shell code: low byte L, bit PURE = pure d shell (5 functions)."""
+    L = code & 0xff
+    return 5 if (code & PURE) and L == 2 else ncart(L)
 
 
 def cart_components(L: int):
@@ -179,18 +194,18 @@ class Workload:
 
     @property
     def shell_func_off(self):
-        nc = np.array([ncart(int(L)) for L in self.shell_L], dtype=np.int64)
+        nc = np.array([nfun(int(L)) for L in self.shell_L], dtype=np.int64)
         return np.concatenate([[0], np.cumsum(nc)[:-1]]).astype(np.int32)
 
 
-def _build_basis(atoms_Z):
+def _build_basis(atoms_Z, pure_d=False):
     eb = element_basis()
     shell_atom, shell_L, shell_nprim, shell_off, exps, coefs = [], [], [], [], [], []
     off = 0
     for ia, Z in enumerate(atoms_Z):
         for (L, a, d) in eb[int(Z)]:
             shell_atom.append(ia)
-            shell_L.append(L)
+            shell_L.append(L | PURE if (pure_d and L == 2) else L)
             shell_nprim.append(len(a))
             shell_off.append(off)
             exps.append(a)
@@ -214,8 +229,27 @@ def _int1d_table(p, PA, PB, la, lb):
     return out
 
 
+# rows: the five pure d functions (m = -2..2) in terms of xx, xy, xz, yy, yz, zz (all with the radial part whose xx
+# component has unit norm): sqrt3 xy, sqrt3 yz, zz - (xx + yy)/2, sqrt3 xz, (sqrt3/2)(xx - yy)
+_PURE_D = np.array([[0, 3 ** 0.5, 0, 0, 0, 0], [0, 0, 0, 0, 3 ** 0.5, 0], [-0.5, 0, 0, -0.5, 0, 1.0],
+                    [0, 0, 3 ** 0.5, 0, 0, 0], [0.5 * 3 ** 0.5, 0, 0, -0.5 * 3 ** 0.5, 0, 0]])
+
+
 def overlap_matrix(w: "Workload") -> np.ndarray:
-    """Closed-form overlap S of the contracted Cartesian basis (Gaussian product theorem)."""
+    """Closed-form overlap S of the contracted basis (Gaussian product theorem); pure d shells: T S_cart T^T."""
+    if np.any(np.asarray(w.shell_L) & PURE):
+        wc = dataclasses.replace(w, shell_L=(np.asarray(w.shell_L) & 0xff).astype(np.int32), P=None)
+        wc.n_basis = int(sum(ncart(int(L)) for L in wc.shell_L))
+        Sc = overlap_matrix(wc)
+        T = np.zeros((w.n_basis, wc.n_basis))
+        fo, fc = w.shell_func_off, wc.shell_func_off
+        for s_, code in enumerate(w.shell_L):
+            n_ = ncart(int(code) & 0xff)
+            if int(code) & PURE and (int(code) & 0xff) == 2:
+                T[fo[s_]:fo[s_] + 5, fc[s_]:fc[s_] + 6] = _PURE_D
+            else:
+                T[fo[s_]:fo[s_] + n_, fc[s_]:fc[s_] + n_] = np.eye(n_)
+        return T @ Sc @ T.T
     nb = w.n_basis
     S = np.zeros((nb, nb))
     foff = w.shell_func_off
@@ -273,13 +307,13 @@ def make_workload(name: str, with_P: bool = True, cache: bool = True) -> Workloa
     cfg = CONFIGS[name]
     rng = np.random.default_rng(cfg.geom_seed)
     xyz, Z = _geometry(rng, cfg.lattice)
-    sa, sL, sn, so, exps, coefs = _build_basis(Z)
-    nb = int(sum(ncart(int(L)) for L in sL))
+    sa, sL, sn, so, exps, coefs = _build_basis(Z, cfg.pure_d)
+    nb = int(sum(nfun(int(L)) for L in sL))
     w = Workload(name, xyz, Z.astype(np.int32), sa, sL, sn, so, exps, coefs, nb, cfg.n_occ, cfg.n_rad, cfg.n_ang,
                  cfg.functional, None)
     if not with_P:
         return w
-    key = hashlib.sha1(("v1|%d|%s|%d|%d" % (cfg.geom_seed, cfg.lattice, cfg.n_occ, BASIS_SEED)).encode()).hexdigest()[:16]
+    key = hashlib.sha1(("v1|%d|%s|%d|%d%s" % (cfg.geom_seed, cfg.lattice, cfg.n_occ, BASIS_SEED, "|pure" if cfg.pure_d else "")).encode()).hexdigest()[:16]
     path = os.path.join(_cache_dir(), "P_%s_%s.npy" % (cfg.name if cfg.name not in ("c3", "u2", "s2") else "c2", key))
     if cache and os.path.exists(path):
         P = np.load(path)
