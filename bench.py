@@ -181,7 +181,8 @@ def run_workload(name, steps, warmup, peaks, do_e2e=True, device=0, sampler=None
     res["builds_per_s"] = 1e3 / ms
     ex = plan.export()
     nq = np.diff(ex.batch_off)
-    foff = (np.asarray(w.shell_L, np.int64) + 1) * (np.asarray(w.shell_L, np.int64) + 2) // 2
+    from workloads import nfun
+    foff = np.array([nfun(int(c)) for c in w.shell_L], dtype=np.int64)
     csum = np.concatenate([[0], np.cumsum(foff[ex.shells])])
     nbj = csum[ex.shell_off[1:]] - csum[ex.shell_off[:-1]]
     res["nq_hist"] = _hist(nq)

@@ -21,6 +21,9 @@
  *   - units: bohr / hartree.  All floating point is IEEE double.
  *   - function order in P and V: shells in input order; inside a shell the Cartesian components
  *     (l,m,n), l descending then m descending: p = x,y,z; d = xx,xy,xz,yy,yz,zz ((L+1)(L+2)/2 of them).
+ *     A d shell flagged XC_SHELL_PURE holds the five real solid harmonics instead ("spherical Gaussian
+ *     functions", L323 cc-pVDZ; reading A19), m = -2..2, in terms of the Cartesian functions of the same radial part:
+ *     sqrt3 xy, sqrt3 yz, zz - (xx + yy)/2, sqrt3 xz, (sqrt3/2)(xx - yy).
  *   - coefficients are used as given (primitive norms included by the caller); nothing is renormalised.
  *   - every entry point returns 0 (XC_OK) or a negative XC_E* code; nothing throws or aborts across the
  *     ABI.  xc_last_error() returns a thread-local text for the last failure (CUDA error string included).
@@ -44,7 +47,8 @@ extern "C" {
 #define XC_ECUDA        -4  /* CUDA runtime error (text in xc_last_error) */
 
 typedef struct { double x, y, z; int32_t Z; int32_t _pad; } xc_atom;           /* position (bohr), atomic number */
-typedef struct { int32_t atom; int32_t L; int32_t nprim; int32_t prim_off; } xc_shell; /* Cartesian shell, Eq. (7) */
+#define XC_SHELL_PURE 0x100  /* OR-ed into xc_shell.L: pure (real solid harmonic) shell; changes d shells only (5 functions) */
+typedef struct { int32_t atom; int32_t L; int32_t nprim; int32_t prim_off; } xc_shell; /* contracted shell, Eq. (7); L = 0..2 [| XC_SHELL_PURE] */
 
 typedef struct {
   int32_t n_rad, n_ang;   /* radial x angular points per atom (Table 2) */

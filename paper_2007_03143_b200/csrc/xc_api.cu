@@ -58,7 +58,7 @@ struct xc_plan {
   ShellRec* d_shells = nullptr;
   double *d_exps = nullptr, *d_coefs = nullptr;
   BatchRec* d_batches = nullptr;
-  int32_t *d_bshells = nullptr, *d_bsfoff = nullptr, *d_bfidx = nullptr, *d_bfinfo = nullptr;
+  int32_t *d_bshells = nullptr, *d_bsfoff = nullptr, *d_bfidx = nullptr;
   double* d_wbox = nullptr;
   int32_t *d_watoms = nullptr, *d_wsmall = nullptr, *d_wlarge = nullptr;
   int32_t *d_ids_small = nullptr, *d_ids_large = nullptr;
@@ -89,7 +89,7 @@ static void free_plan(xc_plan* p) {
   if (p->device < 0) { delete p; return; }
   DeviceGuard guard(p->device);
   void* ptrs[] = {p->d_px, p->d_py, p->d_pz, p->d_wq, p->d_w, p->d_parent, p->d_atoms, p->d_invR, p->d_rnn, p->d_shells,
-                  p->d_exps, p->d_coefs, p->d_batches, p->d_bshells, p->d_bsfoff, p->d_bfidx, p->d_bfinfo, p->d_ids_small,
+                  p->d_exps, p->d_coefs, p->d_batches, p->d_bshells, p->d_bsfoff, p->d_bfidx, p->d_ids_small,
                   p->d_ids_large, p->d_ppk, p->d_vhi, p->d_vlo, p->d_Epart, p->d_Npart, p->d_result,
                   p->d_rho, p->d_grho, p->d_Ptmp, p->d_Vtmp, p->d_watoms, p->d_wsmall, p->d_wlarge, p->d_wbox, p->d_paircnt};
   for (void* q : ptrs) if (q) cudaFree(q);
@@ -157,7 +157,7 @@ int xc_plan_create(const xc_atom* atoms, int32_t natoms, const xc_shell* shells,
   UP(d_atoms, hp.atoms);
   UP(d_invR, ptab);
   UP(d_shells, hp.shells); UP(d_exps, hp.exps); UP(d_coefs, hp.coefs);
-  UP(d_batches, hp.batches); UP(d_bshells, hp.bshells); UP(d_bsfoff, hp.bsfoff); UP(d_bfidx, hp.bfidx); UP(d_bfinfo, hp.bfinfo);
+  UP(d_batches, hp.batches); UP(d_bshells, hp.bshells); UP(d_bsfoff, hp.bsfoff); UP(d_bfidx, hp.bfidx);
   UP(d_wbox, hp.wbox);
   UP(d_watoms, hp.watoms); UP(d_wsmall, hp.wbatch_small); UP(d_wlarge, hp.wbatch_large);
   UP(d_ids_small, hp.ids_small); UP(d_ids_large, hp.ids_large);
@@ -265,7 +265,7 @@ int xc_eval(xc_plan* p, const double* dP, int64_t ldp, double* dV, int64_t ldv, 
   CU(cudaEventRecord(p->ev[ie++], st));
   size_t nb2 = (size_t)hp.nbasis * hp.nbasis;
   BatchArgs ba;
-  ba.batches = p->d_batches; ba.bshells = p->d_bshells; ba.bsfoff = p->d_bsfoff; ba.bfidx = p->d_bfidx; ba.bfinfo = p->d_bfinfo;
+  ba.batches = p->d_batches; ba.bshells = p->d_bshells; ba.bsfoff = p->d_bsfoff; ba.bfidx = p->d_bfidx;
   ba.shells = p->d_shells; ba.exps = p->d_exps; ba.coefs = p->d_coefs;
   ba.px = p->d_px; ba.py = p->d_py; ba.pz = p->d_pz; ba.w = p->d_w;
   ba.P = dP; ba.ldp = ldp; ba.ppk = p->d_ppk;

@@ -20,7 +20,7 @@ constexpr int kWeightSmallList = 256; // SSF weights kernel: atom-list length th
 
 struct ShellRec {      // 48 bytes
   double x, y, z;      // centre
-  int32_t L, nprim, prim_off, func_off;  // func_off: first GLOBAL function index
+  int32_t L, nprim, prim_off, func_off;  // L: shell type (nfun); func_off: first GLOBAL function index
   int32_t atom, _pad;
 };
 
@@ -36,7 +36,9 @@ struct BatchRec {      // one quadrature batch B_j with its shell list S_j (PAPE
 
 
 
-inline int ncart(int L) { return (L + 1) * (L + 2) / 2; }
+// ShellRec::L holds a shell TYPE: 0 = s, 1 = p, 2 = Cartesian d, 3 = pure d (XC_SHELL_PURE; reading A19)
+constexpr int kPureD = 3;
+inline int nfun(int type) { return type == kPureD ? 5 : (type + 1) * (type + 2) / 2; }
 inline int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
 
 // shared-memory footprint of the batch kernel for a batch (bytes); T = points per tile
@@ -59,7 +61,6 @@ struct HostPlan {
   std::vector<int32_t> bshells;        // concatenated S_j (global shell ids, ascending)
   std::vector<int32_t> bsfoff;         // per entry of bshells: first LOCAL function index of that shell in its batch
   std::vector<int32_t> bfidx;          // concatenated global function indices of S_j
-  std::vector<int32_t> bfinfo;         // per local function: (local shell slot << 8) | (l<<4 | m<<2 | n)
   std::vector<int32_t> watoms;         // concatenated per-batch atom lists of the weights kernel (sorted by distance to the batch box)
   std::vector<double> wbox;            // [nbatch][6] tight bounding boxes
   std::vector<int32_t> wbatch_small, wbatch_large;  // SSF weights kernel: batches with non-trivial points, by list length (two launches)

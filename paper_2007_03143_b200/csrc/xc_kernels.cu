@@ -100,6 +100,7 @@ __device__ __forceinline__ void grad_cart(int info, double dx, double dy, double
 // vr = df/drho, vs = df/dsigma, sigma = |grad rho|^2 (A10-A12).
 // ------------------------------------------------------------------------------------------------
 #define XC_PI 3.14159265358979323846264338327950288
+constexpr double kSqrt3 = 1.7320508075688772935274463415058724;
 #define XC_CX 0.7385587663820224058842300326808360  // (3/4)(3/pi)^(1/3)
 #define XC_RSFAC 0.6203504908994000166680068120477781  // (3/(4 pi))^(1/3)
 
@@ -385,7 +386,6 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
   double* sRed = (double*)sp; sp += (size_t)NT * 4 * 8; // partial rho / grad rho: [groups][4][T]
   double* sExpT = (double*)sp; sp += (size_t)64 * 8;    // 2^(j/64)
   ShellRec* sSh = (ShellRec*)sp; sp += (size_t)ns * sizeof(ShellRec);
-  int* sInfo = (int*)sp; sp += (size_t)nb16 * 4;
   int* sIdx = (int*)sp; sp += (size_t)nb16 * 4;
   int* sOrd = (int*)sp; sp += (size_t)((ns + 3) & ~3) * 4;   // [ns] shell slots, most primitives first
   double2* sPrim = (double2*)sp;                        // (alpha, d) of the batch's primitives, shell by shell
@@ -420,7 +420,6 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
   // ---- per batch: metadata, zero padding rows, V^j block assignment ----
   {
     const int32_t* fidx = a.bfidx + b.f_off;
-    const int32_t* finfo = a.bfinfo + b.f_off;
     for (int k = tid; k < ns; k += NT) {
       ShellRec r = a.shells[a.bshells[b.sh_off + k]];
       r._pad = a.bsfoff[b.sh_off + k];         // first local function of the shell
@@ -429,7 +428,6 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
     }
     for (int f = tid; f < nb16; f += NT) {
       sIdx[f] = f < nb ? fidx[f] : 0;
-      sInfo[f] = f < nb ? finfo[f] : 0;
     }
     for (int e = tid; e < (nb16 - nb) * LD; e += NT) {
       sPhi[(size_t)nb * LD + e] = 0.0;
@@ -508,10 +506,15 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
         dst[0] = R0;
       } else if (sh.L == 1) {
         dst[0] = dx * R0; dst[LD] = dy * R0; dst[2 * LD] = dz * R0;
-      } else {
+      } else if (sh.L == 2) {
         const double xr = dx * R0, yr = dy * R0;
         dst[0] = dx * xr; dst[LD] = dy * xr; dst[2 * LD] = dz * xr;
         dst[3 * LD] = dy * yr; dst[4 * LD] = dz * yr; dst[5 * LD] = dz * dz * R0;
+      } else {
+        // pure d (reading A19), m = -2..2: sqrt3 xy, sqrt3 yz, zz - (xx + yy)/2, sqrt3 xz, (sqrt3/2)(xx - yy)
+        const double xr = dx * R0, yr = dy * R0, zr = dz * R0;
+        dst[0] = kSqrt3 * dy * xr; dst[LD] = kSqrt3 * dz * yr; dst[2 * LD] = fma(dz, zr, -0.5 * fma(dx, xr, dy * yr));
+        dst[3 * LD] = kSqrt3 * dz * xr; dst[4 * LD] = (0.5 * kSqrt3) * fma(dx, xr, -dy * yr);
       }
     }
     __syncthreads();
@@ -602,7 +605,15 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
           Gx = xp[0]; Gy = xp[LD]; Gz = xp[2 * LD];
           S0 = fma(Gx, dx, fma(Gy, dy, Gz * dz));
         } else {
-          const double Xxx = xp[0], Xxy = xp[LD], Xxz = xp[2 * LD], Xyy = xp[3 * LD], Xyz = xp[4 * LD], Xzz = xp[5 * LD];
+          double Xxx, Xxy, Xxz, Xyy, Xyz, Xzz;
+          if (sh.L == 2) {
+            Xxx = xp[0]; Xxy = xp[LD]; Xxz = xp[2 * LD]; Xyy = xp[3 * LD]; Xyz = xp[4 * LD]; Xzz = xp[5 * LD];
+          } else {
+            // pure d: sum_q X_q d_q = sum_c (T^T X)_c (Cartesian d)_c
+            const double X0 = xp[0], X1 = xp[LD], X2 = xp[2 * LD], X3 = xp[3 * LD], X4 = xp[4 * LD];
+            Xxx = fma(0.5 * kSqrt3, X4, -0.5 * X2); Xyy = fma(-0.5 * kSqrt3, X4, -0.5 * X2); Xzz = X2;
+            Xxy = kSqrt3 * X0; Xyz = kSqrt3 * X1; Xxz = kSqrt3 * X3;
+          }
           Gx = fma(2.0 * Xxx, dx, fma(Xxy, dy, Xxz * dz));
           Gy = fma(Xxy, dx, fma(2.0 * Xyy, dy, Xyz * dz));
           Gz = fma(Xxz, dx, fma(Xyz, dy, 2.0 * Xzz * dz));
@@ -687,12 +698,18 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
         } else {
           const double bx = dx * base, by = dy * base;
           const double r0 = R.x;
-          zp[0] = fma(dx, bx, 2.0 * r0 * dx * g0);
-          zp[LD] = fma(dy, bx, r0 * fma(dy, g0, dx * g1));
-          zp[2 * LD] = fma(dz, bx, r0 * fma(dz, g0, dx * g2));
-          zp[3 * LD] = fma(dy, by, 2.0 * r0 * dy * g1);
-          zp[4 * LD] = fma(dz, by, r0 * fma(dz, g1, dy * g2));
-          zp[5 * LD] = fma(dz * dz, base, 2.0 * r0 * dz * g2);
+          const double Zxx = fma(dx, bx, 2.0 * r0 * dx * g0);
+          const double Zxy = fma(dy, bx, r0 * fma(dy, g0, dx * g1));
+          const double Zxz = fma(dz, bx, r0 * fma(dz, g0, dx * g2));
+          const double Zyy = fma(dy, by, 2.0 * r0 * dy * g1);
+          const double Zyz = fma(dz, by, r0 * fma(dz, g1, dy * g2));
+          const double Zzz = fma(dz * dz, base, 2.0 * r0 * dz * g2);
+          if (sh.L == 2) {
+            zp[0] = Zxx; zp[LD] = Zxy; zp[2 * LD] = Zxz; zp[3 * LD] = Zyy; zp[4 * LD] = Zyz; zp[5 * LD] = Zzz;
+          } else {                                  // pure d: Z_q = sum_c T_qc (Cartesian Z)_c
+            zp[0] = kSqrt3 * Zxy; zp[LD] = kSqrt3 * Zyz; zp[2 * LD] = Zzz - 0.5 * (Zxx + Zyy);
+            zp[3 * LD] = kSqrt3 * Zxz; zp[4 * LD] = (0.5 * kSqrt3) * (Zxx - Zyy);
+          }
         }
       }
       __syncthreads();

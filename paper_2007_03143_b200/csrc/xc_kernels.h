@@ -11,7 +11,6 @@ struct BatchArgs {
   const int32_t* bshells;
   const int32_t* bsfoff;
   const int32_t* bfidx;
-  const int32_t* bfinfo;
   const ShellRec* shells;
   const double* exps;
   const double* coefs;

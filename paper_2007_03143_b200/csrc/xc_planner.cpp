@@ -105,7 +105,7 @@ size_t batch_smem_bytes(int T, bool gga, int nb, int ns, int npr, int nthreads) 
   b += 64 * 8;                                   // 2^(j/64) table of the collocation exp
   b += (size_t)npr * 16;                         // (exponent, coefficient) of the batch's primitives
   b += (size_t)ns * sizeof(ShellRec);            // shell records
-  b += nb16 * 4 * 2;                             // function info + global function index
+  b += nb16 * 4;                                 // global function index
   b += (size_t)((ns + 3) & ~3) * 4;              // collocation order
   return b + 64;
 }
@@ -187,12 +187,15 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     if (sh.atom < 0 || sh.atom >= natoms || sh.nprim < 1 || sh.prim_off < 0 || sh.prim_off + sh.nprim > nprim_total || sh.L < 0) {
       err = "bad shell record"; return XC_EINVAL;
     }
-    if (sh.L > kMaxL) { err = "angular momentum L > 2 is not supported"; return XC_EUNSUPPORTED; }
+    if ((sh.L & ~(0xff | XC_SHELL_PURE)) != 0) { err = "bad shell record (unknown bits in L)"; return XC_EINVAL; }
+    const int Lq = sh.L & 0xff;
+    if (Lq > kMaxL) { err = "angular momentum L > 2 is not supported"; return XC_EUNSUPPORTED; }
+    const int type = ((sh.L & XC_SHELL_PURE) && Lq == 2) ? kPureD : Lq;   // a pure s or p shell is the Cartesian one
     if (sh.nprim > kMaxPrim) { err = "contraction depth > 16 is not supported"; return XC_EUNSUPPORTED; }
     ShellRec& r = hp.shells[s];
     r.x = atoms[sh.atom].x; r.y = atoms[sh.atom].y; r.z = atoms[sh.atom].z;
-    r.L = sh.L; r.nprim = sh.nprim; r.prim_off = sh.prim_off; r.func_off = foff; r.atom = sh.atom; r._pad = 0;
-    foff += ncart(sh.L);
+    r.L = type; r.nprim = sh.nprim; r.prim_off = sh.prim_off; r.func_off = foff; r.atom = sh.atom; r._pad = 0;
+    foff += nfun(type);
     double m = 0.0;  // Eq. (10)
     for (int k = 0; k < sh.nprim; ++k) {
       double al = exps[sh.prim_off + k];
@@ -305,7 +308,7 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     for (int a = 0; a < natoms; ++a) {
       if (!sphere_hits_box(&hp.atoms[3 * a], atom_rmax[a], b)) continue;
       for (int s : atom_shells[a])
-        if (sphere_hits_box(&hp.atoms[3 * a], hp.rcut[s], b)) { out.push_back(s); nb += ncart(hp.shells[s].L); }
+        if (sphere_hits_box(&hp.atoms[3 * a], hp.rcut[s], b)) { out.push_back(s); nb += nfun(hp.shells[s].L); }
     }
     std::sort(out.begin(), out.end());
   };
@@ -448,7 +451,7 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     if (sh_off >= ((int64_t)1 << 31) || f_off >= ((int64_t)1 << 31)) { err = "batch lists exceed 2^31 entries"; return XC_EUNSUPPORTED; }
   }
   hp.ppk_doubles = ppk;
-  hp.bshells.resize(sh_off); hp.bsfoff.resize(sh_off); hp.bfidx.resize(f_off); hp.bfinfo.resize(f_off);
+  hp.bshells.resize(sh_off); hp.bsfoff.resize(sh_off); hp.bfidx.resize(f_off);
 #pragma omp parallel for schedule(dynamic, 64)
   for (int64_t j = 0; j < nbatch; ++j) {
     const BatchRec& b = hp.batches[j];
@@ -457,13 +460,7 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
       int s = lists[j][k];
       hp.bshells[b.sh_off + k] = s;
       hp.bsfoff[b.sh_off + k] = f - b.f_off;
-      int L = hp.shells[s].L, c = 0;
-      for (int l = L; l >= 0; --l)
-        for (int m = L - l; m >= 0; --m, ++c, ++f) {
-          int n = L - l - m;
-          hp.bfidx[f] = hp.shells[s].func_off + c;
-          hp.bfinfo[f] = (k << 8) | (l << 4) | (m << 2) | n;
-        }
+      for (int c = 0; c < nfun(hp.shells[s].L); ++c, ++f) hp.bfidx[f] = hp.shells[s].func_off + c;
     }
   }
   hp.sum_nbnq = hp.sum_nb2 = hp.flops = 0; hp.max_nb = hp.max_ns = 0; hp.smem_small = hp.smem_large = 0;

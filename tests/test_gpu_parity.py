@@ -94,6 +94,17 @@ def test_w27_pbe(xc, orc):
     plan.close()
 
 
+@pytest.mark.parametrize("name", ["p1", "p8", "p8l", "p27"])
+def test_pure_d_shells(xc, orc, name):
+    """the O d shell as five pure functions (XC_SHELL_PURE), monomer / 8 / 27
+    waters, PBE and (p8l) LDA: every output against the oracle, which holds its own statement of the transformation."""
+    w = make_workload(name)
+    assert w.n_basis == 24 * len(w.atoms_Z) // 3
+    _, plan, g, r = _full_parity(orc, name, w.functional)
+    assert plan.n_basis == w.n_basis
+    plan.close()
+
+
 def test_c2_lda_64_waters(xc, orc):
     w, plan, g, r = _full_parity(orc, "c2", 0)
     assert abs(g["N"] - 640.0) / 640.0 < 2e-4
@@ -166,6 +177,13 @@ def test_determinism_ld_host_path_and_one_shot(xc, orc):
 
 
 def test_error_codes(xc):
+    w0 = make_workload("c1")
+    bad_L = w0.shell_L.copy()
+    bad_L[0] |= 0x200                                        # unknown bit in xc_shell.L
+    with pytest.raises(xc.XcError) as e0:
+        xc.Plan(w0.atoms_xyz, w0.atoms_Z, w0.shell_atom, bad_L, w0.shell_nprim, w0.shell_prim_off, w0.exps, w0.coefs,
+                xc.grid_spec(10, 26, 0))
+    assert e0.value.code == -1
     import torch
     w = make_workload("c1")
     with pytest.raises(xc.XcError) as e:
