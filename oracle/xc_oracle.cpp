@@ -14,6 +14,9 @@
 // sum w rho = tr(P S) (P2), V symmetric (P3), finite-difference dE/dP = V (P4), unscreened brute
 // force (P5), functional values vs 40-digit mpmath (P6), functional limits (P7), collocation vs
 // finite differences and closed-form overlaps (P8), plan validity (P9), translation invariance (P10);
+// spin-unrestricted path and tau (readings A20-A22; tests/test_oracle_uks.py): polarised functionals vs 40-digit mpmath,
+// ferromagnetic uniform gas, zeta = 0 and spin-scaling reductions to the pinned unpolarised forms, P_a = P_b limit,
+// tr(P_s S), dE/dP^s = V^s, int tau = (2L+3) alpha/2 for one primitive, tau against the einsum definition;
 // pure d shells (reading A19): typed values, orthonormality with s and p on a fine grid, Unsold's theorem, tr(PS), dE/dP = V.
 // Parity UNPINNED against the paper itself: the paper prints no E_xc / V_xc / N_el value.
 //
@@ -262,6 +265,136 @@ inline void shell_at_point(int code, int nprim, const double* alpha, const doubl
       }
     }
   }
+}
+
+
+// =============================================================================================================
+// Spin-unrestricted densities and the meta-GGA intermediate tau ("may be
+// extended to both spin-unrestricted ... as well as ... the meta-GGA with the addition of only a few intermediates").
+// DESIGN.md readings A20-A22.  Variables: rho_a, rho_b, s_aa = |grad rho_a|^2, s_ab = grad rho_a . grad rho_b,
+// s_bb = |grad rho_b|^2.  f = energy per unit volume; the five partial derivatives come from forward-mode duals.
+// =============================================================================================================
+struct D5 {
+  double v;
+  double d[5];
+};
+inline D5 mk5(double v) { return {v, {0, 0, 0, 0, 0}}; }
+inline D5 var5(double v, int k) { D5 r = mk5(v); r.d[k] = 1.0; return r; }
+inline D5 lin5(const D5& x, double fv, double fp) {   // g(x) with value fv and derivative fp at x.v
+  D5 r; r.v = fv;
+  for (int k = 0; k < 5; ++k) r.d[k] = fp * x.d[k];
+  return r;
+}
+inline D5 operator+(D5 x, D5 y) { D5 r; r.v = x.v + y.v; for (int k = 0; k < 5; ++k) r.d[k] = x.d[k] + y.d[k]; return r; }
+inline D5 operator-(D5 x, D5 y) { D5 r; r.v = x.v - y.v; for (int k = 0; k < 5; ++k) r.d[k] = x.d[k] - y.d[k]; return r; }
+inline D5 operator-(D5 x) { D5 r; r.v = -x.v; for (int k = 0; k < 5; ++k) r.d[k] = -x.d[k]; return r; }
+inline D5 operator*(D5 x, D5 y) { D5 r; r.v = x.v * y.v; for (int k = 0; k < 5; ++k) r.d[k] = x.d[k] * y.v + x.v * y.d[k]; return r; }
+inline D5 operator/(D5 x, D5 y) {
+  D5 r; r.v = x.v / y.v;
+  for (int k = 0; k < 5; ++k) r.d[k] = (x.d[k] - r.v * y.d[k]) / y.v;
+  return r;
+}
+inline D5 operator+(D5 x, double c) { x.v += c; return x; }
+inline D5 operator+(double c, D5 x) { x.v += c; return x; }
+inline D5 operator-(D5 x, double c) { x.v -= c; return x; }
+inline D5 operator-(double c, D5 x) { return mk5(c) - x; }
+inline D5 operator*(D5 x, double c) { x.v *= c; for (int k = 0; k < 5; ++k) x.d[k] *= c; return x; }
+inline D5 operator*(double c, D5 x) { return x * c; }
+inline D5 operator/(D5 x, double c) { return x * (1.0 / c); }
+inline D5 operator/(double c, D5 x) { return mk5(c) / x; }
+inline D5 dlog(D5 x) { return lin5(x, std::log(x.v), 1.0 / x.v); }
+inline D5 dexp(D5 x) { double e = std::exp(x.v); return lin5(x, e, e); }
+inline D5 datan(D5 x) { return lin5(x, std::atan(x.v), 1.0 / (1.0 + x.v * x.v)); }
+inline D5 dsqrt(D5 x) { double s = std::sqrt(x.v); return lin5(x, s, 0.5 / s); }
+inline D5 dcbrt(D5 x) { double c = std::cbrt(x.v); return lin5(x, c, c / (3.0 * x.v)); }
+inline D5 dpow(D5 x, double p) { double w = std::pow(x.v, p); return lin5(x, w, p * w / x.v); }   // x.v > 0
+
+// f(zeta) = ((1+z)^(4/3) + (1-z)^(4/3) - 2) / (2^(4/3) - 2) and f''(0) = 4 / (9 (2^(1/3) - 1))   (von Barth-Hedin form)
+inline D5 f_zeta(D5 z) { return (dpow(1.0 + z, 4.0 / 3.0) + dpow(1.0 - z, 4.0 / 3.0) - 2.0) / (std::pow(2.0, 4.0 / 3.0) - 2.0); }
+const double kFpp0 = 4.0 / (9.0 * (std::cbrt(2.0) - 1.0));
+
+// VWN 1980 fit "V" interpolation G(x; A, x0, b, c), x = sqrt(r_s): paramagnetic, ferromagnetic and spin-stiffness sets
+inline D5 vwn_G(D5 x, double A, double x0, double b, double c) {
+  const double Q = std::sqrt(4.0 * c - b * b);
+  const double X0 = x0 * x0 + b * x0 + c;
+  D5 X = x * x + b * x + c;
+  D5 at = datan(Q / (2.0 * x + b));
+  return A * (dlog(x * x / X) + (2.0 * b / Q) * at - (b * x0 / X0) * (dlog((x - x0) * (x - x0) / X) + (2.0 * (b + 2.0 * x0) / Q) * at));
+}
+// Slater exchange, spin-scaled: E_x[ra, rb] = (E_x[2 ra] + E_x[2 rb]) / 2
+inline D5 f_slater_pol(D5 ra, D5 rb) { return -kCx * 0.5 * (2.0 * ra * dcbrt(2.0 * ra) + 2.0 * rb * dcbrt(2.0 * rb)); }
+// VWN5 correlation energy per particle at (r_s, zeta):
+// eps = eps_P + alpha_c f(z)/f''(0) (1 - z^4) + (eps_F - eps_P) f(z) z^4
+inline D5 eps_vwn5_pol(D5 rho, D5 zeta) {
+  D5 x = dsqrt(dcbrt(mk5(3.0 / (4.0 * kPi)) / rho));
+  D5 eP = vwn_G(x, 0.0310907, -0.10498, 3.72744, 12.9352);
+  D5 eF = vwn_G(x, 0.01554535, -0.32500, 7.06042, 18.0578);
+  D5 ac = vwn_G(x, -1.0 / (6.0 * kPi * kPi), -0.0047584, 1.13107, 13.0045);
+  D5 fz = f_zeta(zeta), z4 = zeta * zeta * zeta * zeta;
+  return eP + ac * (fz / kFpp0) * (1.0 - z4) + (eF - eP) * fz * z4;
+}
+// PW92 G(r_s; A, a1, b1..b4) and the interpolation in zeta (the third set fits -alpha_c)
+inline D5 pw92_G(D5 r, double A, double a1, double b1, double b2, double b3, double b4) {
+  D5 sr = dsqrt(r);
+  D5 q = 2.0 * A * (b1 * sr + b2 * r + b3 * r * sr + b4 * r * r);
+  return -2.0 * A * (1.0 + a1 * r) * dlog(1.0 + 1.0 / q);
+}
+inline D5 eps_pw92_pol(D5 rho, D5 zeta) {
+  D5 r = dcbrt(mk5(3.0 / (4.0 * kPi)) / rho);
+  D5 e0 = pw92_G(r, 0.0310907, 0.21370, 7.5957, 3.5876, 1.6382, 0.49294);
+  D5 e1 = pw92_G(r, 0.01554535, 0.20548, 14.1189, 6.1977, 3.3662, 0.62517);
+  D5 mac = pw92_G(r, 0.0168869, 0.11125, 10.357, 3.6231, 0.88026, 0.49671);   // = -alpha_c
+  D5 fz = f_zeta(zeta), z4 = zeta * zeta * zeta * zeta;
+  return e0 - mac * (fz / kFpp0) * (1.0 - z4) + (e1 - e0) * fz * z4;
+}
+// PBE exchange of one spin channel at density 2 r, sigma 4 s (spin scaling), per unit volume
+inline D5 f_pbe_x_channel(D5 r2, D5 s4) {
+  const double kappa = 0.804, mu = 0.2195149727645171;
+  D5 s2 = s4 / (4.0 * std::pow(3.0 * kPi * kPi, 2.0 / 3.0) * dpow(r2, 8.0 / 3.0));
+  D5 F = 1.0 + kappa - kappa / (1.0 + mu * s2 / kappa);
+  return -kCx * r2 * dcbrt(r2) * F;
+}
+inline D5 f_pbe_x_pol(D5 ra, D5 rb, D5 saa, D5 sbb) {
+  return 0.5 * (f_pbe_x_channel(2.0 * ra, 4.0 * saa) + f_pbe_x_channel(2.0 * rb, 4.0 * sbb));
+}
+// PBE correlation at (rho, zeta, sigma = |grad rho|^2): rho (eps_unif + H), phi = ((1+z)^(2/3) + (1-z)^(2/3)) / 2,
+// t^2 = sigma / (4 phi^2 k_s^2 rho^2), A = (beta/gamma) / (exp(-eps/(gamma phi^3)) - 1)
+inline D5 f_pbe_c_pol(D5 rho, D5 zeta, D5 sigma) {
+  const double gamma = (1.0 - std::log(2.0)) / (kPi * kPi), beta = 0.06672455060314922;
+  D5 eu = eps_pw92_pol(rho, zeta);
+  D5 phi = 0.5 * (dpow(1.0 + zeta, 2.0 / 3.0) + dpow(1.0 - zeta, 2.0 / 3.0));
+  D5 phi3 = phi * phi * phi;
+  D5 kF = dcbrt(3.0 * kPi * kPi * rho);
+  D5 ks2 = 4.0 * kF / kPi;
+  D5 t2 = sigma / (4.0 * phi * phi * ks2 * rho * rho);
+  D5 Ac = (beta / gamma) / (dexp(-eu / (gamma * phi3)) - 1.0);
+  D5 At2 = Ac * t2;
+  D5 H = gamma * phi3 * dlog(1.0 + (beta / gamma) * t2 * (1.0 + At2) / (1.0 + At2 + At2 * At2));
+  return rho * (eu + H);
+}
+// kind: 0 = LDA Slater+VWN5, 1 = GGA PBE; pin kinds 2 = Slater, 3 = VWN5 (rho eps), 4 = PW92 (rho eps), 5 = PBE x, 6 = PBE c
+inline D5 f_xc_pol(int kind, D5 ra, D5 rb, D5 saa, D5 sab, D5 sbb) {
+  D5 rho = ra + rb, zeta = (ra - rb) / rho, sigma = saa + 2.0 * sab + sbb;
+  switch (kind) {
+    case 0: return f_slater_pol(ra, rb) + rho * eps_vwn5_pol(rho, zeta);
+    case 1: return f_pbe_x_pol(ra, rb, saa, sbb) + f_pbe_c_pol(rho, zeta, sigma);
+    case 2: return f_slater_pol(ra, rb);
+    case 3: return rho * eps_vwn5_pol(rho, zeta);
+    case 4: return rho * eps_pw92_pol(rho, zeta);
+    case 5: return f_pbe_x_pol(ra, rb, saa, sbb);
+    default: return f_pbe_c_pol(rho, zeta, sigma);
+  }
+}
+// Reading A20: a point contributes nothing when rho_a + rho_b <= rho_tol; otherwise a spin density below rho_tol is
+// raised to rho_tol before the functional is evaluated (zeta = +-1 is a singular point of the zeta interpolation), and
+// the derivative with respect to it is the one at the raised value.
+inline void eval_point_pol(int kind, double ra, double rb, double saa, double sab, double sbb, double rho_tol, double* f, double* v) {
+  *f = 0.0;
+  for (int k = 0; k < 5; ++k) v[k] = 0.0;
+  if (ra + rb <= rho_tol) return;
+  D5 r = f_xc_pol(kind, var5(std::max(ra, rho_tol), 0), var5(std::max(rb, rho_tol), 1), var5(saa, 2), var5(sab, 3), var5(sbb, 4));
+  *f = r.v;
+  for (int k = 0; k < 5; ++k) v[k] = r.d[k];
 }
 
 }  // namespace
@@ -809,6 +942,132 @@ double orc_plan_flops(int64_t nbatch, const int64_t* batch_off, const int64_t* s
     tot += 4.0 * nb * nb * (double)(batch_off[j + 1] - batch_off[j]);
   }
   return tot;
+}
+
+// Spin-polarised functional exposed (A20): f and the five partials at n points.
+void orc_functional_pol(int kind, int64_t n, const double* ra, const double* rb, const double* saa, const double* sab,
+                        const double* sbb, double rho_tol, double* f, double* v5 /* [n][5]: d/d ra, rb, saa, sab, sbb */) {
+  for (int64_t i = 0; i < n; ++i)
+    eval_point_pol(kind, ra[i], rb[i], saa ? saa[i] : 0.0, sab ? sab[i] : 0.0, sbb ? sbb[i] : 0.0, rho_tol, f + i, v5 + 5 * i);
+}
+
+// Alg. 4, Mode A, for spin-unrestricted densities (readings A20-A22):
+//   X^s = P^s,j Phi^j;  rho_s,i = sum_mu Phi X^s;  grad rho_s,i = 2 sum_mu grad Phi X^s          (Eqs. (13)-(15) per spin)
+//   tau_s,i = 1/2 sum_mu grad Phi_mu,i . grad X^s_mu,i,  grad X^s = P^s,j grad Phi^j              (meta-GGA intermediate)
+//   Z^s = 1/2 (w v_rho_s) Phi + w (2 v_s_ss grad rho_s + v_s_ab grad rho_s') . grad Phi;  V^s,j = Z^s Phi^T + Phi Z^s^T
+// P_a, P_b: N_b x N_b (ld = ldp) with rho_s = sum P^s phi phi (no factor 2).  Va, Vb (may be null) are INCREMENTED.
+// rho_out [2][npts], grho_out [2][npts][3], tau_out [2][npts] may be null.  N_out[2] = (N_a, N_b).
+void orc_eval_uks(int64_t nbatch, const int64_t* batch_off, const int64_t* shell_off, const int32_t* shells,
+                  const int64_t* subset, int64_t nsub, int64_t npts, const double* pts, const double* w, const int32_t* shell_atom,
+                  const int32_t* shell_L, const int32_t* shell_nprim, const int32_t* shell_prim_off,
+                  const int32_t* func_off, const double* exps, const double* coefs, const double* xyz, int nbasis,
+                  const double* Pa, const double* Pb, int64_t ldp, int kind, double rho_tol, double* Va, double* Vb,
+                  double* E_out, double* N_out, double* rho_out, double* grho_out, double* tau_out) {
+  const bool gga = is_gga(kind);
+  int64_t njobs = subset ? nsub : nbatch;
+  std::vector<long double> Eb(njobs, 0.0L), Na(njobs, 0.0L), Nb(njobs, 0.0L);
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int64_t job = 0; job < njobs; ++job) {
+    int64_t j = subset ? subset[job] : job;
+    int64_t q0 = batch_off[j], nq = batch_off[j + 1] - q0;
+    const int32_t* S = shells + shell_off[j];
+    int ns = (int)(shell_off[j + 1] - shell_off[j]);
+    std::vector<int> fidx;
+    for (int k = 0; k < ns; ++k)
+      for (int c = 0; c < nfun(shell_L[S[k]]); ++c) fidx.push_back(func_off[S[k]] + c);
+    size_t nb = fidx.size();
+    if (nb == 0 || nq == 0) continue;
+    const bool need_grad = gga || tau_out;
+    std::vector<double> Phi(nb * nq), G[3];
+    if (need_grad) for (int c = 0; c < 3; ++c) G[c].resize(nb * nq);
+    orc_collocation(ns, S, shell_atom, shell_L, shell_nprim, shell_prim_off, exps, coefs, xyz, nq, pts + 3 * q0,
+                    Phi.data(), need_grad ? G[0].data() : nullptr, need_grad ? G[1].data() : nullptr, need_grad ? G[2].data() : nullptr);
+    // per spin: P^s,j, X^s, rho_s, grad rho_s, tau_s
+    std::vector<double> rho[2], gr[2][3], tau[2];
+    for (int s = 0; s < 2; ++s) {
+      const double* P = s == 0 ? Pa : Pb;
+      std::vector<double> X(nb * nq, 0.0);
+      for (size_t m = 0; m < nb; ++m)
+        for (size_t n = 0; n < nb; ++n) {
+          double p = P[(size_t)fidx[m] * ldp + fidx[n]];
+          for (int64_t i = 0; i < nq; ++i) X[m * nq + i] += p * Phi[n * nq + i];
+        }
+      rho[s].assign(nq, 0.0);
+      for (int c = 0; c < 3; ++c) gr[s][c].assign(nq, 0.0);
+      for (size_t m = 0; m < nb; ++m)
+        for (int64_t i = 0; i < nq; ++i) {
+          rho[s][i] += Phi[m * nq + i] * X[m * nq + i];
+          if (need_grad)
+            for (int c = 0; c < 3; ++c) gr[s][c][i] += 2.0 * G[c][m * nq + i] * X[m * nq + i];
+        }
+      if (tau_out) {
+        tau[s].assign(nq, 0.0);
+        for (int c = 0; c < 3; ++c) {
+          std::vector<double> GX(nb * nq, 0.0);   // grad_c X^s = P^s,j grad_c Phi^j
+          for (size_t m = 0; m < nb; ++m)
+            for (size_t n = 0; n < nb; ++n) {
+              double p = P[(size_t)fidx[m] * ldp + fidx[n]];
+              for (int64_t i = 0; i < nq; ++i) GX[m * nq + i] += p * G[c][n * nq + i];
+            }
+          for (size_t m = 0; m < nb; ++m)
+            for (int64_t i = 0; i < nq; ++i) tau[s][i] += 0.5 * G[c][m * nq + i] * GX[m * nq + i];
+        }
+      }
+    }
+    // functional (A20), energy and electron counts
+    std::vector<double> a[2], gz[2][3];   // Z^s = a_s Phi + gz_s . grad Phi
+    for (int s = 0; s < 2; ++s) { a[s].resize(nq); for (int c = 0; c < 3; ++c) gz[s][c].assign(nq, 0.0); }
+    long double e = 0.0L, na = 0.0L, nbl = 0.0L;
+    for (int64_t i = 0; i < nq; ++i) {
+      double saa = 0.0, sab = 0.0, sbb = 0.0;
+      if (gga)
+        for (int c = 0; c < 3; ++c) { saa += gr[0][c][i] * gr[0][c][i]; sab += gr[0][c][i] * gr[1][c][i]; sbb += gr[1][c][i] * gr[1][c][i]; }
+      double f, v[5];
+      eval_point_pol(kind, rho[0][i], rho[1][i], saa, sab, sbb, rho_tol, &f, v);
+      const double wi = w[q0 + i];
+      a[0][i] = 0.5 * wi * v[0];
+      a[1][i] = 0.5 * wi * v[1];
+      if (gga)
+        for (int c = 0; c < 3; ++c) {
+          gz[0][c][i] = wi * (2.0 * v[2] * gr[0][c][i] + v[3] * gr[1][c][i]);
+          gz[1][c][i] = wi * (2.0 * v[4] * gr[1][c][i] + v[3] * gr[0][c][i]);
+        }
+      e += (long double)wi * (long double)f;
+      na += (long double)wi * (long double)rho[0][i];
+      nbl += (long double)wi * (long double)rho[1][i];
+      for (int s = 0; s < 2; ++s) {
+        if (rho_out) rho_out[(size_t)s * npts + q0 + i] = rho[s][i];
+        if (grho_out && need_grad) for (int c = 0; c < 3; ++c) grho_out[((size_t)s * npts + q0 + i) * 3 + c] = gr[s][c][i];
+        if (tau_out) tau_out[(size_t)s * npts + q0 + i] = tau[s][i];
+      }
+    }
+    Eb[job] = e; Na[job] = na; Nb[job] = nbl;
+    for (int s = 0; s < 2; ++s) {
+      double* V = s == 0 ? Va : Vb;
+      if (!V) continue;
+      std::vector<double> Z(nb * nq);
+      for (size_t m = 0; m < nb; ++m)
+        for (int64_t i = 0; i < nq; ++i) {
+          double z = a[s][i] * Phi[m * nq + i];
+          if (gga) for (int c = 0; c < 3; ++c) z += gz[s][c][i] * G[c][m * nq + i];
+          Z[m * nq + i] = z;
+        }
+      std::vector<double> Vj(nb * nb, 0.0);
+      for (size_t m = 0; m < nb; ++m)
+        for (size_t n = 0; n < nb; ++n) {
+          double acc = 0.0;
+          for (int64_t i = 0; i < nq; ++i) acc += Z[m * nq + i] * Phi[n * nq + i] + Phi[m * nq + i] * Z[n * nq + i];
+          Vj[m * nb + n] = acc;
+        }
+#pragma omp critical(orc_v_increment_uks)
+      for (size_t m = 0; m < nb; ++m)
+        for (size_t n = 0; n < nb; ++n) V[(size_t)fidx[m] * nbasis + fidx[n]] += Vj[m * nb + n];
+    }
+  }
+  long double E = 0.0L, A = 0.0L, B = 0.0L;
+  for (int64_t job = 0; job < njobs; ++job) { E += Eb[job]; A += Na[job]; B += Nb[job]; }
+  if (E_out) *E_out = (double)E;
+  if (N_out) { N_out[0] = (double)A; N_out[1] = (double)B; }
 }
 
 }  // extern "C"

@@ -237,3 +237,55 @@ def evaluate_unscreened(pts, w, basis, xyz, P, kind, rho_tol=1e-15, want_V=True)
 def plan_flops(plan: Plan, shell_L) -> float:
     boff, soff, sh, sL = _i64(plan.batch_off), _i64(plan.shell_off), _i32(plan.shells), _i32(shell_L)
     return float(lib().orc_plan_flops(C.c_int64(len(boff) - 1), _l(boff), _l(soff), _i(sh), _i(sL)))
+
+
+def functional_pol(kind, ra, rb, saa=None, sab=None, sbb=None, rho_tol=1e-15):
+    """Spin-polarised functional (reading A20): f and d f / d (rho_a, rho_b, s_aa, s_ab, s_bb), shape (n, 5)."""
+    ra, rb = _f64(np.atleast_1d(ra)), _f64(np.atleast_1d(rb))
+    z = np.zeros_like(ra)
+    saa = z if saa is None else _f64(np.atleast_1d(saa))
+    sab = z if sab is None else _f64(np.atleast_1d(sab))
+    sbb = z if sbb is None else _f64(np.atleast_1d(sbb))
+    f = np.empty_like(ra)
+    v = np.empty((len(ra), 5))
+    lib().orc_functional_pol(C.c_int(kind), C.c_int64(len(ra)), _d(ra), _d(rb), _d(saa), _d(sab), _d(sbb),
+                             C.c_double(rho_tol), _d(f), _d(v))
+    return f, v
+
+
+@dataclasses.dataclass
+class ResultUks:
+    E_xc: float
+    N_a: float
+    N_b: float
+    Va: np.ndarray | None
+    Vb: np.ndarray | None
+    rho: np.ndarray | None = None        # (2, npts)
+    grad_rho: np.ndarray | None = None   # (2, npts, 3)
+    tau: np.ndarray | None = None        # (2, npts)
+
+
+def evaluate_uks(plan: Plan, w, basis, xyz, Pa, Pb, kind, rho_tol=1e-15, subset=None, want_V=True, want_rho=False,
+                 want_tau=False) -> ResultUks:
+    """Mode A evaluation for spin-unrestricted densities (rho_s = sum P^s phi phi) and the meta-GGA intermediate tau."""
+    sa, sL, sn, so, ex, co = basis
+    sa, sL, sn, so, ex, co = _i32(sa), _i32(sL), _i32(sn), _i32(so), _f64(ex), _f64(co)
+    foff, nbf = _func_off(sL)
+    xyz, Pa, Pb, w = _f64(xyz), _f64(Pa), _f64(Pb), _f64(w)
+    pts = _f64(plan.pts)
+    boff, soff, sh = _i64(plan.batch_off), _i64(plan.shell_off), _i32(plan.shells)
+    nbat = len(boff) - 1
+    sub = _i64(subset) if subset is not None else None
+    Va = np.zeros((nbf, nbf)) if want_V else None
+    Vb = np.zeros((nbf, nbf)) if want_V else None
+    n = len(pts)
+    rho = np.zeros((2, n)) if want_rho else None
+    gr = np.zeros((2, n, 3)) if want_rho else None
+    tau = np.zeros((2, n)) if want_tau else None
+    E = C.c_double(0.0)
+    N = (C.c_double * 2)(0.0, 0.0)
+    lib().orc_eval_uks(C.c_int64(nbat), _l(boff), _l(soff), _i(sh), _l(sub), C.c_int64(0 if sub is None else len(sub)),
+                       C.c_int64(n), _d(pts), _d(w), _i(sa), _i(sL), _i(sn), _i(so), _i(foff), _d(ex), _d(co), _d(xyz),
+                       C.c_int(nbf), _d(Pa), _d(Pb), C.c_int64(Pa.shape[1]), C.c_int(kind), C.c_double(rho_tol), _d(Va), _d(Vb),
+                       C.byref(E), N, _d(rho), _d(gr), _d(tau))
+    return ResultUks(E.value, N[0], N[1], Va, Vb, rho, gr, tau)

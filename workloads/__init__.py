@@ -6,4 +6,4 @@ functionals.  The only mathematics here is what is needed to *construct an input
 Gaussian overlap matrix S used to S-orthonormalise the random orbitals (so that tr(P S) = 2 N_occ).
 """
 from .water_clusters import (CONFIGS, Workload, make_workload, overlap_matrix,  # noqa: F401
-                             ncart, nfun, PURE, cart_components, ANGSTROM)
+                             ncart, nfun, PURE, cart_components, ANGSTROM, spin_density_matrices)

@@ -333,3 +333,16 @@ def make_workload(name: str, with_P: bool = True, cache: bool = True) -> Workloa
         np.save(tmp, P)
         os.replace(tmp, path)
     return w
+
+
+def spin_density_matrices(w: Workload, n_a: int, n_b: int, seed: int = 7):
+    """(P_a, P_b) of a spin-unrestricted determinant: P_s = C[:, :n_s] C[:, :n_s]^T with C random, S-orthonormal
+    (C^T S C = 1), so tr(P_s S) = n_s; n_b <= n_a (the first n_b orbitals are doubly occupied)."""
+    rng = np.random.default_rng(BASIS_SEED + 1000 + seed)
+    C = rng.standard_normal((w.n_basis, max(n_a, n_b)))
+    S = overlap_matrix(w)
+    M = C.T @ (S @ C)
+    Lc = np.linalg.cholesky(0.5 * (M + M.T))
+    C = np.linalg.solve(Lc, C.T).T
+    Pa, Pb = C[:, :n_a] @ C[:, :n_a].T, C[:, :n_b] @ C[:, :n_b].T
+    return 0.5 * (Pa + Pa.T), 0.5 * (Pb + Pb.T)
