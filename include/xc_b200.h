@@ -114,6 +114,24 @@ int xc_eval(xc_plan* plan, const double* dP, int64_t ldp, double* dV, int64_t ld
 int xc_eval_host(xc_plan* plan, const double* hP, int64_t ldp, double* hV, int64_t ldv,
                  double* E_xc, double* N_el, int32_t flags);
 
+/* Spin-unrestricted build ("may be extended to ... spin-unrestricted ... with the
+ * addition of only a few intermediates"; readings A20-A22).  rho_s = sum P^s_mu,nu phi_mu phi_nu for s = a, b (no factor 2:
+ * a closed shell is P^a = P^b = P/2), f = f(rho_a, rho_b, s_aa, s_ab, s_bb) is the spin-polarised Slater+VWN5 or PBE,
+ *   Z^s = 1/2 w v_rho_s Phi + w (2 v_ss grad rho_s + v_ab grad rho_s') . grad Phi,  V^s,j = Z^s Phi^T + Phi Z^s^T.
+ *   dPa, dPb [device] read-only, symmetric; dVa, dVb [device] OVERWRITTEN, symmetric, bit-identical from run to run.
+ *   E_xc [host] scalar; N_ab [host] two doubles: sum w rho_a, sum w rho_b.
+ *   A point contributes nothing when rho_a + rho_b <= rho_tol; a spin density below rho_tol is raised to rho_tol before
+ *   the functional is evaluated (zeta = +-1 is singular), so grid_spec.rho_tol must be > 0 (else XC_EINVAL).
+ *   flags: XC_EVAL_REUSE_WEIGHTS.  Error behaviour, re-entrancy and stream semantics as xc_eval.
+ * The same kernels run as passes: per spin {P^s,j pack, collocation + X GEMM + densities}, the functional over the grid,
+ * per spin {collocation + Z^s + V^s,j GEMM + increment, finalise}. */
+int xc_eval_uks(xc_plan* plan, const double* dPa, const double* dPb, int64_t ldp, double* dVa, double* dVb, int64_t ldv,
+                double* E_xc, double* N_ab, int32_t flags, void* cuda_stream);
+
+/* rho_s [2][n_points] and grad rho_s [2][n_points][3] (GGA plans) of the last xc_eval_uks, plan order, [host], either may
+ * be NULL; entries of points with w = 0 are undefined (never evaluated). */
+int xc_eval_uks_densities(const xc_plan* plan, double* rho, double* grad_rho);
+
 /* Diagnostics of the last xc_eval on this plan, for parity tests at full size.  All [host], may be NULL:
  *   w n_points final partition weights (plan order);  rho n_points;  grad_rho 3*n_points (zeros for LDA) -- these two
  *   only if that xc_eval ran with XC_EVAL_DIAG (else XC_EINVAL), and only at points with w != 0;

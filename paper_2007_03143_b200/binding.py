@@ -57,6 +57,8 @@ def _load():
     lib.xc_plan_export.argtypes = [vp, dp, dp, ip, lp, lp, lp, ip]
     lib.xc_eval.argtypes = [vp, vp, C.c_int64, vp, C.c_int64, dp, dp, C.c_int32, vp]
     lib.xc_eval_host.argtypes = [vp, vp, C.c_int64, vp, C.c_int64, dp, dp, C.c_int32]
+    lib.xc_eval_uks.argtypes = [vp, vp, vp, C.c_int64, vp, vp, C.c_int64, dp, dp, C.c_int32, vp]
+    lib.xc_eval_uks_densities.argtypes = [vp, dp, dp]
     lib.xc_eval_diagnostics.argtypes = [vp, dp, dp, dp, dp, dp]
     lib.xc_eval_timings.argtypes = [vp, C.POINTER(C.c_float), ip]
     lib.xc_eval_counters.argtypes = [vp, lp, lp]
@@ -71,7 +73,7 @@ def _load():
     return lib
 
 
-EXPORTED = ["xc_plan_create", "xc_plan_info", "xc_plan_export", "xc_eval", "xc_eval_host", "xc_eval_diagnostics",
+EXPORTED = ["xc_plan_create", "xc_plan_info", "xc_plan_export", "xc_eval", "xc_eval_host", "xc_eval_uks", "xc_eval_uks_densities", "xc_eval_diagnostics",
             "xc_eval_timings", "xc_eval_counters", "xc_plan_stats", "xc_plan_destroy", "xc_integrate", "xc_partition_weights",
             "xc_functional", "xc_measure_fp64_peak", "xc_strerror", "xc_last_error"]
 
@@ -184,6 +186,33 @@ class Plan:
                             C.byref(E), C.byref(N), (XC_EVAL_REUSE_WEIGHTS if reuse_weights else 0) | (XC_EVAL_DIAG if diag else 0) | (XC_EVAL_COUNT_PAIRS if count_pairs else 0),
                             _stream_ptr(stream)))
         return E.value, N.value, V
+
+    def eval_uks(self, Pa, Pb, Va=None, Vb=None, reuse_weights=False, stream=None):
+        """Spin-unrestricted build (xc_eval_uks): Pa, Pb torch CUDA float64 (n_basis x n_basis, same row stride).
+        Returns (E_xc, (N_a, N_b), Va, Vb)."""
+        import torch
+        for t in (Pa, Pb):
+            assert t.is_cuda and t.dtype == torch.float64 and t.dim() == 2 and t.stride(1) == 1
+        assert Pa.stride(0) == Pb.stride(0)
+        if Va is None:
+            Va = torch.empty((self.n_basis, self.n_basis), dtype=torch.float64, device=Pa.device)
+        if Vb is None:
+            Vb = torch.empty((self.n_basis, self.n_basis), dtype=torch.float64, device=Pa.device)
+        assert Va.stride(1) == 1 and Vb.stride(1) == 1 and Va.stride(0) == Vb.stride(0)
+        E = C.c_double()
+        N = (C.c_double * 2)()
+        _check(_lib.xc_eval_uks(self._h, C.c_void_p(Pa.data_ptr()), C.c_void_p(Pb.data_ptr()), Pa.stride(0),
+                                C.c_void_p(Va.data_ptr()), C.c_void_p(Vb.data_ptr()), Va.stride(0), C.byref(E), N,
+                                XC_EVAL_REUSE_WEIGHTS if reuse_weights else 0, _stream_ptr(stream)))
+        return E.value, (N[0], N[1]), Va, Vb
+
+    def uks_densities(self, want_grad=True):
+        """rho_s (2, n_points) and grad rho_s (2, n_points, 3) of the last eval_uks (undefined where w = 0)."""
+        n = self.n_points
+        rho = np.empty((2, n))
+        gr = np.empty((2, n, 3)) if want_grad else None
+        _check(_lib.xc_eval_uks_densities(self._h, _dp(rho), _dp(gr)))
+        return rho, gr
 
     def eval_host(self, P, V=None, reuse_weights=False):
         """P, V: host buffers (numpy arrays or pinned torch CPU tensors), float64, row-major."""

@@ -72,6 +72,9 @@ struct xc_plan {
   long long ssf_pairs = -1;    // pair factors evaluated by the last counted build (-1: none)
   int vexp = 0;                // exponent of the fixed-point V accumulator: resolution 2^(vexp - 64), range 2^(vexp + 31)
   double *d_Ptmp = nullptr, *d_Vtmp = nullptr;  // for xc_eval_host
+  // spin-unrestricted build (xc_eval_uks), allocated on first use: rho_s [2][npts], grad rho_s [2][npts][3], the
+  // coefficients of Z^s a_s [2][npts], g_s [2][npts][3], block partials of the functional kernel, (E, N_a, N_b)
+  double *d_urho = nullptr, *d_ugrho = nullptr, *d_ucA = nullptr, *d_ucG = nullptr, *d_upart = nullptr, *d_ures = nullptr;
   bool weights_valid = false;
   std::vector<cudaEvent_t> ev;
   float ms[5] = {0, 0, 0, 0, 0};
@@ -91,7 +94,8 @@ static void free_plan(xc_plan* p) {
   void* ptrs[] = {p->d_px, p->d_py, p->d_pz, p->d_wq, p->d_w, p->d_parent, p->d_atoms, p->d_invR, p->d_rnn, p->d_shells,
                   p->d_exps, p->d_coefs, p->d_batches, p->d_bshells, p->d_bsfoff, p->d_bfidx, p->d_ids_small,
                   p->d_ids_large, p->d_ppk, p->d_vhi, p->d_vlo, p->d_Epart, p->d_Npart, p->d_result,
-                  p->d_rho, p->d_grho, p->d_Ptmp, p->d_Vtmp, p->d_watoms, p->d_wsmall, p->d_wlarge, p->d_wbox, p->d_paircnt};
+                  p->d_rho, p->d_grho, p->d_Ptmp, p->d_Vtmp, p->d_watoms, p->d_wsmall, p->d_wlarge, p->d_wbox, p->d_paircnt,
+                  p->d_urho, p->d_ugrho, p->d_ucA, p->d_ucG, p->d_upart, p->d_ures};
   for (void* q : ptrs) if (q) cudaFree(q);
   if (p->h_result) cudaFreeHost(p->h_result);
   for (cudaEvent_t e : p->ev) cudaEventDestroy(e);
@@ -110,6 +114,38 @@ static void pair_table(const std::vector<double>& atoms, int natoms, std::vector
     }
 }
 
+
+// step (a) of a build (Alg. 4 l.4.1): the partition weights, unless the caller reuses those of the last build
+static int run_weights(xc_plan* p, int32_t flags, cudaStream_t st, int& launches) {
+  HostPlan& hp = p->hp;
+  if (!(flags & XC_EVAL_REUSE_WEIGHTS) || !p->weights_valid) {
+    WeightArgs wa;
+    wa.batches = p->d_batches; wa.watoms = p->d_watoms; wa.atoms = p->d_atoms; wa.invR = p->d_invR;
+    wa.paircnt = nullptr;
+    if ((flags & XC_EVAL_COUNT_PAIRS) && hp.spec.partition == 0) {
+      if (!p->d_paircnt) CU(cudaMalloc((void**)&p->d_paircnt, 8));
+      CU(cudaMemsetAsync(p->d_paircnt, 0, 8, st));
+      wa.paircnt = p->d_paircnt;
+    }
+    wa.wbox = p->d_wbox; wa.natoms = hp.natoms; wa.px = p->d_px; wa.py = p->d_py; wa.pz = p->d_pz; wa.wq = p->d_wq; wa.parent = p->d_parent; wa.w = p->d_w;
+    if (hp.spec.partition == 0) {                          // long lists first: they are the long pole
+      if (!hp.wbatch_large.empty()) { CUK(launch_weights_ssf(wa, p->d_wlarge, (int)hp.wbatch_large.size(), hp.w_max_large, st), st); ++launches; }
+      if (!hp.wbatch_small.empty()) { CUK(launch_weights_ssf(wa, p->d_wsmall, (int)hp.wbatch_small.size(), hp.w_max_small, st), st); ++launches; }
+    } else if (!hp.batches.empty()) {
+      CUK(launch_weights_becke(wa, nullptr, (int)hp.batches.size(), hp.w_warps, hp.w_max_list, st), st);
+      ++launches;
+    }
+    p->weights_valid = true;
+    p->ssf_pairs = -1;
+    if (wa.paircnt) {
+      unsigned long long v = 0;
+      CU(cudaMemcpyAsync(&v, p->d_paircnt, 8, cudaMemcpyDeviceToHost, st));
+      CU(cudaStreamSynchronize(st));
+      p->ssf_pairs = (long long)v;
+    }
+  }
+  return XC_OK;
+}
 
 extern "C" {
 
@@ -236,32 +272,7 @@ int xc_eval(xc_plan* p, const double* dP, int64_t ldp, double* dV, int64_t ldv, 
     CU(cudaMalloc((void**)&p->d_grho, std::max<size_t>(hp.npts * 24, 8)));
   }
   CU(cudaEventRecord(p->ev[ie++], st));
-  if (!(flags & XC_EVAL_REUSE_WEIGHTS) || !p->weights_valid) {
-    WeightArgs wa;
-    wa.batches = p->d_batches; wa.watoms = p->d_watoms; wa.atoms = p->d_atoms; wa.invR = p->d_invR;
-    wa.paircnt = nullptr;
-    if ((flags & XC_EVAL_COUNT_PAIRS) && hp.spec.partition == 0) {
-      if (!p->d_paircnt) CU(cudaMalloc((void**)&p->d_paircnt, 8));
-      CU(cudaMemsetAsync(p->d_paircnt, 0, 8, st));
-      wa.paircnt = p->d_paircnt;
-    }
-    wa.wbox = p->d_wbox; wa.natoms = hp.natoms; wa.px = p->d_px; wa.py = p->d_py; wa.pz = p->d_pz; wa.wq = p->d_wq; wa.parent = p->d_parent; wa.w = p->d_w;
-    if (hp.spec.partition == 0) {                          // long lists first: they are the long pole
-      if (!hp.wbatch_large.empty()) { CUK(launch_weights_ssf(wa, p->d_wlarge, (int)hp.wbatch_large.size(), hp.w_max_large, st), st); ++launches; }
-      if (!hp.wbatch_small.empty()) { CUK(launch_weights_ssf(wa, p->d_wsmall, (int)hp.wbatch_small.size(), hp.w_max_small, st), st); ++launches; }
-    } else if (!hp.batches.empty()) {
-      CUK(launch_weights_becke(wa, nullptr, (int)hp.batches.size(), hp.w_warps, hp.w_max_list, st), st);
-      ++launches;
-    }
-    p->weights_valid = true;
-    p->ssf_pairs = -1;
-    if (wa.paircnt) {
-      unsigned long long v = 0;
-      CU(cudaMemcpyAsync(&v, p->d_paircnt, 8, cudaMemcpyDeviceToHost, st));
-      CU(cudaStreamSynchronize(st));
-      p->ssf_pairs = (long long)v;
-    }
-  }
+  { const int rc = run_weights(p, flags, st, launches); if (rc != XC_OK) return rc; }
   CU(cudaEventRecord(p->ev[ie++], st));
   size_t nb2 = (size_t)hp.nbasis * hp.nbasis;
   BatchArgs ba;
@@ -271,7 +282,7 @@ int xc_eval(xc_plan* p, const double* dP, int64_t ldp, double* dV, int64_t ldv, 
   ba.P = dP; ba.ldp = ldp; ba.ppk = p->d_ppk;
   ba.rho_out = diag ? p->d_rho : nullptr; ba.grho_out = (diag && gga) ? p->d_grho : nullptr;
   ba.Epart = p->d_Epart; ba.Npart = p->d_Npart; ba.vhi = p->d_vhi; ba.vlo = p->d_vlo; ba.nbasis = hp.nbasis;
-  ba.rho_tol = hp.spec.rho_tol;
+  ba.rho_tol = hp.spec.rho_tol; ba.cA = nullptr; ba.cG = nullptr;
   ba.vflags = (unsigned*)(p->d_result + 2);
   if (diag) {
     CU(cudaMemsetAsync(p->d_rho, 0, hp.npts * 8, st));
@@ -290,8 +301,8 @@ int xc_eval(xc_plan* p, const double* dP, int64_t ldp, double* dV, int64_t ldv, 
     CU(cudaMemsetAsync(p->d_vlo, 0, nb2 * 8, st));
     CU(cudaMemsetAsync(p->d_result + 2, 0, 16, st));
     if (attempt == 0) CU(cudaEventRecord(p->ev[ie++], st));
-    if (!hp.ids_large.empty()) { CUK(launch_batch(1, gga, ba, p->d_ids_large, (int)hp.ids_large.size(), hp.smem_large, st), st); ++launches; }
-    if (!hp.ids_small.empty()) { CUK(launch_batch(0, gga, ba, p->d_ids_small, (int)hp.ids_small.size(), hp.smem_small, st), st); ++launches; }
+    if (!hp.ids_large.empty()) { CUK(launch_batch(1, gga, 0, ba, p->d_ids_large, (int)hp.ids_large.size(), hp.smem_large, st), st); ++launches; }
+    if (!hp.ids_small.empty()) { CUK(launch_batch(0, gga, 0, ba, p->d_ids_small, (int)hp.ids_small.size(), hp.smem_small, st), st); ++launches; }
     if (attempt == 0) CU(cudaEventRecord(p->ev[ie++], st));
     CUK(launch_reduce((int64_t)hp.batches.size(), p->d_Epart, p->d_Npart, p->d_result, st), st);
     CUK(launch_finalize(hp.nbasis, p->d_vhi, p->d_vlo, dV, ldv, p->vexp, false, st), st);   // speculative: almost always the last word
@@ -328,6 +339,118 @@ int xc_eval(xc_plan* p, const double* dP, int64_t ldp, double* dV, int64_t ldv, 
   CU(cudaEventElapsedTime(&t, p->ev[3], p->ev[4])); p->ms[3] = t;
   CU(cudaEventElapsedTime(&t, p->ev[0], p->ev[4])); p->ms[4] = t;
   p->launches = launches;
+  return XC_OK;
+}
+
+// Spin-unrestricted build (readings A20-A22): rho_s = sum P^s phi phi for s = a, b, the spin-polarised
+// functional couples them, V^a and V^b come out.  Same plan, same kernels, run as passes: per spin {pack P^s, densities},
+// the functional over the grid, per spin {Z^s, V^s,j, increment, finalise}.
+int xc_eval_uks(xc_plan* p, const double* dPa, const double* dPb, int64_t ldp, double* dVa, double* dVb, int64_t ldv,
+                double* E_xc, double* N_ab, int32_t flags, void* cuda_stream) {
+  if (!p || !dPa || !dPb || !dVa || !dVb || !E_xc || !N_ab) return fail(XC_EINVAL, "null argument");
+  if (p->device < 0) return fail(XC_ECUDA, "host-only plan (device = -1): no CUDA device bound, and there is no CPU fallback");
+  HostPlan& hp = p->hp;
+  if (ldp < hp.nbasis || ldv < hp.nbasis) return fail(XC_EINVAL, "leading dimension smaller than n_basis");
+  if (!(hp.spec.rho_tol > 0.0)) return fail(XC_EINVAL, "the spin-unrestricted build needs rho_tol > 0 (reading A20)");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  DeviceGuard guard(p->device);
+  const bool gga = hp.spec.functional == 1;
+  const int64_t npts = hp.npts;
+  int launches = 0;
+  if (!p->d_urho) {
+    const size_t n = std::max<size_t>((size_t)npts, 1);
+    CU(cudaMalloc((void**)&p->d_urho, 2 * n * 8));
+    CU(cudaMalloc((void**)&p->d_ugrho, 6 * n * 8));
+    CU(cudaMalloc((void**)&p->d_ucA, 2 * n * 8));
+    CU(cudaMalloc((void**)&p->d_ucG, 6 * n * 8));
+    CU(cudaMalloc((void**)&p->d_upart, std::max<size_t>((size_t)uks_functional_blocks(npts), 1) * 3 * 8));
+    CU(cudaMalloc((void**)&p->d_ures, 4 * 8));
+  }
+  CU(cudaEventRecord(p->ev[0], st));
+  { const int rc = run_weights(p, flags, st, launches); if (rc != XC_OK) return rc; }
+  CU(cudaEventRecord(p->ev[1], st));
+  const size_t nb2 = (size_t)hp.nbasis * hp.nbasis;
+  BatchArgs ba;
+  ba.batches = p->d_batches; ba.bshells = p->d_bshells; ba.bsfoff = p->d_bsfoff; ba.bfidx = p->d_bfidx;
+  ba.shells = p->d_shells; ba.exps = p->d_exps; ba.coefs = p->d_coefs;
+  ba.px = p->d_px; ba.py = p->d_py; ba.pz = p->d_pz; ba.w = p->d_w;
+  ba.ldp = ldp; ba.ppk = p->d_ppk;
+  ba.Epart = p->d_Epart; ba.Npart = p->d_Npart; ba.vhi = p->d_vhi; ba.vlo = p->d_vlo; ba.nbasis = hp.nbasis;
+  ba.rho_tol = hp.spec.rho_tol; ba.vexp = p->vexp;
+  ba.vflags = (unsigned*)(p->d_result + 2);
+  ba.cA = nullptr; ba.cG = nullptr;
+  // ---- densities of both spins (Alg. 4 l.4.2-4.5 per spin) ----
+  for (int s = 0; s < 2; ++s) {
+    ba.P = s == 0 ? dPa : dPb;
+    ba.rho_out = p->d_urho + (size_t)s * npts; ba.grho_out = p->d_ugrho + (size_t)s * npts * 3;
+    if (!hp.ids_large.empty()) { CUK(launch_pack(ba, p->d_ids_large, (int)hp.ids_large.size(), !gga, st), st); ++launches; }
+    if (!hp.ids_small.empty()) { CUK(launch_pack(ba, p->d_ids_small, (int)hp.ids_small.size(), !gga, st), st); ++launches; }
+    if (!hp.ids_large.empty()) { CUK(launch_batch(1, gga, 1, ba, p->d_ids_large, (int)hp.ids_large.size(), hp.smem_large, st), st); ++launches; }
+    if (!hp.ids_small.empty()) { CUK(launch_batch(0, gga, 1, ba, p->d_ids_small, (int)hp.ids_small.size(), hp.smem_small, st), st); ++launches; }
+  }
+  CU(cudaEventRecord(p->ev[2], st));
+  // ---- functional, E_xc, N_a, N_b (l.4.6-4.7) ----
+  CUK(launch_functional_uks(gga, npts, p->d_w, p->d_urho, p->d_ugrho, hp.spec.rho_tol, p->d_ucA, p->d_ucG, p->d_upart, p->d_ures, st), st);
+  launches += 2;
+  // ---- Z^s, V^s,j, increment (l.4.8-4.10) per spin; the accumulator's exponent adapts as in xc_eval ----
+  ba.rho_out = nullptr; ba.grho_out = nullptr; ba.P = nullptr;
+  for (int s = 0; s < 2; ++s) {
+    double* dV = s == 0 ? dVa : dVb;
+    ba.cA = p->d_ucA + (size_t)s * npts; ba.cG = p->d_ucG + (size_t)s * npts * 3;
+    for (int attempt = 0;; ++attempt) {
+      ba.vexp = p->vexp;
+      CU(cudaMemsetAsync(p->d_vhi, 0, nb2 * 8, st));
+      CU(cudaMemsetAsync(p->d_vlo, 0, nb2 * 8, st));
+      CU(cudaMemsetAsync(p->d_result + 2, 0, 16, st));
+      if (!hp.ids_large.empty()) { CUK(launch_batch(1, gga, 2, ba, p->d_ids_large, (int)hp.ids_large.size(), hp.smem_large, st), st); ++launches; }
+      if (!hp.ids_small.empty()) { CUK(launch_batch(0, gga, 2, ba, p->d_ids_small, (int)hp.ids_small.size(), hp.smem_small, st), st); ++launches; }
+      CUK(launch_finalize(hp.nbasis, p->d_vhi, p->d_vlo, dV, ldv, p->vexp, false, st), st);
+      ++launches;
+      CU(cudaMemcpyAsync(p->h_result, p->d_result, 32, cudaMemcpyDeviceToHost, st));
+      CU(cudaStreamSynchronize(st));
+      unsigned vf[4];
+      std::memcpy(vf, p->h_result + 2, 16);
+      if (vf[1] != 0) {
+        CUK(launch_finalize(hp.nbasis, p->d_vhi, p->d_vlo, dVa, ldv, p->vexp, true, st), st);
+        CUK(launch_finalize(hp.nbasis, p->d_vhi, p->d_vlo, dVb, ldv, p->vexp, true, st), st);
+        CU(cudaStreamSynchronize(st));
+        *E_xc = N_ab[0] = N_ab[1] = std::nan("");
+        return fail(XC_EINVAL, "non-finite value met while accumulating V (NaN or Inf in P, or overflow); V is filled with NaN");
+      }
+      const int e = vf[0] ? (int)(vf[0] >> 20) - 1023 : p->vexp;
+      const bool fits = p->vexp >= e - 10 && p->vexp <= e + 14;
+      if (fits || attempt == 1) {
+        if (!fits) return fail(XC_EUNSUPPORTED, "V increments span more than the fixed-point accumulator covers");
+        break;
+      }
+      p->vexp = e - 8;
+    }
+  }
+  CU(cudaEventRecord(p->ev[3], st));
+  double res[4];
+  CU(cudaMemcpyAsync(res, p->d_ures, 24, cudaMemcpyDeviceToHost, st));
+  CU(cudaEventRecord(p->ev[4], st));
+  CU(cudaStreamSynchronize(st));
+  *E_xc = res[0]; N_ab[0] = res[1]; N_ab[1] = res[2];
+  float t;
+  CU(cudaEventElapsedTime(&t, p->ev[0], p->ev[1])); p->ms[0] = t;   // weights
+  CU(cudaEventElapsedTime(&t, p->ev[1], p->ev[2])); p->ms[1] = t;   // pack + densities of both spins
+  CU(cudaEventElapsedTime(&t, p->ev[2], p->ev[3])); p->ms[2] = t;   // functional + potentials of both spins
+  p->ms[3] = 0.f;
+  CU(cudaEventElapsedTime(&t, p->ev[0], p->ev[4])); p->ms[4] = t;
+  p->launches = launches;
+  p->diag_valid = false;
+  return XC_OK;
+}
+
+// rho_s [2][npts] and grad rho_s [2][npts][3] of the last xc_eval_uks, plan order (grad only for GGA plans); entries of
+// points with w = 0 are not defined (they are never evaluated)
+int xc_eval_uks_densities(const xc_plan* p, double* rho, double* grho) {
+  if (!p) return fail(XC_EINVAL, "plan is null");
+  if (p->device < 0 || !p->d_urho) return fail(XC_EINVAL, "no spin-unrestricted build has run on this plan");
+  DeviceGuard guard(p->device);
+  if (rho) CU(cudaMemcpy(rho, p->d_urho, (size_t)p->hp.npts * 16, cudaMemcpyDeviceToHost));
+  if (grho) CU(cudaMemcpy(grho, p->d_ugrho, (size_t)p->hp.npts * 48, cudaMemcpyDeviceToHost));
   return XC_OK;
 }
 

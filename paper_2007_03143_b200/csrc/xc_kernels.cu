@@ -364,7 +364,11 @@ struct BatchCfg {
   static constexpr int NG = NT / T;            // thread groups of the per-(shell, point) passes
 };
 
-template <int NT, int T, bool GGA, int NTW, int ROUNDS, int MINB>
+// MODE 0: the fused restricted build (all stages).  The spin-unrestricted build (xc_eval_uks, readings
+// A20-A22) runs the same stages as separate passes, once per spin: MODE 1 = stages 1-2 only, rho_s (and grad rho_s) of the
+// live points written to rho_out / grho_out; then k_functional_uks couples the spins; MODE 2 = stages 1, 4-6 with the
+// per-point coefficients of Z^s read from cA / cG instead of a functional evaluation.
+template <int NT, int T, bool GGA, int NTW, int ROUNDS, int MINB, int MODE>
 __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_t* __restrict__ batch_ids) {
   using Cfg = BatchCfg<NT, T>;
   constexpr int LD = Cfg::LD;
@@ -412,7 +416,7 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
     if (live) sLive[off + __popc(lm & ((1u << lane) - 1u))] = (short)tid;
     __syncthreads();
     if (nqe == 0) {                              // block-uniform
-      if (tid == 0) { a.Epart[bidx] = 0.0; a.Npart[bidx] = 0.0; }
+      if (tid == 0 && MODE == 0) { a.Epart[bidx] = 0.0; a.Npart[bidx] = 0.0; }
       return;
     }
   }
@@ -521,7 +525,7 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
     PH(2);
 
     // ---- 2. X^T = Phi^T P^j and the density reductions ----
-    {
+    if (MODE != 2) {
       double C[2][NTW][2];
 #pragma unroll
       for (int u = 0; u < 2; ++u)
@@ -587,8 +591,8 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
         }
       }
     }
-    __syncthreads();
-    if (GGA) {
+    if (MODE != 2) __syncthreads();
+    if (GGA && MODE != 2) {
       // density pass per (shell, point): thread = (group, point); a group walks over the shells group, group + NG, ...
       const int i = tid % T, grp = tid / T;
       const double xi = sx[i], yi = sy[i], zi = sz[i];
@@ -642,7 +646,14 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
       nx[li] = a.px[gi]; nx[T + li] = a.py[gi]; nx[2 * T + li] = a.pz[gi];
       nx[3 * T + li] = li < nn ? a.w[gi] : 0.0;
     }
-    if (tid < T) {
+    if (tid < T && MODE == 2) {
+      // per-point coefficients of Z^s from the functional kernel: a (LDA: w v_rho_s; GGA: 1/2 w v_rho_s), g (GGA)
+      const int64_t gi = (int64_t)b.pt_off + sLive[t0 + min(tid, npt - 1)];
+      const bool ok = tid < npt;
+      sA[tid] = ok ? a.cA[gi] : 0.0;
+      if (GGA) { sG0[tid] = ok ? a.cG[3 * gi] : 0.0; sG1[tid] = ok ? a.cG[3 * gi + 1] : 0.0; sG2[tid] = ok ? a.cG[3 * gi + 2] : 0.0; }
+    }
+    if (tid < T && MODE != 2) {
       double rho = 0.0, gx = 0.0, gy = 0.0, gz = 0.0;
       for (int q = 0; q < (GGA ? Cfg::NG : Cfg::WM); ++q) {
         rho += sRed[(size_t)(q * 4 + 0) * T + tid];
@@ -654,31 +665,40 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
       }
       if (!GGA) rho *= 2.0;                      // LDA: the X GEMM ran over the lower triangle of P^j (half the diagonal)
       gx *= 2.0; gy *= 2.0; gz *= 2.0;
-      const double sigma = gx * gx + gy * gy + gz * gz;
-      const double wi = sw[tid];
-      double f, vr, vs;
-      xc_point<GGA>(rho, sigma, a.rho_tol, f, vr, vs);
-      sA[tid] = GGA ? 0.5 * wi * vr : wi * vr;   // LDA: V^j = sum_i (w v_rho)_i Phi_mu,i Phi_nu,i
-      const double gs = 2.0 * wi * vs;
-      sG0[tid] = gs * gx; sG1[tid] = gs * gy; sG2[tid] = gs * gz;
-      if (tid < npt && a.rho_out) {
-        const int64_t gi = (int64_t)b.pt_off + sLive[t0 + tid];
-        a.rho_out[gi] = rho;
-        if (a.grho_out) { a.grho_out[3 * gi] = gx; a.grho_out[3 * gi + 1] = gy; a.grho_out[3 * gi + 2] = gz; }
-      }
-      double e = wi * f, n = wi * rho;
+      if (MODE == 1) {
+        if (tid < npt) {
+          const int64_t gi = (int64_t)b.pt_off + sLive[t0 + tid];
+          a.rho_out[gi] = rho;
+          if (GGA) { a.grho_out[3 * gi] = gx; a.grho_out[3 * gi + 1] = gy; a.grho_out[3 * gi + 2] = gz; }
+        }
+      } else {
+        const double sigma = gx * gx + gy * gy + gz * gz;
+        const double wi = sw[tid];
+        double f, vr, vs;
+        xc_point<GGA>(rho, sigma, a.rho_tol, f, vr, vs);
+        sA[tid] = GGA ? 0.5 * wi * vr : wi * vr;   // LDA: V^j = sum_i (w v_rho)_i Phi_mu,i Phi_nu,i
+        const double gs = 2.0 * wi * vs;
+        sG0[tid] = gs * gx; sG1[tid] = gs * gy; sG2[tid] = gs * gz;
+        if (tid < npt && a.rho_out) {
+          const int64_t gi = (int64_t)b.pt_off + sLive[t0 + tid];
+          a.rho_out[gi] = rho;
+          if (a.grho_out) { a.grho_out[3 * gi] = gx; a.grho_out[3 * gi + 1] = gy; a.grho_out[3 * gi + 2] = gz; }
+        }
+        double e = wi * f, n = wi * rho;
 #pragma unroll
-      for (int o = 16; o >= 1; o >>= 1) {
-        e += __shfl_xor_sync(0xffffffffu, e, o);
-        n += __shfl_xor_sync(0xffffffffu, n, o);
+        for (int o = 16; o >= 1; o >>= 1) {
+          e += __shfl_xor_sync(0xffffffffu, e, o);
+          n += __shfl_xor_sync(0xffffffffu, n, o);
+        }
+        if (lane == 0) { sE[warp] = e; sN[warp] = n; }
       }
-      if (lane == 0) { sE[warp] = e; sN[warp] = n; }
     }
     __syncthreads();
     PH(4);
-    if (tid == 0) {
+    if (tid == 0 && MODE == 0) {
       for (int q = 0; q < T / 32; ++q) { Eacc += sE[q]; Nacc += sN[q]; }
     }
+    if (MODE == 1) continue;                     // densities only: next tile (the barrier at the top of the loop orders the buffers)
 
     // ---- 4. GGA: Z (Eq. (20)) per (shell, point); overwrites X^T ----
     if (GGA) {
@@ -752,7 +772,8 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
 
   PH(7);
   // ---- 6. increment of V (Eq. (17)), lower triangle; global indices ascend with local ones ----
-  if (tid == 0) { a.Epart[bidx] = Eacc; a.Npart[bidx] = Nacc; }
+  if (MODE == 1) return;
+  if (tid == 0 && MODE == 0) { a.Epart[bidx] = Eacc; a.Npart[bidx] = Nacc; }
   unsigned vmax = 0;
   bool bad = false;
 #pragma unroll
@@ -846,22 +867,29 @@ cudaError_t launch_pack(const BatchArgs& a, const int32_t* batch_ids, int nbatch
   return cudaGetLastError();
 }
 
-template <int NT, int T, bool GGA, int NTW, int ROUNDS, int MINB>
+template <int NT, int T, bool GGA, int NTW, int ROUNDS, int MINB, int MODE>
 static cudaError_t launch_batch_t(const BatchArgs& a, const int32_t* batch_ids, int nbatches, size_t smem, cudaStream_t st) {
-  cudaError_t e = cudaFuncSetAttribute(k_xc_batch<NT, T, GGA, NTW, ROUNDS, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaError_t e = cudaFuncSetAttribute(k_xc_batch<NT, T, GGA, NTW, ROUNDS, MINB, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  k_xc_batch<NT, T, GGA, NTW, ROUNDS, MINB><<<nbatches, NT, smem, st>>>(a, batch_ids);
+  k_xc_batch<NT, T, GGA, NTW, ROUNDS, MINB, MODE><<<nbatches, NT, smem, st>>>(a, batch_ids);
   return cudaGetLastError();
 }
+template <int MODE>
+static cudaError_t launch_batch_m(int cls, bool gga, const BatchArgs& a, const int32_t* batch_ids, int nbatches, size_t smem, cudaStream_t st) {
+  if (cls == 0) return gga ? launch_batch_t<512, 64, true, 4, 2, 1, MODE>(a, batch_ids, nbatches, smem, st)
+                           : launch_batch_t<512, 64, false, 4, 2, 1, MODE>(a, batch_ids, nbatches, smem, st);
+  return gga ? launch_batch_t<512, 32, true, 3, 5, 1, MODE>(a, batch_ids, nbatches, smem, st)
+             : launch_batch_t<512, 32, false, 3, 5, 1, MODE>(a, batch_ids, nbatches, smem, st);
+}
 
-// cls 0: N_b^j <= kSmallNb, tiles of 64 points; cls 1: N_b^j <= kMaxNb, tiles of 32 points; 16 warps, one CTA per SM
-cudaError_t launch_batch(int cls, bool gga, const BatchArgs& a, const int32_t* batch_ids, int nbatches, size_t smem,
+// cls 0: N_b^j <= kSmallNb, tiles of 64 points; cls 1: N_b^j <= kMaxNb, tiles of 32 points; 16 warps, one CTA per SM.
+// mode 0: fused restricted build; 1: densities of one spin; 2: potential of one spin from given coefficients (xc_eval_uks)
+cudaError_t launch_batch(int cls, bool gga, int mode, const BatchArgs& a, const int32_t* batch_ids, int nbatches, size_t smem,
                          cudaStream_t st) {
   if (nbatches <= 0) return cudaSuccess;
-  if (cls == 0) return gga ? launch_batch_t<512, 64, true, 4, 2, 1>(a, batch_ids, nbatches, smem, st)
-                           : launch_batch_t<512, 64, false, 4, 2, 1>(a, batch_ids, nbatches, smem, st);
-  return gga ? launch_batch_t<512, 32, true, 3, 5, 1>(a, batch_ids, nbatches, smem, st)
-             : launch_batch_t<512, 32, false, 3, 5, 1>(a, batch_ids, nbatches, smem, st);
+  if (mode == 1) return launch_batch_m<1>(cls, gga, a, batch_ids, nbatches, smem, st);
+  if (mode == 2) return launch_batch_m<2>(cls, gga, a, batch_ids, nbatches, smem, st);
+  return launch_batch_m<0>(cls, gga, a, batch_ids, nbatches, smem, st);
 }
 
 cudaError_t launch_finalize(int nbasis, const unsigned long long* vhi, const unsigned long long* vlo, double* V,

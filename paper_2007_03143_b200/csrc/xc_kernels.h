@@ -17,7 +17,8 @@ struct BatchArgs {
   const double* px; const double* py; const double* pz; const double* w;
   const double* P; int64_t ldp;
   double* ppk;                         // packed P^j of every batch (DMMA B-fragment order)
-  double* rho_out; double* grho_out;   // optional diagnostics (may be null)
+  double* rho_out; double* grho_out;   // optional diagnostics (may be null); mode 1: rho_s / grad rho_s of one spin
+  const double* cA; const double* cG;  // mode 2: per-point coefficients of Z^s, a [npts] and g [npts][3]
   double* Epart; double* Npart;        // one partial per batch
   unsigned long long* vhi; unsigned long long* vlo;   // fixed-point V accumulator (lower triangle), value = (hi 2^32 + lo) 2^(vexp - 64)
   int vexp;
@@ -45,8 +46,13 @@ cudaError_t launch_weights_becke(const WeightArgs& a, const int32_t* batch_ids, 
 cudaError_t launch_functional(int kind, int64_t n, const double* rho, const double* sigma, double rho_tol, double* f,
                               double* vr, double* vs, cudaStream_t st);
 cudaError_t launch_pack(const BatchArgs& a, const int32_t* batch_ids, int nbatches, bool tri, cudaStream_t st);
-cudaError_t launch_batch(int cls, bool gga, const BatchArgs& a, const int32_t* batch_ids, int nbatches, size_t smem,
+cudaError_t launch_batch(int cls, bool gga, int mode, const BatchArgs& a, const int32_t* batch_ids, int nbatches, size_t smem,
                          cudaStream_t st);
+// spin-unrestricted build: functional over the grid (xc_uks.cu); rho [2][npts], grho [2][npts][3] in, cA [2][npts], cG [2][npts][3]
+// and out3 = (E_xc, N_a, N_b) out; part: scratch of 3 * uks_functional_blocks(npts) doubles
+int64_t uks_functional_blocks(int64_t npts);
+cudaError_t launch_functional_uks(bool gga, int64_t npts, const double* w, const double* rho, const double* grho, double rho_tol,
+                                  double* cA, double* cG, double* part, double* out3, cudaStream_t st);
 cudaError_t launch_finalize(int nbasis, const unsigned long long* vhi, const unsigned long long* vlo, double* V,
                             int64_t ldv, int vexp, bool poison, cudaStream_t st);
 cudaError_t launch_reduce(int64_t n, const double* ep, const double* np, double* out, cudaStream_t st);

@@ -438,3 +438,56 @@ def test_bad_geometry_is_rejected(xc):
     with pytest.raises(xc.XcError) as e:
         xc.Plan(xyz, w.atoms_Z, w.shell_atom, w.shell_L, w.shell_nprim, w.shell_prim_off, w.exps, w.coefs, xc.grid_spec(10, 26, 0))
     assert e.value.code == -1
+
+
+# ---- spin-unrestricted build, SURVEY 8(f) item 3 (readings A20-A22) -----------------------------
+@pytest.mark.parametrize("name,functional,n_a,n_b", [("c1", 0, 6, 4), ("c1", 1, 6, 4), ("w8", 1, 44, 36), ("p8", 1, 42, 38),
+                                                     ("w27", 0, 140, 130), ("w27", 1, 139, 131)])
+def test_uks_parity(xc, orc, name, functional, n_a, n_b):
+    """xc_eval_uks against the oracle's spin-unrestricted Alg. 4 on the library's exported plan: V_a, V_b, E_xc, N_a, N_b
+    at the north_star tolerances, rho_s / grad rho_s point by point; bit-identical repeat."""
+    import torch
+    from workloads import spin_density_matrices
+    w = make_workload(name)
+    Pa, Pb = spin_density_matrices(w, n_a, n_b)
+    plan = xc.Plan.from_workload(w, spec=xc.grid_spec(w.n_rad, w.n_ang, functional))
+    Pad, Pbd = torch.from_numpy(Pa).cuda(), torch.from_numpy(Pb).cuda()
+    E, (Na, Nb), Va, Vb = plan.eval_uks(Pad, Pbd)
+    ex = plan.export()
+    op = oracle_plan(orc, ex)
+    wts = orc.partition_weights(w.atoms_xyz, op.pts, op.wq, op.parent, 0, True)
+    r = orc.evaluate_uks(op, wts, basis_of(w), w.atoms_xyz, Pa, Pb, functional, want_rho=True)
+    vmax = max(np.max(np.abs(r.Va)), np.max(np.abs(r.Vb)))
+    Vah, Vbh = Va.cpu().numpy(), Vb.cpu().numpy()
+    assert np.max(np.abs(Vah - r.Va)) <= TOL_V * vmax and np.max(np.abs(Vbh - r.Vb)) <= TOL_V * vmax
+    assert np.array_equal(Vah, Vah.T) and np.array_equal(Vbh, Vbh.T)
+    assert np.max(np.abs(Vah - Vbh)) > 1e-3 * vmax                      # genuinely spin-polarised
+    assert abs(E - r.E_xc) <= TOL_S * abs(r.E_xc)
+    assert abs(Na - r.N_a) <= TOL_S * r.N_a and abs(Nb - r.N_b) <= TOL_S * r.N_b
+    gw = plan.diagnostics()["w"]
+    assert np.max(np.abs(gw - wts)) <= 1e-13 * np.max(wts)
+    rho, gr = plan.uks_densities()
+    m = gw != 0.0
+    for s in range(2):
+        assert np.max(np.abs(rho[s][m] - r.rho[s][m])) <= 1e-12 * np.max(np.abs(r.rho))
+        if functional == 1:
+            assert np.max(np.abs(gr[s][m] - r.grad_rho[s][m])) <= 1e-12 * np.max(np.abs(r.grad_rho))
+    E2, N2, Va2, Vb2 = plan.eval_uks(Pad, Pbd, reuse_weights=True)
+    assert E2 == E and N2 == (Na, Nb) and torch.equal(Va, Va2) and torch.equal(Vb, Vb2)
+    plan.close()
+
+
+@pytest.mark.parametrize("functional", [0, 1])
+def test_uks_closed_shell_limit_is_the_restricted_build(xc, functional):
+    """P_a = P_b = P/2 through the pass-wise spin-unrestricted build against the fused restricted kernel (two code paths
+    of the library: closed-form derivatives vs forward-mode tangents, fused vs separate passes)."""
+    import torch
+    w = make_workload("w8")
+    plan = xc.Plan.from_workload(w, spec=xc.grid_spec(w.n_rad, w.n_ang, functional))
+    P = torch.from_numpy(w.P).cuda()
+    E0, N0, V0 = plan.eval(P)
+    E, (Na, Nb), Va, Vb = plan.eval_uks(0.5 * P, 0.5 * P)
+    vmax = float(V0.abs().max())
+    assert abs(E - E0) <= 1e-12 * abs(E0) and abs(Na + Nb - N0) <= 1e-12 * N0 and abs(Na - Nb) <= 1e-14 * N0
+    assert float((Va - V0).abs().max()) <= 1e-12 * vmax and float((Va - Vb).abs().max()) <= 1e-14 * vmax
+    plan.close()
