@@ -132,6 +132,13 @@ int xc_eval_uks(xc_plan* plan, const double* dPa, const double* dPb, int64_t ldp
  * be NULL; entries of points with w = 0 are undefined (never evaluated). */
 int xc_eval_uks_densities(const xc_plan* plan, double* rho, double* grad_rho);
 
+/* The meta-GGA intermediate ("more advanced DFAs (such as the meta-GGA) with the addition of only a few
+ * intermediates"; reading A22): tau_i = 1/2 sum_mu grad Phi_mu,i . grad X_mu,i, X = P^j Phi^j (Eq. (15)), for the
+ * density matrix dP [device] (one spin's, or the total one), with the batches' shell lists as for rho.
+ *   d_tau [device] n_points doubles, plan order (xc_plan_export), OVERWRITTEN; 0 at the points with w = 0 (never
+ *   evaluated).  Runs step (a) first unless XC_EVAL_REUSE_WEIGHTS.  No tau-dependent functional is built on it. */
+int xc_eval_tau(xc_plan* plan, const double* dP, int64_t ldp, double* d_tau, int32_t flags, void* cuda_stream);
+
 /* Diagnostics of the last xc_eval on this plan, for parity tests at full size.  All [host], may be NULL:
  *   w n_points final partition weights (plan order);  rho n_points;  grad_rho 3*n_points (zeros for LDA) -- these two
  *   only if that xc_eval ran with XC_EVAL_DIAG (else XC_EINVAL), and only at points with w != 0;

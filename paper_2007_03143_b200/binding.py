@@ -59,6 +59,7 @@ def _load():
     lib.xc_eval_host.argtypes = [vp, vp, C.c_int64, vp, C.c_int64, dp, dp, C.c_int32]
     lib.xc_eval_uks.argtypes = [vp, vp, vp, C.c_int64, vp, vp, C.c_int64, dp, dp, C.c_int32, vp]
     lib.xc_eval_uks_densities.argtypes = [vp, dp, dp]
+    lib.xc_eval_tau.argtypes = [vp, vp, C.c_int64, vp, C.c_int32, vp]
     lib.xc_eval_diagnostics.argtypes = [vp, dp, dp, dp, dp, dp]
     lib.xc_eval_timings.argtypes = [vp, C.POINTER(C.c_float), ip]
     lib.xc_eval_counters.argtypes = [vp, lp, lp]
@@ -73,7 +74,7 @@ def _load():
     return lib
 
 
-EXPORTED = ["xc_plan_create", "xc_plan_info", "xc_plan_export", "xc_eval", "xc_eval_host", "xc_eval_uks", "xc_eval_uks_densities", "xc_eval_diagnostics",
+EXPORTED = ["xc_plan_create", "xc_plan_info", "xc_plan_export", "xc_eval", "xc_eval_host", "xc_eval_uks", "xc_eval_uks_densities", "xc_eval_tau", "xc_eval_diagnostics",
             "xc_eval_timings", "xc_eval_counters", "xc_plan_stats", "xc_plan_destroy", "xc_integrate", "xc_partition_weights",
             "xc_functional", "xc_measure_fp64_peak", "xc_strerror", "xc_last_error"]
 
@@ -205,6 +206,15 @@ class Plan:
                                 C.c_void_p(Va.data_ptr()), C.c_void_p(Vb.data_ptr()), Va.stride(0), C.byref(E), N,
                                 XC_EVAL_REUSE_WEIGHTS if reuse_weights else 0, _stream_ptr(stream)))
         return E.value, (N[0], N[1]), Va, Vb
+
+    def eval_tau(self, P, reuse_weights=False, stream=None):
+        """tau_i = 1/2 sum grad Phi . grad X for the density matrix P (torch CUDA float64): tensor of n_points, plan order."""
+        import torch
+        assert P.is_cuda and P.dtype == torch.float64 and P.dim() == 2 and P.stride(1) == 1
+        tau = torch.empty(self.n_points, dtype=torch.float64, device=P.device)
+        _check(_lib.xc_eval_tau(self._h, C.c_void_p(P.data_ptr()), P.stride(0), C.c_void_p(tau.data_ptr()),
+                                XC_EVAL_REUSE_WEIGHTS if reuse_weights else 0, _stream_ptr(stream)))
+        return tau
 
     def uks_densities(self, want_grad=True):
         """rho_s (2, n_points) and grad rho_s (2, n_points, 3) of the last eval_uks (undefined where w = 0)."""

@@ -454,6 +454,36 @@ int xc_eval_uks_densities(const xc_plan* p, double* rho, double* grho) {
   return XC_OK;
 }
 
+// The meta-GGA intermediate (reading A22): tau_i = 1/2 sum_mu grad Phi_mu,i . grad X_mu,i with
+// X = P^j Phi^j, for the density matrix dP (one spin, or the total one), at every point with w != 0.
+int xc_eval_tau(xc_plan* p, const double* dP, int64_t ldp, double* d_tau, int32_t flags, void* cuda_stream) {
+  if (!p || !dP || !d_tau) return fail(XC_EINVAL, "null argument");
+  if (p->device < 0) return fail(XC_ECUDA, "host-only plan (device = -1): no CUDA device bound, and there is no CPU fallback");
+  HostPlan& hp = p->hp;
+  if (ldp < hp.nbasis) return fail(XC_EINVAL, "leading dimension smaller than n_basis");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  DeviceGuard guard(p->device);
+  int launches = 0;
+  { const int rc = run_weights(p, flags, st, launches); if (rc != XC_OK) return rc; }
+  BatchArgs ba;
+  ba.batches = p->d_batches; ba.bshells = p->d_bshells; ba.bsfoff = p->d_bsfoff; ba.bfidx = p->d_bfidx;
+  ba.shells = p->d_shells; ba.exps = p->d_exps; ba.coefs = p->d_coefs;
+  ba.px = p->d_px; ba.py = p->d_py; ba.pz = p->d_pz; ba.w = p->d_w;
+  ba.P = dP; ba.ldp = ldp; ba.ppk = p->d_ppk;
+  ba.rho_out = d_tau; ba.grho_out = nullptr; ba.cA = nullptr; ba.cG = nullptr;
+  ba.Epart = p->d_Epart; ba.Npart = p->d_Npart; ba.vhi = p->d_vhi; ba.vlo = p->d_vlo; ba.nbasis = hp.nbasis;
+  ba.rho_tol = hp.spec.rho_tol; ba.vexp = p->vexp; ba.vflags = (unsigned*)(p->d_result + 2);
+  CU(cudaMemsetAsync(d_tau, 0, (size_t)hp.npts * 8, st));
+  if (!hp.ids_large.empty()) { CUK(launch_pack(ba, p->d_ids_large, (int)hp.ids_large.size(), true, st), st); ++launches; }
+  if (!hp.ids_small.empty()) { CUK(launch_pack(ba, p->d_ids_small, (int)hp.ids_small.size(), true, st), st); ++launches; }
+  if (!hp.ids_large.empty()) { CUK(launch_batch(1, false, 3, ba, p->d_ids_large, (int)hp.ids_large.size(), hp.smem_large, st), st); ++launches; }
+  if (!hp.ids_small.empty()) { CUK(launch_batch(0, false, 3, ba, p->d_ids_small, (int)hp.ids_small.size(), hp.smem_small, st), st); ++launches; }
+  CU(cudaStreamSynchronize(st));
+  p->launches = launches;
+  p->diag_valid = false;
+  return XC_OK;
+}
+
 int xc_eval_host(xc_plan* p, const double* hP, int64_t ldp, double* hV, int64_t ldv, double* E_xc, double* N_el, int32_t flags) {
   if (!p || !hP || !hV) return fail(XC_EINVAL, "null argument");
   if (p->device < 0) return fail(XC_ECUDA, "host-only plan (device = -1): no CUDA device bound, and there is no CPU fallback");

@@ -367,7 +367,9 @@ struct BatchCfg {
 // MODE 0: the fused restricted build (all stages).  The spin-unrestricted build (xc_eval_uks, readings
 // A20-A22) runs the same stages as separate passes, once per spin: MODE 1 = stages 1-2 only, rho_s (and grad rho_s) of the
 // live points written to rho_out / grho_out; then k_functional_uks couples the spins; MODE 2 = stages 1, 4-6 with the
-// per-point coefficients of Z^s read from cA / cG instead of a functional evaluation.
+// per-point coefficients of Z^s read from cA / cG instead of a functional evaluation.  MODE 3 (xc_eval_tau): the meta-GGA
+// intermediate tau = 1/2 sum_mu grad Phi_mu . grad X_mu: stages 1-2 once per gradient component with
+// d_c Phi in the Phi buffer, tau = sum_c (d_c Phi)^T L (d_c Phi) from the LDA epilogue, written to rho_out.
 template <int NT, int T, bool GGA, int NTW, int ROUNDS, int MINB, int MODE>
 __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_t* __restrict__ batch_ids) {
   using Cfg = BatchCfg<NT, T>;
@@ -487,6 +489,8 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
     __syncthreads();                           // previous tile's readers of sPhi / sZ are done; tables / points visible
     PH(1);
 
+    double tau_acc = 0.0;                        // MODE 3: tau of this thread's point
+    for (int comp = 0; comp < (MODE == 3 ? 3 : 1); ++comp) {   // MODE 3: one pass per gradient component
     // ---- 1. collocation (Eq. (7); same shell across a warp) ----
     for (int q = warp; q < ns * (T / 32); q += Cfg::NW) {
       const int slot = sOrd[q / (T / 32)], i = (q % (T / 32)) * 32 + lane;
@@ -506,7 +510,27 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
       }
       if (GGA) *reinterpret_cast<double2*>(sR + ((size_t)slot * T + i) * 2) = make_double2(R0, R1);
       double* dst = sPhi + (size_t)sh._pad * LD + i;
-      if (sh.L == 0) {
+      if (MODE == 3) {
+        // d/dr_c of the shell's functions: d_c (m R0) = (d_c m) R0 + m (r - R)_c R1
+        const double dc = comp == 0 ? dx : (comp == 1 ? dy : dz);
+        const double base = dc * R1;
+        const double ex = comp == 0 ? R0 : 0.0, ey = comp == 1 ? R0 : 0.0, ez = comp == 2 ? R0 : 0.0;   // R0 d(r - R)_k / dr_c
+        if (sh.L == 0) {
+          dst[0] = base;
+        } else if (sh.L == 1) {
+          dst[0] = fma(dx, base, ex); dst[LD] = fma(dy, base, ey); dst[2 * LD] = fma(dz, base, ez);
+        } else {
+          const double bx = dx * base, by = dy * base;
+          const double Dxx = fma(dx, bx, 2.0 * dx * ex), Dxy = fma(dy, bx, fma(dy, ex, dx * ey)), Dxz = fma(dz, bx, fma(dz, ex, dx * ez));
+          const double Dyy = fma(dy, by, 2.0 * dy * ey), Dyz = fma(dz, by, fma(dz, ey, dy * ez)), Dzz = fma(dz * dz, base, 2.0 * dz * ez);
+          if (sh.L == 2) {
+            dst[0] = Dxx; dst[LD] = Dxy; dst[2 * LD] = Dxz; dst[3 * LD] = Dyy; dst[4 * LD] = Dyz; dst[5 * LD] = Dzz;
+          } else {
+            dst[0] = kSqrt3 * Dxy; dst[LD] = kSqrt3 * Dyz; dst[2 * LD] = Dzz - 0.5 * (Dxx + Dyy);
+            dst[3 * LD] = kSqrt3 * Dxz; dst[4 * LD] = (0.5 * kSqrt3) * (Dxx - Dyy);
+          }
+        }
+      } else if (sh.L == 0) {
         dst[0] = R0;
       } else if (sh.L == 1) {
         dst[0] = dx * R0; dst[LD] = dy * R0; dst[2 * LD] = dz * R0;
@@ -592,6 +616,10 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
       }
     }
     if (MODE != 2) __syncthreads();
+    if (MODE == 3 && tid < T) {                  // (grad_c Phi)^T L (grad_c Phi) = 1/2 (grad_c Phi)^T P (grad_c Phi): tau's share
+      for (int q = 0; q < Cfg::WM; ++q) tau_acc += sRed[(size_t)(q * 4) * T + tid];
+    }
+    }                                            // component loop (one pass unless MODE 3)
     if (GGA && MODE != 2) {
       // density pass per (shell, point): thread = (group, point); a group walks over the shells group, group + NG, ...
       const int i = tid % T, grp = tid / T;
@@ -665,7 +693,9 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
       }
       if (!GGA) rho *= 2.0;                      // LDA: the X GEMM ran over the lower triangle of P^j (half the diagonal)
       gx *= 2.0; gy *= 2.0; gz *= 2.0;
-      if (MODE == 1) {
+      if (MODE == 3) {                           // tau_s = 1/2 sum_mu grad Phi . grad X^s, to rho_out
+        if (tid < npt) a.rho_out[(int64_t)b.pt_off + sLive[t0 + tid]] = tau_acc;
+      } else if (MODE == 1) {
         if (tid < npt) {
           const int64_t gi = (int64_t)b.pt_off + sLive[t0 + tid];
           a.rho_out[gi] = rho;
@@ -698,7 +728,7 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
     if (tid == 0 && MODE == 0) {
       for (int q = 0; q < T / 32; ++q) { Eacc += sE[q]; Nacc += sN[q]; }
     }
-    if (MODE == 1) continue;                     // densities only: next tile (the barrier at the top of the loop orders the buffers)
+    if (MODE == 1 || MODE == 3) continue;        // densities only: next tile (the barrier at the top of the loop orders the buffers)
 
     // ---- 4. GGA: Z (Eq. (20)) per (shell, point); overwrites X^T ----
     if (GGA) {
@@ -772,7 +802,7 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
 
   PH(7);
   // ---- 6. increment of V (Eq. (17)), lower triangle; global indices ascend with local ones ----
-  if (MODE == 1) return;
+  if (MODE == 1 || MODE == 3) return;
   if (tid == 0 && MODE == 0) { a.Epart[bidx] = Eacc; a.Npart[bidx] = Nacc; }
   unsigned vmax = 0;
   bool bad = false;
@@ -889,6 +919,10 @@ cudaError_t launch_batch(int cls, bool gga, int mode, const BatchArgs& a, const 
   if (nbatches <= 0) return cudaSuccess;
   if (mode == 1) return launch_batch_m<1>(cls, gga, a, batch_ids, nbatches, smem, st);
   if (mode == 2) return launch_batch_m<2>(cls, gga, a, batch_ids, nbatches, smem, st);
+  if (mode == 3) {   // tau: gradient components through the LDA (lower-triangle) X GEMM, whatever the plan's functional
+    return cls == 0 ? launch_batch_t<512, 64, false, 4, 2, 1, 3>(a, batch_ids, nbatches, smem, st)
+                    : launch_batch_t<512, 32, false, 3, 5, 1, 3>(a, batch_ids, nbatches, smem, st);
+  }
   return launch_batch_m<0>(cls, gga, a, batch_ids, nbatches, smem, st);
 }
 

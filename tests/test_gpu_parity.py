@@ -491,3 +491,29 @@ def test_uks_closed_shell_limit_is_the_restricted_build(xc, functional):
     assert abs(E - E0) <= 1e-12 * abs(E0) and abs(Na + Nb - N0) <= 1e-12 * N0 and abs(Na - Nb) <= 1e-14 * N0
     assert float((Va - V0).abs().max()) <= 1e-12 * vmax and float((Va - Vb).abs().max()) <= 1e-14 * vmax
     plan.close()
+
+
+@pytest.mark.parametrize("name,functional", [("c1", 0), ("w8", 1), ("p8", 1), ("w27", 0)])
+def test_tau_parity(xc, orc, name, functional):
+    """xc_eval_tau (meta-GGA intermediate) against the oracle's tau on the library's plan, for the two spin
+    density matrices of an open-shell determinant, point by point where w != 0; zero elsewhere."""
+    import torch
+    from workloads import spin_density_matrices
+    w = make_workload(name)
+    n_occ = w.n_occ
+    Pa, Pb = spin_density_matrices(w, n_occ + 1, n_occ - 1)
+    plan = xc.Plan.from_workload(w, spec=xc.grid_spec(w.n_rad, w.n_ang, functional))
+    ta = plan.eval_tau(torch.from_numpy(Pa).cuda()).cpu().numpy()
+    tb = plan.eval_tau(torch.from_numpy(Pb).cuda(), reuse_weights=True).cpu().numpy()
+    ex = plan.export()
+    op = oracle_plan(orc, ex)
+    wts = orc.partition_weights(w.atoms_xyz, op.pts, op.wq, op.parent, 0, True)
+    r = orc.evaluate_uks(op, wts, basis_of(w), w.atoms_xyz, Pa, Pb, 0, want_V=False, want_rho=True, want_tau=True)
+    gw = plan.diagnostics()["w"]
+    m = gw != 0.0
+    scale = np.max(np.abs(r.tau))
+    assert np.max(np.abs(ta[m] - r.tau[0][m])) <= 1e-12 * scale and np.max(np.abs(tb[m] - r.tau[1][m])) <= 1e-12 * scale
+    assert np.all(ta[~m] == 0.0) and np.all(tb[~m] == 0.0)
+    # the kinetic-energy integrals of the two spin channels (sum w tau), relative 1e-11
+    assert abs(np.sum(gw * ta) - np.sum(wts * r.tau[0])) <= 1e-11 * abs(np.sum(wts * r.tau[0]))
+    plan.close()
