@@ -15,6 +15,9 @@ constexpr int kBatchThreads = 512;  // 16 warps per batch CTA
 constexpr int kSmallNb = 112;   // N_b^j limit of the 64-point-tile instantiation (<= 28 lower-triangle 16x16 blocks = 2 per warp of 16)
 constexpr int kMaxNb = 192;     // N_b^j limit of the batch kernel (<= 78 blocks = 5 per warp); the planner splits larger batches
 constexpr size_t kSmemLimit = 227 * 1024;
+constexpr size_t kBatchStaticSmem = 2048;   // static shared memory of k_xc_batch (live-point list, counters, ring barriers), rounded up
+constexpr int kRingStages = 2;              // P^j staging ring of k_xc_batch: slots ...
+constexpr int kRingGMax = 16;                // ... of at most this many k-steps each (256 B per mu-tile and k-step)
 constexpr int kWeightThreads = 256;  // Becke-88 weights kernel: 8 warps per batch CTA
 constexpr int kWeightSmallList = 256; // SSF weights kernel: atom-list length that separates its two launches
 
@@ -31,7 +34,7 @@ struct BatchRec {      // one quadrature batch B_j with its shell list S_j (PAPE
   int64_t ppk_off;             // offset (doubles) of this batch's packed P^j (nb4 x nb8, DMMA fragment order)
   int64_t wa_off;              // offset into the weight-kernel atom lists
   int32_t wa_nB, wa_nC;        // atoms that can own weight here / atoms that can appear in a cell product
-  int32_t ntriv, _pad;         // SSF: the first ntriv points of the batch have w = w^q exactly (r_A < (1-a)/2 R_nn(A))
+  int32_t ntriv, ring_g;       // ring_g: k-steps per stage of the P^j staging ring this batch can afford (xc_kernels.cu); SSF: the first ntriv points of the batch have w = w^q exactly (r_A < (1-a)/2 R_nn(A))
 };
 
 
@@ -42,7 +45,8 @@ inline int nfun(int type) { return type == kPureD ? 5 : (type + 1) * (type + 2) 
 inline int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
 
 // shared-memory footprint of the batch kernel for a batch (bytes); T = points per tile
-size_t batch_smem_bytes(int T, bool gga, int nb, int ns, int npr, int nthreads);   // npr: primitives of the batch's shells
+size_t batch_smem_bytes(int T, bool gga, int nb, int ns, int npr, int nthreads, int ring_g);   // npr: primitives of the batch's shells
+int batch_ring_g(size_t bytes_without_ring, int nb);   // k-steps per ring stage that fit beside it (0: none)
 size_t weights_smem_bytes(int nC, int warps);
 // atom list of the weights kernels for the box [lo, hi] of points: owners = out[0 .. nB), partners = all of out (sorted by distance to the box)
 void weight_atom_list(const double* atoms, int natoms, const double lo[3], const double hi[3], bool ssf, std::vector<int32_t>& out, int& nB);

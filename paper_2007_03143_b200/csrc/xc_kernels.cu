@@ -272,45 +272,104 @@ __device__ __forceinline__ void fixed_add(unsigned long long* hi, unsigned long 
 //                 symmetric product (half the flops); the scaling by a_i is applied to the A fragment.
 //   per batch  6  increment of V (Eq. (17)): one fixed-point add per lower-triangle element.
 // ------------------------------------------------------------------------------------------------
-// X^T tile of one warp: C[u][v] += A_u(16 points x 4 nu) * B_v(4 nu x 8 mu) over all k-steps; NV mu-tiles (compile
-// time), B fragments (packed P^j, global/L1) loaded one k-step ahead into registers and kPfDist k-steps ahead
-// into L1 (the fragments of a batch are re-read for every tile, from L2 once they have left L1).
-constexpr int kPfDist = 4;
-template <int NV, int NTW, int BS>
-__device__ __forceinline__ void xgemm_tile(double (&C)[2][NTW][2], const double* __restrict__ Ap, const double* __restrict__ Bp,
-                                           int nks, int astep, int bstep) {
-  double Bn[NV];
+// ------------------------------------------------------------------------------------------------
+// P^j staging (north_star (d): "P_sub gathered through TMA or shared-memory staging"; PAPER.md:L379-L385 names the P^j
+// pack as the paper's own bottleneck).  The packed P^j of the batch is streamed through a ring of kRingStages
+// shared-memory slots of G k-steps each (G = BatchRec::ring_g: what the batch's tiles leave of the SM's shared memory) by the bulk asynchronous copy engine (cp.async.bulk, one elected thread),
+// each slot guarded by a full / empty mbarrier pair: every fragment crosses L2 -> SM once per tile pass for the whole
+// CTA (it used to be fetched by each of the four warps that share a mu-tile, through an L1 that the 200+ KB
+// shared-memory carve-out leaves almost empty), the copies run kRingStages - 1 slots ahead of the DMMAs across tile
+// boundaries, and the GEMM warps issue no global loads at all.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  unsigned done = 0;
+  for (unsigned spin = 0; !done; ++spin) {
+    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    if (spin > (1u << 28)) __trap();           // a copy or an arrival was lost: fail loudly instead of hanging the device
+  }
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+struct PRing {
+  const double* ppk;            // packed P^j of the batch (global)
+  double* buf;                  // [kRingStages][G * ntile * 32]
+  unsigned long long* full;     // [kRingStages]
+  unsigned long long* empty;    // [kRingStages]
+  int ntile, nks, G, spp;       // mu-tiles, k-steps, k-steps per stage, stages per pass over P^j (= ceil(nks / G))
+  unsigned total;               // stages the whole batch consumes
+  unsigned n;                   // next stage this thread consumes (same value in every thread of the CTA)
+};
+// the elected thread: start the copy of stage number q (P^j k-steps [kb G, ...) of pass q / spp) into its slot
+__device__ __forceinline__ void ring_issue(const PRing& r, unsigned q) {
+  const int slot = q % kRingStages, kb = (q % r.spp) * r.G;
+  const unsigned bytes = (unsigned)(min(r.G, r.nks - kb) * r.ntile) * 256u;
+  mbar_expect_tx(r.full + slot, bytes);
+  bulk_g2s(r.buf + (size_t)slot * (r.G * r.ntile * 32), r.ppk + (size_t)kb * r.ntile * 32, bytes, r.full + slot);
+}
+
+// X^T tile of one warp over one pass of P^j: C[u][v] += A_u(16 points x 4 nu) * B_v(4 nu x 8 mu) over all k-steps; NV
+// mu-tiles (compile time: mt0, mt0 + wmstep, ...), A fragments from sPhi, B fragments from the ring.  TRI (LDA): only the
+// lower triangle of P^j is packed non-zero, so mu-tile mt skips the k-steps ks >= 2 mt + 2 (warp-uniform branch: a
+// predicated-off DMMA would still take its slot in the FP64 tensor pipe).  Every warp of the CTA walks every stage
+// (warps without tiles included): the slot is handed back when all NW warps have arrived.
+template <int NV, int NTW, bool TRI>
+__device__ __forceinline__ void xgemm_ring(double (&C)[2][NTW][2], const double* __restrict__ Ap, int astep, PRing& r, int mt0,
+                                           int wmstep, int lane, bool elected) {
+  int lim[4];
 #pragma unroll
-  for (int v = 0; v < NV; ++v) Bn[v] = __ldg(Bp + v * BS);
-#pragma unroll
-  for (int d = 1; d < kPfDist; ++d)
-    if (d < nks) {
-#pragma unroll
-      for (int v = 0; v < NV; ++v) asm volatile("prefetch.global.L1 [%0];" ::"l"(Bp + (size_t)d * bstep + v * BS));
+  for (int v = 0; v < 4; ++v) lim[v] = (TRI && v < NV) ? min(r.nks, 2 * (mt0 + v * wmstep) + 2) : r.nks;
+  for (int kb = 0; kb < r.nks; kb += r.G) {
+    const unsigned q = r.n;
+    const int slot = q % kRingStages;
+    if (elected) {
+      // keep the ring kRingStages - 1 stages ahead: the slot of stage q - 1 is refilled once every warp has left it
+      const unsigned nxt = q + kRingStages - 1;
+      if (nxt < r.total) {
+        if (q >= 1) mbar_wait(r.empty + (q - 1) % kRingStages, ((q - 1) / kRingStages) & 1);
+        ring_issue(r, nxt);
+      }
     }
-  for (int ks = 0; ks < nks; ++ks) {
-    const double A0 = Ap[0], A1 = Ap[8];
-    double Bc[NV];
+    mbar_wait(r.full + slot, (q / kRingStages) & 1);
+    const double* Bs = r.buf + (size_t)slot * (r.G * r.ntile * 32) + (size_t)mt0 * 32 + lane;
+    const int gend = min(r.G, r.nks - kb);
+    for (int g = 0; g < gend; ++g) {
+      const int ks = kb + g;
+      {
+        const double A0 = Ap[0], A1 = Ap[8];
+        Ap += astep;
 #pragma unroll
-    for (int v = 0; v < NV; ++v) Bc[v] = Bn[v];
-    Ap += astep;
-    Bp += bstep;
-    if (ks + kPfDist < nks) {
-#pragma unroll
-      for (int v = 0; v < NV; ++v) asm volatile("prefetch.global.L1 [%0];" ::"l"(Bp + (size_t)(kPfDist - 1) * bstep + v * BS));
+        for (int v = 0; v < NV; ++v) {
+          if (!TRI || ks < lim[v]) {
+            const double Bv = Bs[(size_t)(g * r.ntile + v * wmstep) * 32];
+            dmma884(C[0][v][0], C[0][v][1], A0, Bv);
+            dmma884(C[1][v][0], C[1][v][1], A1, Bv);
+          }
+        }
+      }
     }
-    if (ks + 1 < nks) {
-#pragma unroll
-      for (int v = 0; v < NV; ++v) Bn[v] = __ldg(Bp + v * BS);
-    }
-#pragma unroll
-    for (int v = 0; v < NV; ++v) {
-      dmma884(C[0][v][0], C[0][v][1], A0, Bc[v]);
-      dmma884(C[1][v][0], C[1][v][1], A1, Bc[v]);
-    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(r.empty + slot);
+    r.n = q + 1;
   }
 }
 
+// LDA (and the tau passes): the packed lower triangle is read straight from global memory, one k-step ahead in registers
+// and kPfDist k-steps ahead in L1 -- each mu-tile stops at its diagonal, so a ring that every warp has to walk in step would
+// make the warps with short k-ranges wait (measured: 7 % slower on c2 than this path).
+constexpr int kPfDist = 4;
 // LDA: X' = L Phi (k_pack_P, tri).  mu-tile mt only has non-zero fragments for the k-steps ks < 2 mt + 2, so the tiles of
 // a warp (mt0, mt0 + WM, ...) drop in one after the other: k-steps [lim_{v-1}, lim_v) run the tiles v .. NV-1, each range
 // with its own fully unrolled loop (no predicated-off DMMA).
@@ -390,6 +449,7 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
   double* sR = (double*)sp; if (GGA) sp += (size_t)ns * T * 16;
   double* sPt = (double*)sp; sp += (size_t)16 * T * 8;  // points x, y, z, w of two tiles (double buffer) + 8 T scratch
   double* sRed = (double*)sp; sp += (size_t)NT * 4 * 8; // partial rho / grad rho: [groups][4][T]
+  double* sRing = (double*)sp; sp += (size_t)kRingStages * b.ring_g * ntile * 32 * 8;   // P^j staging ring (16-byte aligned)
   double* sExpT = (double*)sp; sp += (size_t)64 * 8;    // 2^(j/64)
   ShellRec* sSh = (ShellRec*)sp; sp += (size_t)ns * sizeof(ShellRec);
   int* sIdx = (int*)sp; sp += (size_t)nb16 * 4;
@@ -477,7 +537,19 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
 #pragma unroll
       for (int v = 0; v < 2; ++v) V[r][u][v][0] = V[r][u][v][1] = 0.0;
   }
-  const double* __restrict__ ppk = a.ppk + b.ppk_off;
+  // ---- P^j staging ring: barriers, and the first kRingStages - 1 stages on their way before the first tile ----
+  __shared__ __align__(8) unsigned long long sBar[2 * kRingStages];
+  PRing ring;
+  ring.ppk = a.ppk + b.ppk_off; ring.buf = sRing; ring.full = sBar; ring.empty = sBar + kRingStages;
+  ring.ntile = ntile; ring.nks = nks; ring.G = max(1, b.ring_g); ring.spp = (nks + ring.G - 1) / ring.G;
+  ring.total = (MODE == 2 || !GGA) ? 0u : (unsigned)(((nqe + T - 1) / T) * ring.spp);   // GGA X GEMM only
+  ring.n = 0;
+  if (MODE != 2 && GGA && tid == 0) {
+    for (int k = 0; k < kRingStages; ++k) { mbar_init(ring.full + k, 1); mbar_init(ring.empty + k, Cfg::NW); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    for (unsigned q = 0; q < (unsigned)(kRingStages - 1) && q < ring.total; ++q) ring_issue(ring, q);
+  }
   const int wp = warp % Cfg::WP, wm = warp / Cfg::WP;
   double Eacc = 0.0, Nacc = 0.0;
   PH_DECL
@@ -556,19 +628,19 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
 #pragma unroll
         for (int v = 0; v < NTW; ++v) C[u][v][0] = C[u][v][1] = 0.0;
       const double* Ap = sPhi + (size_t)t4 * LD + wp * 16 + g4;
-      const double* Bp = ppk + (size_t)wm * 32 + lane;
-      // number of mu-tiles of this warp (warp-uniform): one fully unrolled loop per count, so that no DMMA is
-      // ever issued predicated-off (a predicated-off DMMA still takes its slot in the FP64 tensor pipe)
+      // number of mu-tiles of this warp (warp-uniform): one fully unrolled loop per count
       const int nv = wm < ntile ? min(NTW, (ntile - wm + Cfg::WM - 1) / Cfg::WM) : 0;
       if (GGA) {
+        const bool elected = tid == 0;
         switch (nv) {
-          case 1: xgemm_tile<1, NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
-          case 2: xgemm_tile<(NTW >= 2 ? 2 : 1), NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
-          case 3: xgemm_tile<(NTW >= 3 ? 3 : 1), NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
-          case 4: xgemm_tile<(NTW >= 4 ? 4 : 1), NTW, Cfg::WM * 32>(C, Ap, Bp, nks, 4 * LD, ntile * 32); break;
-          default: break;
+          case 1: xgemm_ring<1, NTW, false>(C, Ap, 4 * LD, ring, wm, Cfg::WM, lane, elected); break;
+          case 2: xgemm_ring<(NTW >= 2 ? 2 : 1), NTW, false>(C, Ap, 4 * LD, ring, wm, Cfg::WM, lane, elected); break;
+          case 3: xgemm_ring<(NTW >= 3 ? 3 : 1), NTW, false>(C, Ap, 4 * LD, ring, wm, Cfg::WM, lane, elected); break;
+          case 4: xgemm_ring<(NTW >= 4 ? 4 : 1), NTW, false>(C, Ap, 4 * LD, ring, wm, Cfg::WM, lane, elected); break;
+          default: xgemm_ring<0, NTW, false>(C, Ap, 4 * LD, ring, 0, Cfg::WM, lane, elected); break;   // no tile: walk the stages
         }
       } else {                                 // LDA: lower triangle only, rho = 2 Phi . (L Phi)
+        const double* Bp = ring.ppk + (size_t)wm * 32 + lane;
         switch (nv) {
           case 1: xgemm_tri<1, NTW, Cfg::WM * 32>(C, Ap, Bp, nks, wm, Cfg::WM, 4 * LD, ntile * 32); break;
           case 2: xgemm_tri<(NTW >= 2 ? 2 : 1), NTW, Cfg::WM * 32>(C, Ap, Bp, nks, wm, Cfg::WM, 4 * LD, ntile * 32); break;
@@ -778,10 +850,15 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
         for (int kk = 0; kk < T / 4; ++kk) {
           const double Pm0 = sPhi[om + 4 * kk], Pm1 = sPhi[om + 8 * LD + 4 * kk], Zm0 = sZ[om + 4 * kk], Zm1 = sZ[om + 8 * LD + 4 * kk];
           const double Pn0 = sPhi[on + 4 * kk], Pn1 = sPhi[on + 8 * LD + 4 * kk], Zn0 = sZ[on + 4 * kk], Zn1 = sZ[on + 8 * LD + 4 * kk];
-          dmma884(V[r][0][0][0], V[r][0][0][1], Zm0, Pn0); dmma884(V[r][0][0][0], V[r][0][0][1], Pm0, Zn0);
-          dmma884(V[r][1][0][0], V[r][1][0][1], Zm1, Pn0); dmma884(V[r][1][0][0], V[r][1][0][1], Pm1, Zn0);
-          dmma884(V[r][1][1][0], V[r][1][1][1], Zm1, Pn1); dmma884(V[r][1][1][0], V[r][1][1][1], Pm1, Zn1);
-          if (!diag) { dmma884(V[r][0][1][0], V[r][0][1][1], Zm0, Pn1); dmma884(V[r][0][1][0], V[r][0][1][1], Pm0, Zn1); }
+          // the two DMMAs of one accumulator are kept apart (a dependent DMMA waits for the result of the one before)
+          dmma884(V[r][0][0][0], V[r][0][0][1], Zm0, Pn0);
+          dmma884(V[r][1][0][0], V[r][1][0][1], Zm1, Pn0);
+          dmma884(V[r][1][1][0], V[r][1][1][1], Zm1, Pn1);
+          if (!diag) dmma884(V[r][0][1][0], V[r][0][1][1], Zm0, Pn1);
+          dmma884(V[r][0][0][0], V[r][0][0][1], Pm0, Zn0);
+          dmma884(V[r][1][0][0], V[r][1][0][1], Pm1, Zn0);
+          dmma884(V[r][1][1][0], V[r][1][1][1], Pm1, Zn1);
+          if (!diag) dmma884(V[r][0][1][0], V[r][0][1][1], Pm0, Zn1);
         }
       } else {
 #pragma unroll 4

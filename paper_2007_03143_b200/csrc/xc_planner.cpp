@@ -93,7 +93,7 @@ struct Leaf { int64_t begin, end; };
 
 }  // namespace
 
-size_t batch_smem_bytes(int T, bool gga, int nb, int ns, int npr, int nthreads) {
+size_t batch_smem_bytes(int T, bool gga, int nb, int ns, int npr, int nthreads, int ring_g) {
   // must mirror the shared-memory carve of k_xc_batch (xc_kernels.cu)
   size_t nb16 = round_up(nb, 16);
   size_t b = 0;
@@ -102,12 +102,22 @@ size_t batch_smem_bytes(int T, bool gga, int nb, int ns, int npr, int nthreads) 
   if (gga) b += (size_t)ns * T * 2 * 8;          // R0/R1 panel
   b += (size_t)T * 8 * 16;                       // x,y,z,w of two tiles, scratch, a,g0,g1,g2
   b += (size_t)nthreads * 4 * 8;                 // cross-warp reduction buffer
+  b += (size_t)kRingStages * ring_g * 256 * (round_up(nb, 8) / 8);   // P^j staging ring: kRingStages x ring_g k-steps x ntile fragments of 256 B
   b += 64 * 8;                                   // 2^(j/64) table of the collocation exp
   b += (size_t)npr * 16;                         // (exponent, coefficient) of the batch's primitives
   b += (size_t)ns * sizeof(ShellRec);            // shell records
   b += nb16 * 4;                                 // global function index
   b += (size_t)((ns + 3) & ~3) * 4;              // collocation order
   return b + 64;
+}
+
+// every batch CTA is launched with all of the SM's shared memory; what its tiles leave free goes to the ring
+int batch_ring_g(size_t bytes_without_ring, int nb) {
+  const size_t lim = kSmemLimit - kBatchStaticSmem;
+  if (nb <= 0) return kRingGMax;
+  if (bytes_without_ring >= lim) return 0;
+  const size_t per_g = (size_t)kRingStages * 256 * (round_up(nb, 8) / 8);
+  return (int)std::min<size_t>(kRingGMax, (lim - bytes_without_ring) / per_g);
 }
 
 size_t weights_smem_bytes(int nC, int warps) { return (size_t)nC * (24 + 4) + (size_t)warps * nC * 8 + 64; }
@@ -322,7 +332,7 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     std::vector<Leaf> L2; std::vector<std::vector<int32_t>> S2; std::vector<int> N2;
     bool any = false;
     for (size_t j = 0; j < leaves.size(); ++j)
-      if (nbs[j] > kMaxNb || batch_smem_bytes(32, gga, nbs[j], (int)lists[j].size(), prim_sum(lists[j]), kBatchThreads) > kSmemLimit) { any = true; break; }
+      if (nbs[j] > kMaxNb || batch_ring_g(batch_smem_bytes(32, gga, nbs[j], (int)lists[j].size(), prim_sum(lists[j]), kBatchThreads, 0), nbs[j]) < 1) { any = true; break; }
     if (any) {
       for (size_t j = 0; j < leaves.size(); ++j) {
         std::vector<Leaf> st{leaves[j]};
@@ -332,7 +342,7 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
           std::vector<int32_t> sl; int nb;
           if (first) { sl = lists[j]; nb = nbs[j]; first = false; } else screen(cur, sl, nb);
           int64_t n = cur.end - cur.begin;
-          if (nb <= kMaxNb && batch_smem_bytes(32, gga, nb, (int)sl.size(), prim_sum(sl), kBatchThreads) <= kSmemLimit) { L2.push_back(cur); S2.push_back(sl); N2.push_back(nb); continue; }
+          if (nb <= kMaxNb && batch_ring_g(batch_smem_bytes(32, gga, nb, (int)sl.size(), prim_sum(sl), kBatchThreads, 0), nb) >= 1) { L2.push_back(cur); S2.push_back(sl); N2.push_back(nb); continue; }
           if (n <= 1) { err = "a single grid point sees more basis functions than the batch kernel supports"; return XC_EUNSUPPORTED; }
           double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
           for (int64_t k = cur.begin; k < cur.end; ++k)
@@ -441,7 +451,7 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     b.wa_off = (int64_t)hp.watoms.size(); b.wa_nB = wnB[j]; b.wa_nC = (int32_t)wlists[j].size();
     hp.watoms.insert(hp.watoms.end(), wlists[j].begin(), wlists[j].end());
     hp.w_max_list = std::max(hp.w_max_list, (int)b.wa_nC);
-    b.ntriv = ntriv[j]; b._pad = 0;
+    b.ntriv = ntriv[j]; b.ring_g = 0;
     if (spec->partition == 0 && b.ntriv < b.nq) {          // SSF: batches whose points are all trivial need no kernel
       const int len = b.wa_nC;
       if (len <= kWeightSmallList) { hp.wbatch_small.push_back((int32_t)j); hp.w_max_small = std::max(hp.w_max_small, len); }
@@ -473,12 +483,19 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     int npr = 0;
     for (int k = 0; k < b.ns; ++k) npr += hp.shells[hp.bshells[b.sh_off + k]].nprim;
     // class 0: 64-point tiles, 16 warps, one CTA per SM; class 1 (N_b^j > kSmallNb or a 64-point tile does not fit): 32-point tiles
-    size_t s64 = batch_smem_bytes(64, gga, b.nb, b.ns, npr, kBatchThreads);
-    if (b.nb <= kSmallNb && s64 <= kSmemLimit - 1024) {
-      hp.smem_small = std::max(hp.smem_small, s64);
+    // the ring serves the GGA X GEMM only (LDA reads its lower-triangle fragments through L1, which needs the shared
+    // memory it does not use)
+    const size_t f64 = batch_smem_bytes(64, gga, b.nb, b.ns, npr, kBatchThreads, 0);
+    const int g64 = batch_ring_g(f64, b.nb);
+    BatchRec& bw = hp.batches[j];
+    if (b.nb <= kSmallNb && g64 >= 2) {
+      bw.ring_g = gga ? g64 : 0;
+      hp.smem_small = std::max(hp.smem_small, batch_smem_bytes(64, gga, b.nb, b.ns, npr, kBatchThreads, bw.ring_g));
       hp.ids_small.push_back((int32_t)j);
     } else {
-      hp.smem_large = std::max(hp.smem_large, batch_smem_bytes(32, gga, b.nb, b.ns, npr, kBatchThreads));
+      const size_t f32 = batch_smem_bytes(32, gga, b.nb, b.ns, npr, kBatchThreads, 0);
+      bw.ring_g = gga ? batch_ring_g(f32, b.nb) : 0;
+      hp.smem_large = std::max(hp.smem_large, batch_smem_bytes(32, gga, b.nb, b.ns, npr, kBatchThreads, bw.ring_g));
       hp.ids_large.push_back((int32_t)j);
     }
   }
