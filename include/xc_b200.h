@@ -110,7 +110,8 @@ int xc_plan_export(const xc_plan* plan, double* pts, double* wq, int32_t* parent
 int xc_eval(xc_plan* plan, const double* dP, int64_t ldp, double* dV, int64_t ldv,
             double* E_xc, double* N_el, int32_t flags, void* cuda_stream);
 
-/* Same build with HOST buffers: copies P to the device, runs xc_eval, copies V back.  hP, hV [host]. */
+/* Same build with HOST buffers: copies P to the device (on a stream of its own, overlapping step (a), which reads no P),
+ * runs xc_eval on the default stream, copies V back.  hP, hV [host] (pinned memory makes the copies asynchronous). */
 int xc_eval_host(xc_plan* plan, const double* hP, int64_t ldp, double* hV, int64_t ldv,
                  double* E_xc, double* N_el, int32_t flags);
 

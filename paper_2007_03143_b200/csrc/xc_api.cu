@@ -72,6 +72,9 @@ struct xc_plan {
   long long ssf_pairs = -1;    // pair factors evaluated by the last counted build (-1: none)
   int vexp = 0;                // exponent of the fixed-point V accumulator: resolution 2^(vexp - 64), range 2^(vexp + 31)
   double *d_Ptmp = nullptr, *d_Vtmp = nullptr;  // for xc_eval_host
+  cudaStream_t copy_stream = nullptr;           // xc_eval_host: P crosses PCIe while step (a), which does not read P, runs
+  cudaEvent_t ev_P = nullptr;                   // ... recorded behind that copy
+  bool wait_P = false;                          // the next xc_eval waits for ev_P before its first read of P
   // spin-unrestricted build (xc_eval_uks), allocated on first use: rho_s [2][npts], grad rho_s [2][npts][3], the
   // coefficients of Z^s a_s [2][npts], g_s [2][npts][3], block partials of the functional kernel, (E, N_a, N_b)
   double *d_urho = nullptr, *d_ugrho = nullptr, *d_ucA = nullptr, *d_ucG = nullptr, *d_upart = nullptr, *d_ures = nullptr;
@@ -99,6 +102,8 @@ static void free_plan(xc_plan* p) {
   for (void* q : ptrs) if (q) cudaFree(q);
   if (p->h_result) cudaFreeHost(p->h_result);
   for (cudaEvent_t e : p->ev) cudaEventDestroy(e);
+  if (p->ev_P) cudaEventDestroy(p->ev_P);
+  if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
   delete p;
 }
 
@@ -273,6 +278,7 @@ int xc_eval(xc_plan* p, const double* dP, int64_t ldp, double* dV, int64_t ldv, 
   }
   CU(cudaEventRecord(p->ev[ie++], st));
   { const int rc = run_weights(p, flags, st, launches); if (rc != XC_OK) return rc; }
+  if (p->wait_P) { p->wait_P = false; CU(cudaStreamWaitEvent(st, p->ev_P, 0)); }   // xc_eval_host: P is on its way on the copy stream
   CU(cudaEventRecord(p->ev[ie++], st));
   size_t nb2 = (size_t)hp.nbasis * hp.nbasis;
   BatchArgs ba;
@@ -493,8 +499,17 @@ int xc_eval_host(xc_plan* p, const double* hP, int64_t ldp, double* hV, int64_t 
   size_t bytes = (size_t)n * n * 8;
   if (!p->d_Ptmp) CU(cudaMalloc((void**)&p->d_Ptmp, bytes));
   if (!p->d_Vtmp) CU(cudaMalloc((void**)&p->d_Vtmp, bytes));
-  CU(cudaMemcpy2DAsync(p->d_Ptmp, (size_t)n * 8, hP, (size_t)ldp * 8, (size_t)n * 8, n, cudaMemcpyHostToDevice, 0));
+  if (!p->copy_stream) {
+    CU(cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
+    CU(cudaEventCreateWithFlags(&p->ev_P, cudaEventDisableTiming));
+  }
+  // the upload of P overlaps step (a) (Alg. 4 l.4.1 reads no P): xc_eval waits for it right before the P^j pack
+  CU(cudaMemcpy2DAsync(p->d_Ptmp, (size_t)n * 8, hP, (size_t)ldp * 8, (size_t)n * 8, n, cudaMemcpyHostToDevice, p->copy_stream));
+  CU(cudaEventRecord(p->ev_P, p->copy_stream));
+  p->wait_P = true;
   int rc = xc_eval(p, p->d_Ptmp, n, p->d_Vtmp, n, E_xc, N_el, flags, nullptr);
+  p->wait_P = false;
+  if (rc != XC_OK) CU(cudaStreamSynchronize(p->copy_stream));   // hP must not be in flight when the caller gets it back
   if (rc != XC_OK) return rc;
   CU(cudaMemcpy2D(hV, (size_t)ldv * 8, p->d_Vtmp, (size_t)n * 8, (size_t)n * 8, n, cudaMemcpyDeviceToHost));
   return XC_OK;
