@@ -35,7 +35,7 @@ DESCR = {
     "c4": "c4: 256-water cluster, 768 atoms, 6400 basis functions, 75x302 grid",
     "c5": "c5: 512-water cluster, 1536 atoms, 12800 basis functions, 100x302 grid",
     "u2": "u2: 64-water cluster on a UFG-shaped 99x590 grid (SURVEY 8(f))",
-    "s2": "s2: 64-water cluster on an SFG-shaped 175x974 grid (SURVEY 8(f))",
+    "s2": "s2: 64-water cluster, 192 atoms, 1600 basis functions, on an SFG-shaped 175x974 grid (SURVEY 8(f))",
     "g1": "g1: irregular 410-water cluster, 1230 atoms, 10250 basis functions, 75x302 grid (SURVEY 8(f))",
 }
 
@@ -277,7 +277,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="c5")
-    ap.add_argument("--also", default="c4,c3,c2,c1,u2,g1", help="comma list of extra workloads reported under other_workloads (or 'none')")
+    ap.add_argument("--also", default="c4,c3,c2,c1,u2,s2,g1", help="comma list of extra workloads reported under other_workloads (or 'none')")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-becke", action="store_true", help="skip the Becke-1988 side measurement (on c2)")
@@ -384,6 +384,31 @@ def main():
             del Pd, Vd
         except Exception as exc:
             line["becke88"] = {"error": repr(exc)[:200]}
+    # the spin-unrestricted build (xc_eval_uks: passes of the same kernels) and the meta-GGA
+    # intermediate tau (xc_eval_tau), timed on the 64-water PBE workload with P_a = P_b = P/2 (same shapes as c3)
+    if world == 1 and not args.no_becke:
+        try:
+            wu = make_workload("c3")
+            uplan = xc.Plan.from_workload(wu, spec=xc.grid_spec(wu.n_rad, wu.n_ang, wu.functional), device=local_rank)
+            Ph = torch.from_numpy(0.5 * wu.P).cuda()
+            Va, Vb = torch.empty_like(Ph), torch.empty_like(Ph)
+            uplan.eval_uks(Ph, Ph, Va, Vb)
+            tu = []
+            for _ in range(3):
+                uplan.eval_uks(Ph, Ph, Va, Vb)
+                tu.append(uplan.timings()["total_ms"])
+            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            uplan.eval_tau(Ph, reuse_weights=True)
+            ev0.record()
+            uplan.eval_tau(Ph, reuse_weights=True)
+            ev1.record()
+            torch.cuda.synchronize()
+            line["uks"] = {"workload": "c3 (P_a = P_b = P/2)", "ms_per_step": statistics.median(tu),
+                           "points_per_s": uplan.n_points / (statistics.median(tu) * 1e-3), "tau_ms_cached_weights": ev0.elapsed_time(ev1)}
+            uplan.close()
+            del Ph, Va, Vb
+        except Exception as exc:
+            line["uks"] = {"error": repr(exc)[:200]}
     if not args.no_cpu_baseline:
         cb = oracle_sample(w, args.workload)
         line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample", "seconds")}
