@@ -5,7 +5,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libxc_b200.so")
-SOURCES = ["xc_api.cu", "xc_kernels.cu", "xc_weights.cu", "xc_uks.cu", "xc_peak.cu", "xc_planner.cpp"]
+SOURCES = ["xc_api.cu", "xc_kernels.cu", "xc_weights.cu", "xc_uks.cu", "xc_gpu_planner.cu", "xc_peak.cu", "xc_planner.cpp"]
 HEADERS = ["xc_internal.h", "xc_kernels.h", os.path.join("..", "..", "include", "xc_b200.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-fopenmp,-O2", "-shared", "-lgomp"]

@@ -183,7 +183,7 @@ int xc_plan_create(const xc_atom* atoms, int32_t natoms, const xc_shell* shells,
   int rc;
   std::vector<double> ptab;   // 1 / R_BC (Becke-88 only: the SSF kernel forms its pair terms per tile)
   try {
-    rc = build_host_plan(atoms, natoms, shells, nshells, exps, coefs, nprim_total, spec, p->hp, err);
+    rc = build_host_plan(atoms, natoms, shells, nshells, exps, coefs, nprim_total, spec, device, p->hp, err);
     if (rc == XC_OK && device != -1 && p->hp.spec.partition == 1) pair_table(p->hp.atoms, p->hp.natoms, ptab);
   } catch (const std::bad_alloc&) {
     rc = XC_ENOMEM; err = "host allocation failed in planner";

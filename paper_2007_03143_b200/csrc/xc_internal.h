@@ -3,6 +3,7 @@
 #pragma once
 #include <cstdint>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "../../include/xc_b200.h"
@@ -79,7 +80,20 @@ struct HostPlan {
 };
 
 // Builds grid, batches, screening, work lists.  Returns XC_OK or an error code (message in err).
+// device >= 0: the grid and the bisection run on that GPU (xc_gpu_planner.cu; the plan is identical either way)
 int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, int nshells, const double* exps,
-                    const double* coefs, int nprim_total, const xc_grid_spec* spec, HostPlan& hp, std::string& err);
+                    const double* coefs, int nprim_total, const xc_grid_spec* spec, int device, HostPlan& hp, std::string& err);
+// step (b) on the GPU (xc_gpu_planner.cu): begin = grid points + global median bisection, returns the cuboids and their tight
+// bounding boxes (lo xyz, hi xyz per cuboid); order = Morton order inside the cuboids, SSF-trivial points first, permuted point
+// arrays; download = hand the points and the order so far to the host (it finishes alone when a batch has to be split again)
+struct GpuPlanner;
+int gpu_planner_begin(int device, int natoms, const double* atoms, int n_rad, int n_ang, const double* rr, const double* au, int maxp,
+                      GpuPlanner** out, std::vector<std::pair<int64_t, int64_t>>& leaves, std::vector<double>& boxes, std::string& err);
+int gpu_planner_download(GpuPlanner* g, std::vector<double>& cx, std::vector<double>& cy, std::vector<double>& cz, std::vector<int64_t>& idx,
+                         std::string& err);
+int gpu_planner_order(GpuPlanner* g, bool ssf, const double* rnn, double lim, const double* rw, int n_rad, const double* aw,
+                      std::vector<double>& px, std::vector<double>& py, std::vector<double>& pz, std::vector<double>& wq,
+                      std::vector<int32_t>& parent, std::vector<int64_t>& orig, std::vector<int32_t>& ntriv, std::string& err);
+void gpu_planner_end(GpuPlanner* g);
 
 }  // namespace xcb

@@ -155,7 +155,7 @@ void weight_atom_list(const double* atoms, int natoms, const double lo[3], const
 }
 
 int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, int nshells, const double* exps,
-                    const double* coefs, int nprim_total, const xc_grid_spec* spec, HostPlan& hp, std::string& err) {
+                    const double* coefs, int nprim_total, const xc_grid_spec* spec, int device, HostPlan& hp, std::string& err) {
   if (!atoms || !shells || !exps || !coefs || !spec) { err = "null argument"; return XC_EINVAL; }
   if (natoms < 1 || nshells < 1 || nprim_total < 1) { err = "empty system"; return XC_EINVAL; }
   if (spec->n_rad < 1 || spec->n_ang < 1 || spec->max_batch_pts < 1 || spec->max_batch_pts > 512) {
@@ -224,7 +224,21 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
   const int64_t npts = per_atom * natoms;
   if (npts >= (int64_t)1 << 31) { err = "more than 2^31 grid points"; return XC_EUNSUPPORTED; }
   hp.npts = npts;
-  std::vector<double> cx(npts), cy(npts), cz(npts);
+  std::vector<double> cx, cy, cz;
+  std::vector<int64_t> idx;
+  std::vector<Leaf> leaves;
+  const int maxp = spec->max_batch_pts;
+  GpuPlanner* gp = nullptr;                    // non-null while the plan is being made on the GPU
+  struct GpGuard { GpuPlanner*& g; ~GpGuard() { if (g) gpu_planner_end(g); } } gp_guard{gp};
+  std::vector<double> gboxes;                  // GPU path: tight bounding boxes of the cuboids
+  if (device >= 0) {
+    // grid and bisection on the GPU (xc_gpu_planner.cu): same points, same cuboids, same order
+    std::vector<std::pair<int64_t, int64_t>> lv;
+    const int rc = gpu_planner_begin(device, natoms, hp.atoms.data(), spec->n_rad, spec->n_ang, rr.data(), au.data(), maxp, &gp, lv, gboxes, err);
+    if (rc != XC_OK) return rc;
+    for (const auto& l : lv) leaves.push_back({l.first, l.second});
+  } else {
+  cx.resize(npts); cy.resize(npts); cz.resize(npts);
 #pragma omp parallel for schedule(static)
   for (int64_t p = 0; p < npts; ++p) {
     int a = (int)(p / per_atom);
@@ -236,11 +250,9 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
   }
 
   // ---- recursive median bisection ----
-  std::vector<int64_t> idx(npts);
+  idx.resize(npts);
   std::iota(idx.begin(), idx.end(), (int64_t)0);
-  const int maxp = spec->max_batch_pts;
   const double* coord[3] = {cx.data(), cy.data(), cz.data()};
-  std::vector<Leaf> leaves;
   {
     // one bisection step: splits `cur` at the median of its longest axis (left part first => depth-first output order
     // is spatially coherent); returns false if the range is a leaf
@@ -298,6 +310,8 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     for (int64_t k = 0; k < (int64_t)front.size(); ++k) subtree(front[k], parts[k]);
     for (auto& v : parts) leaves.insert(leaves.end(), v.begin(), v.end());
   }
+  }   // host grid + bisection
+  const double* coord[3] = {cx.data(), cy.data(), cz.data()};   // (GPU path: null until a download)
 
   // ---- per-batch shell screening (Alg. 1 on the tight bounding box), with re-splitting of batches whose
   //      shell list exceeds the batch kernel's capacity (N_b^j <= kMaxNb, shared memory) ----
@@ -308,12 +322,15 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     atom_rmax[hp.shells[s].atom] = std::max(atom_rmax[hp.shells[s].atom], hp.rcut[s]);
   }
   const bool gga = spec->functional == 1;
-  auto screen = [&](const Leaf& lf, std::vector<int32_t>& out, int& nb, Box* box_out = nullptr) {
+  auto screen = [&](const Leaf& lf, std::vector<int32_t>& out, int& nb, const double* known_box = nullptr) {
     Box b;
-    for (int p = 0; p < 3; ++p) { b.lo[p] = 1e300; b.hi[p] = -1e300; }
-    for (int64_t k = lf.begin; k < lf.end; ++k)
-      for (int p = 0; p < 3; ++p) { double v = coord[p][idx[k]]; b.lo[p] = std::min(b.lo[p], v); b.hi[p] = std::max(b.hi[p], v); }
-    if (box_out) *box_out = b;
+    if (known_box) {
+      for (int p = 0; p < 3; ++p) { b.lo[p] = known_box[p]; b.hi[p] = known_box[3 + p]; }
+    } else {
+      for (int p = 0; p < 3; ++p) { b.lo[p] = 1e300; b.hi[p] = -1e300; }
+      for (int64_t k = lf.begin; k < lf.end; ++k)
+        for (int p = 0; p < 3; ++p) { double v = coord[p][idx[k]]; b.lo[p] = std::min(b.lo[p], v); b.hi[p] = std::max(b.hi[p], v); }
+    }
     out.clear(); nb = 0;
     for (int a = 0; a < natoms; ++a) {
       if (!sphere_hits_box(&hp.atoms[3 * a], atom_rmax[a], b)) continue;
@@ -325,7 +342,7 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
   std::vector<std::vector<int32_t>> lists(leaves.size());
   std::vector<int> nbs(leaves.size());
 #pragma omp parallel for schedule(dynamic, 64)
-  for (int64_t j = 0; j < (int64_t)leaves.size(); ++j) screen(leaves[j], lists[j], nbs[j]);
+  for (int64_t j = 0; j < (int64_t)leaves.size(); ++j) screen(leaves[j], lists[j], nbs[j], gp ? &gboxes[6 * j] : nullptr);
   auto prim_sum = [&](const std::vector<int32_t>& sl) { int n = 0; for (int32_t sh : sl) n += hp.shells[sh].nprim; return n; };
   // re-split oversized batches (rare): sequential fix-up pass
   {
@@ -334,6 +351,12 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     for (size_t j = 0; j < leaves.size(); ++j)
       if (nbs[j] > kMaxNb || batch_ring_g(batch_smem_bytes(32, gga, nbs[j], (int)lists[j].size(), prim_sum(lists[j]), kBatchThreads, 0), nbs[j]) < 1) { any = true; break; }
     if (any) {
+      if (gp) {   // the host finishes this plan: it needs the points and the order so far
+        const int rc = gpu_planner_download(gp, cx, cy, cz, idx, err);
+        gpu_planner_end(gp); gp = nullptr;
+        if (rc != XC_OK) return rc;
+        coord[0] = cx.data(); coord[1] = cy.data(); coord[2] = cz.data();
+      }
       for (size_t j = 0; j < leaves.size(); ++j) {
         std::vector<Leaf> st{leaves[j]};
         bool first = true;
@@ -363,7 +386,7 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
 
   // ---- order the points inside each batch along a Morton curve: neighbouring threads of the weights kernel then
   //      see nearly the same atoms (warp-coherent loop bounds); the batch as a set is unchanged ----
-  {
+  if (!gp) {
     auto spread = [](uint32_t v) { uint64_t x = v & 0x1fffff; x = (x | x << 32) & 0x1f00000000ffffULL; x = (x | x << 16) & 0x1f0000ff0000ffULL;
                                    x = (x | x << 8) & 0x100f00f00f00f00fULL; x = (x | x << 4) & 0x10c30c30c30c30c3ULL; x = (x | x << 2) & 0x1249249249249249ULL; return x; };
 #pragma omp parallel
@@ -393,8 +416,8 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
   // ---- SSF: points with r_A < (1-a)/2 R_nn(A) have w = w^q exactly (every mu_AC <= -a).  They come first in their
   //      batch (each group keeps its Morton order); the weights kernel only visits the others ----
   std::vector<int32_t> ntriv(leaves.size(), 0);
-  if (spec->partition == 0) {
-    const double lim = 0.5 * (1.0 - 0.64);
+  const double lim = 0.5 * (1.0 - 0.64);
+  if (spec->partition == 0 && !gp) {
 #pragma omp parallel for schedule(dynamic, 64)
     for (int64_t j = 0; j < (int64_t)leaves.size(); ++j) {
       auto trivial = [&](int64_t p) {
@@ -418,13 +441,24 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
 #pragma omp parallel for schedule(dynamic, 64)
   for (int64_t j = 0; j < (int64_t)leaves.size(); ++j) {
     double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
-    for (int64_t k = leaves[j].begin; k < leaves[j].end; ++k)
-      for (int p = 0; p < 3; ++p) { double v = coord[p][idx[k]]; lo[p] = std::min(lo[p], v); hi[p] = std::max(hi[p], v); }
+    if (gp) {
+      for (int p = 0; p < 3; ++p) { lo[p] = gboxes[6 * j + p]; hi[p] = gboxes[6 * j + 3 + p]; }
+    } else {
+      for (int64_t k = leaves[j].begin; k < leaves[j].end; ++k)
+        for (int p = 0; p < 3; ++p) { double v = coord[p][idx[k]]; lo[p] = std::min(lo[p], v); hi[p] = std::max(hi[p], v); }
+    }
     for (int p = 0; p < 3; ++p) { hp.wbox[6 * j + p] = lo[p]; hp.wbox[6 * j + 3 + p] = hi[p]; }
     weight_atom_list(hp.atoms.data(), natoms, lo, hi, spec->partition == 0, wlists[j], wnB[j]);
   }
 
   // ---- permuted point arrays ----
+  if (gp) {
+    // GPU path: Morton order, trivial points first and the permuted arrays in one go (identical to the host's stages above)
+    const int rc = gpu_planner_order(gp, spec->partition == 0, hp.rnn.data(), lim, rw.data(), spec->n_rad, aw.data(), hp.px, hp.py, hp.pz, hp.wq,
+                                     hp.parent, hp.orig, ntriv, err);
+    gpu_planner_end(gp); gp = nullptr;
+    if (rc != XC_OK) return rc;
+  } else {
   hp.px.resize(npts); hp.py.resize(npts); hp.pz.resize(npts); hp.wq.resize(npts); hp.parent.resize(npts); hp.orig.resize(npts);
 #pragma omp parallel for schedule(static)
   for (int64_t k = 0; k < npts; ++k) {
@@ -434,6 +468,7 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     int64_t q = p % per_atom;
     hp.wq[k] = rw[q / spec->n_ang] * aw[q % spec->n_ang];
     hp.parent[k] = a; hp.orig[k] = p;
+  }
   }
 
   // ---- batch records, function lists, work items ----

@@ -517,3 +517,22 @@ def test_tau_parity(xc, orc, name, functional):
     # the kinetic-energy integrals of the two spin channels (sum w tau), relative 1e-11
     assert abs(np.sum(gw * ta) - np.sum(wts * r.tau[0])) <= 1e-11 * abs(np.sum(wts * r.tau[0]))
     plan.close()
+
+
+# ---- planner on the GPU, SURVEY 8(f) item 1 ----------------------------------------------------
+@pytest.mark.parametrize("name,kw", [("c1", {}), ("c1", dict(max_batch_pts=37)), ("c1", dict(max_batch_pts=1, n_ang=6, n_rad=10)),
+                                     ("w8", dict(max_batch_pts=100, angular=1, n_ang=288)), ("w27", {}), ("c2", {}), ("g1", {})])
+def test_gpu_planner_equals_host_planner(xc, name, kw):
+    """The grid and the global median bisection run on the GPU when a plan is created for a device (xc_gpu_planner.cu); the
+    host-only plan (device = -1) runs them on the host.  Every exported array must be identical: points, base weights,
+    parents, permutation, batch offsets, shell lists."""
+    w = make_workload(name, with_P=False)
+    kw = dict(kw)
+    spec = xc.grid_spec(kw.pop("n_rad", w.n_rad), kw.pop("n_ang", w.n_ang), w.functional, **kw)
+    pd = xc.Plan.from_workload(w, spec=spec, device=0)
+    ph = xc.Plan.from_workload(w, spec=spec, device=-1)
+    a, b = pd.export(), ph.export()
+    for f in ("pts", "wq", "parent", "orig", "batch_off", "shell_off", "shells"):
+        assert np.array_equal(getattr(a, f), getattr(b, f)), f
+    assert pd.stats() == ph.stats()
+    pd.close(); ph.close()
