@@ -54,6 +54,7 @@ struct xc_plan {
   // device copies
   double *d_px = nullptr, *d_py = nullptr, *d_pz = nullptr, *d_wq = nullptr, *d_w = nullptr;
   int32_t* d_parent = nullptr;
+  int64_t* d_orig = nullptr;            // GPU-made plans only (xc_plan_export reads it back)
   double *d_atoms = nullptr, *d_invR = nullptr, *d_rnn = nullptr;
   ShellRec* d_shells = nullptr;
   double *d_exps = nullptr, *d_coefs = nullptr;
@@ -98,7 +99,7 @@ static void free_plan(xc_plan* p) {
                   p->d_exps, p->d_coefs, p->d_batches, p->d_bshells, p->d_bsfoff, p->d_bfidx, p->d_ids_small,
                   p->d_ids_large, p->d_ppk, p->d_vhi, p->d_vlo, p->d_Epart, p->d_Npart, p->d_result,
                   p->d_rho, p->d_grho, p->d_Ptmp, p->d_Vtmp, p->d_watoms, p->d_wsmall, p->d_wlarge, p->d_wbox, p->d_paircnt,
-                  p->d_urho, p->d_ugrho, p->d_ucA, p->d_ucG, p->d_upart, p->d_ures};
+                  p->d_urho, p->d_ugrho, p->d_ucA, p->d_ucG, p->d_upart, p->d_ures, p->d_orig};
   for (void* q : ptrs) if (q) cudaFree(q);
   if (p->h_result) cudaFreeHost(p->h_result);
   for (cudaEvent_t e : p->ev) cudaEventDestroy(e);
@@ -188,13 +189,18 @@ int xc_plan_create(const xc_atom* atoms, int32_t natoms, const xc_shell* shells,
   } catch (const std::bad_alloc&) {
     rc = XC_ENOMEM; err = "host allocation failed in planner";
   }
+  // a GPU-made plan hands over its point arrays (adopted even on failure, so that free_plan releases them)
+  p->d_px = p->hp.dev.px; p->d_py = p->hp.dev.py; p->d_pz = p->hp.dev.pz; p->d_wq = p->hp.dev.wq;
+  p->d_parent = p->hp.dev.parent; p->d_orig = p->hp.dev.orig;
+  const bool dev_points = p->hp.dev.px != nullptr;
+  p->hp.dev = DevicePoints();
   if (rc != XC_OK) { free_plan(p); return fail(rc, err); }
   HostPlan& hp = p->hp;
   if (device == -1) { *out = p; return XC_OK; }   // host-only plan: info / stats / export only
   auto bail = [&](int code) { free_plan(p); return code; };
   DeviceGuard guard(device);
 #define UP(d, h) do { int _r = upload(&p->d, h); if (_r != XC_OK) return bail(_r); } while (0)
-  UP(d_px, hp.px); UP(d_py, hp.py); UP(d_pz, hp.pz); UP(d_wq, hp.wq); UP(d_parent, hp.parent);
+  if (!dev_points) { UP(d_px, hp.px); UP(d_py, hp.py); UP(d_pz, hp.pz); UP(d_wq, hp.wq); UP(d_parent, hp.parent); }
   UP(d_atoms, hp.atoms);
   UP(d_invR, ptab);
   UP(d_shells, hp.shells); UP(d_exps, hp.exps); UP(d_coefs, hp.coefs);
@@ -249,10 +255,28 @@ int xc_plan_export(const xc_plan* p, double* pts, double* wq, int32_t* parent, i
                    int64_t* shell_off, int32_t* shells) {
   if (!p) return fail(XC_EINVAL, "plan is null");
   const HostPlan& hp = p->hp;
-  if (pts) for (int64_t i = 0; i < hp.npts; ++i) { pts[3 * i] = hp.px[i]; pts[3 * i + 1] = hp.py[i]; pts[3 * i + 2] = hp.pz[i]; }
-  if (wq) std::copy(hp.wq.begin(), hp.wq.end(), wq);
-  if (parent) std::copy(hp.parent.begin(), hp.parent.end(), parent);
-  if (orig) std::copy(hp.orig.begin(), hp.orig.end(), orig);
+  if (hp.px.empty() && hp.npts > 0) {
+    // GPU-made plan: the point arrays live on the device
+    if (p->device < 0 || !p->d_px) return fail(XC_EINVAL, "plan holds no point arrays");
+    DeviceGuard guard(p->device);
+    const size_t n = (size_t)hp.npts;
+    if (pts) {
+      std::vector<double> t(n);
+      const double* src[3] = {p->d_px, p->d_py, p->d_pz};
+      for (int c = 0; c < 3; ++c) {
+        CU(cudaMemcpy(t.data(), src[c], n * 8, cudaMemcpyDeviceToHost));
+        for (size_t i = 0; i < n; ++i) pts[3 * i + c] = t[i];
+      }
+    }
+    if (wq) CU(cudaMemcpy(wq, p->d_wq, n * 8, cudaMemcpyDeviceToHost));
+    if (parent) CU(cudaMemcpy(parent, p->d_parent, n * 4, cudaMemcpyDeviceToHost));
+    if (orig) CU(cudaMemcpy(orig, p->d_orig, n * 8, cudaMemcpyDeviceToHost));
+  } else {
+    if (pts) for (int64_t i = 0; i < hp.npts; ++i) { pts[3 * i] = hp.px[i]; pts[3 * i + 1] = hp.py[i]; pts[3 * i + 2] = hp.pz[i]; }
+    if (wq) std::copy(hp.wq.begin(), hp.wq.end(), wq);
+    if (parent) std::copy(hp.parent.begin(), hp.parent.end(), parent);
+    if (orig) std::copy(hp.orig.begin(), hp.orig.end(), orig);
+  }
   size_t nb = hp.batches.size();
   if (batch_off) { for (size_t j = 0; j < nb; ++j) batch_off[j] = hp.batches[j].pt_off; batch_off[nb] = hp.npts; }
   if (shell_off) { for (size_t j = 0; j < nb; ++j) shell_off[j] = hp.batches[j].sh_off; shell_off[nb] = (int64_t)hp.bshells.size(); }

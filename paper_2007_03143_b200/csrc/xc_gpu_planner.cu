@@ -362,10 +362,10 @@ struct GpuPlanner {
     return cudaSuccess;
   }
 
-  // Morton order inside every batch, SSF-trivial points first (stable), permuted arrays to the host
-  cudaError_t order(bool ssf, const double* rnn, double lim, const double* rw, int n_rad, const double* aw, std::vector<double>& px,
-                    std::vector<double>& py, std::vector<double>& pz, std::vector<double>& wq, std::vector<int32_t>& parent,
-                    std::vector<int64_t>& orig, std::vector<int32_t>& ntriv) {
+  // Morton order inside every batch, SSF-trivial points first (stable); the permuted arrays stay on the device (the plan adopts
+  // them: nothing per point crosses PCIe)
+  cudaError_t order(bool ssf, const double* rnn, double lim, const double* rw, int n_rad, const double* aw, DevicePoints& out,
+                    std::vector<int32_t>& ntriv) {
     const int TPB = 256;
     const unsigned nblk = (unsigned)((n + TPB - 1) / TPB);
     int idx_bits = 1;
@@ -384,20 +384,18 @@ struct GpuPlanner {
     while ((1 << (key_bits - 1)) < nseg) ++key_bits;
     GP_CU(cub::DeviceRadixSort::SortPairs(d_tmp.p, tmp_bytes, d_seg2.p, d_seg.p, d_idx.p, d_idx2.p, (int)n, 0, key_bits));
     std::swap(d_idx.p, d_idx2.p);
-    // gather: reuse the sort buffers as outputs (px, py, pz, wq in key / val buffers; parent, orig in seg / key2)
-    double *o_px = (double*)d_key.p, *o_py = (double*)d_key2.p, *o_pz = (double*)d_val.p, *o_wq = (double*)d_val2.p;
-    DevBuf<long long> d_orig;
-    GP_CU(d_orig.alloc(n));
-    k_gather<<<nblk, TPB>>>(n, d_idx.p, per_atom, n_ang, d_rw.p, d_aw.p, d_cx.p, d_cy.p, d_cz.p, o_px, o_py, o_pz, o_wq, d_seg.p, d_orig.p);
+    // the sort buffers are no longer needed: release them before the plan's arrays are allocated
+    for (void** q : {(void**)&d_key.p, (void**)&d_key2.p, (void**)&d_val.p, (void**)&d_val2.p, (void**)&d_seg.p, (void**)&d_seg2.p,
+                     (void**)&d_idx2.p, (void**)&d_tmp.p}) { cudaFree(*q); *q = nullptr; }
+    const size_t m = std::max<size_t>((size_t)n, 1);
+    GP_CU(cudaMalloc((void**)&out.px, m * 8)); GP_CU(cudaMalloc((void**)&out.py, m * 8)); GP_CU(cudaMalloc((void**)&out.pz, m * 8));
+    GP_CU(cudaMalloc((void**)&out.wq, m * 8)); GP_CU(cudaMalloc((void**)&out.parent, m * 4)); GP_CU(cudaMalloc((void**)&out.orig, m * 8));
+    k_gather<<<nblk, TPB>>>(n, d_idx.p, per_atom, n_ang, d_rw.p, d_aw.p, d_cx.p, d_cy.p, d_cz.p, out.px, out.py, out.pz, out.wq, out.parent,
+                            (long long*)out.orig);
     GP_CU(cudaGetLastError());
-    px.resize(n); py.resize(n); pz.resize(n); wq.resize(n); parent.resize(n); orig.resize(n); ntriv.resize(nseg);
-    GP_CU(cudaMemcpy(px.data(), o_px, (size_t)n * 8, cudaMemcpyDeviceToHost));
-    GP_CU(cudaMemcpy(py.data(), o_py, (size_t)n * 8, cudaMemcpyDeviceToHost));
-    GP_CU(cudaMemcpy(pz.data(), o_pz, (size_t)n * 8, cudaMemcpyDeviceToHost));
-    GP_CU(cudaMemcpy(wq.data(), o_wq, (size_t)n * 8, cudaMemcpyDeviceToHost));
-    GP_CU(cudaMemcpy(parent.data(), d_seg.p, (size_t)n * 4, cudaMemcpyDeviceToHost));
-    GP_CU(cudaMemcpy(orig.data(), d_orig.p, (size_t)n * 8, cudaMemcpyDeviceToHost));
+    ntriv.resize(nseg);
     GP_CU(cudaMemcpy(ntriv.data(), d_ntriv.p, (size_t)nseg * 4, cudaMemcpyDeviceToHost));
+    GP_CU(cudaDeviceSynchronize());
     return cudaSuccess;
   }
 };
@@ -421,9 +419,8 @@ int gpu_planner_download(GpuPlanner* g, std::vector<double>& cx, std::vector<dou
   return e == cudaSuccess ? XC_OK : gp_fail(e, err);
 }
 int gpu_planner_order(GpuPlanner* g, bool ssf, const double* rnn, double lim, const double* rw, int n_rad, const double* aw,
-                      std::vector<double>& px, std::vector<double>& py, std::vector<double>& pz, std::vector<double>& wq,
-                      std::vector<int32_t>& parent, std::vector<int64_t>& orig, std::vector<int32_t>& ntriv, std::string& err) {
-  const cudaError_t e = g->order(ssf, rnn, lim, rw, n_rad, aw, px, py, pz, wq, parent, orig, ntriv);
+                      DevicePoints& out, std::vector<int32_t>& ntriv, std::string& err) {
+  const cudaError_t e = g->order(ssf, rnn, lim, rw, n_rad, aw, out, ntriv);
   return e == cudaSuccess ? XC_OK : gp_fail(e, err);
 }
 void gpu_planner_end(GpuPlanner* g) { delete g; }

@@ -52,6 +52,13 @@ size_t weights_smem_bytes(int nC, int warps);
 // atom list of the weights kernels for the box [lo, hi] of points: owners = out[0 .. nB), partners = all of out (sorted by distance to the box)
 void weight_atom_list(const double* atoms, int natoms, const double lo[3], const double hi[3], bool ssf, std::vector<int32_t>& out, int& nB);
 
+// permuted point arrays made on the device by the GPU planner (plan order); owned by whoever holds the struct
+struct DevicePoints {
+  double *px = nullptr, *py = nullptr, *pz = nullptr, *wq = nullptr;
+  int32_t* parent = nullptr;
+  int64_t* orig = nullptr;
+};
+
 struct HostPlan {
   int natoms = 0, nshells = 0, nbasis = 0, nprim = 0;
   xc_grid_spec spec{};
@@ -59,7 +66,8 @@ struct HostPlan {
   std::vector<double> atoms;           // natoms*3
   std::vector<ShellRec> shells;
   std::vector<double> exps, coefs, rcut;
-  std::vector<double> px, py, pz, wq;  // plan order
+  DevicePoints dev;                    // GPU-made plans: the point arrays live here, and px..orig below stay empty
+  std::vector<double> px, py, pz, wq;  // plan order (host-made plans)
   std::vector<int32_t> parent;
   std::vector<int64_t> orig;
   std::vector<BatchRec> batches;
@@ -92,8 +100,7 @@ int gpu_planner_begin(int device, int natoms, const double* atoms, int n_rad, in
 int gpu_planner_download(GpuPlanner* g, std::vector<double>& cx, std::vector<double>& cy, std::vector<double>& cz, std::vector<int64_t>& idx,
                          std::string& err);
 int gpu_planner_order(GpuPlanner* g, bool ssf, const double* rnn, double lim, const double* rw, int n_rad, const double* aw,
-                      std::vector<double>& px, std::vector<double>& py, std::vector<double>& pz, std::vector<double>& wq,
-                      std::vector<int32_t>& parent, std::vector<int64_t>& orig, std::vector<int32_t>& ntriv, std::string& err);
+                      DevicePoints& out, std::vector<int32_t>& ntriv, std::string& err);
 void gpu_planner_end(GpuPlanner* g);
 
 }  // namespace xcb

@@ -454,8 +454,7 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
   // ---- permuted point arrays ----
   if (gp) {
     // GPU path: Morton order, trivial points first and the permuted arrays in one go (identical to the host's stages above)
-    const int rc = gpu_planner_order(gp, spec->partition == 0, hp.rnn.data(), lim, rw.data(), spec->n_rad, aw.data(), hp.px, hp.py, hp.pz, hp.wq,
-                                     hp.parent, hp.orig, ntriv, err);
+    const int rc = gpu_planner_order(gp, spec->partition == 0, hp.rnn.data(), lim, rw.data(), spec->n_rad, aw.data(), hp.dev, ntriv, err);
     gpu_planner_end(gp); gp = nullptr;
     if (rc != XC_OK) return rc;
   } else {
