@@ -473,7 +473,7 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
   // ---- batch records, function lists, work items ----
   const int64_t nbatch = (int64_t)leaves.size();
   hp.batches.resize(nbatch);
-  int64_t sh_off = 0, f_off = 0, ppk = 0;
+  int64_t sh_off = 0, f_off = 0, ppk = 0, wa_total = 0;
   hp.watoms.clear(); hp.wbatch_small.clear(); hp.wbatch_large.clear(); hp.w_max_small = hp.w_max_large = hp.w_max_list = 0;
   for (int64_t j = 0; j < nbatch; ++j) {
     BatchRec& b = hp.batches[j];
@@ -482,8 +482,8 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     b.f_off = (int32_t)f_off; b.nb = nbs[j];
     b.ppk_off = ppk;
     ppk += round_up(b.nb, 4) * round_up(b.nb, 8);
-    b.wa_off = (int64_t)hp.watoms.size(); b.wa_nB = wnB[j]; b.wa_nC = (int32_t)wlists[j].size();
-    hp.watoms.insert(hp.watoms.end(), wlists[j].begin(), wlists[j].end());
+    b.wa_off = wa_total; b.wa_nB = wnB[j]; b.wa_nC = (int32_t)wlists[j].size();
+    wa_total += b.wa_nC;                                  // the lists themselves are copied in parallel below
     hp.w_max_list = std::max(hp.w_max_list, (int)b.wa_nC);
     b.ntriv = ntriv[j]; b.ring_g = 0;
     if (spec->partition == 0 && b.ntriv < b.nq) {          // SSF: batches whose points are all trivial need no kernel
@@ -495,6 +495,9 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     if (sh_off >= ((int64_t)1 << 31) || f_off >= ((int64_t)1 << 31)) { err = "batch lists exceed 2^31 entries"; return XC_EUNSUPPORTED; }
   }
   hp.ppk_doubles = ppk;
+  hp.watoms.resize(wa_total);
+#pragma omp parallel for schedule(dynamic, 256)
+  for (int64_t j = 0; j < nbatch; ++j) std::copy(wlists[j].begin(), wlists[j].end(), hp.watoms.begin() + hp.batches[j].wa_off);
   hp.bshells.resize(sh_off); hp.bsfoff.resize(sh_off); hp.bfidx.resize(f_off);
 #pragma omp parallel for schedule(dynamic, 64)
   for (int64_t j = 0; j < nbatch; ++j) {

@@ -94,6 +94,14 @@ def test_w27_pbe(xc, orc):
     plan.close()
 
 
+def test_w27_pbe_resplit_batches(xc, orc):
+    """eta = 1e-20: every shell reaches so far that the bisection's batches exceed N_b^j = 192 and are split again (2515
+    batches instead of 2048, N_b^j up to 192: the class-1 kernel at its limit, the GPU planner's hand-back path)."""
+    _, plan, _, _ = _full_parity(orc, "w27", 1, eta=1e-20)
+    assert plan.n_batches > 2048 and plan.stats()["max_nb"] == 192
+    plan.close()
+
+
 @pytest.mark.parametrize("name", ["p1", "p8", "p8l", "p27"])
 def test_pure_d_shells(xc, orc, name):
     """the O d shell as five pure functions (XC_SHELL_PURE), monomer / 8 / 27
@@ -521,11 +529,13 @@ def test_tau_parity(xc, orc, name, functional):
 
 # ---- planner on the GPU, SURVEY 8(f) item 1 ----------------------------------------------------
 @pytest.mark.parametrize("name,kw", [("c1", {}), ("c1", dict(max_batch_pts=37)), ("c1", dict(max_batch_pts=1, n_ang=6, n_rad=10)),
-                                     ("w8", dict(max_batch_pts=100, angular=1, n_ang=288)), ("w27", {}), ("c2", {}), ("g1", {})])
+                                     ("w8", dict(max_batch_pts=100, angular=1, n_ang=288)), ("w27", {}), ("w27", dict(eta=1e-20)), ("c2", {}),
+                                     ("g1", {})])
 def test_gpu_planner_equals_host_planner(xc, name, kw):
     """The grid and the global median bisection run on the GPU when a plan is created for a device (xc_gpu_planner.cu); the
     host-only plan (device = -1) runs them on the host.  Every exported array must be identical: points, base weights,
-    parents, permutation, batch offsets, shell lists."""
+    parents, permutation, batch offsets, shell lists.  (w27 with eta = 1e-20: cutoff radii so large that batches exceed the
+    kernel's N_b^j limit and are split again -- the host then takes the points back from the GPU and finishes alone.)"""
     w = make_workload(name, with_P=False)
     kw = dict(kw)
     spec = xc.grid_spec(kw.pop("n_rad", w.n_rad), kw.pop("n_ang", w.n_ang), w.functional, **kw)
