@@ -839,7 +839,9 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
     }
 
     // ---- 5. V^j += Z Phi^T + Phi Z^T (lower-triangle 16x16 blocks; Eq. (18)) ----
-    // block by block (one block's fragment addresses live at a time), all T/4 k-steps of the tile per block
+    // block by block (one block's fragment addresses live at a time), all k-steps of the tile per block; the last tile of a
+    // batch stops at its last point (columns past npt hold zeros: they would add nothing)
+    const int kkn = (npt + 3) >> 2;
 #pragma unroll
     for (int r = 0; r < ROUNDS; ++r) {
       if (blk_m[r] < 0) continue;
@@ -847,7 +849,7 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
       const bool diag = blk_m[r] == blk_n[r];
       if (GGA) {
 #pragma unroll 4
-        for (int kk = 0; kk < T / 4; ++kk) {
+        for (int kk = 0; kk < kkn; ++kk) {
           const double Pm0 = sPhi[om + 4 * kk], Pm1 = sPhi[om + 8 * LD + 4 * kk], Zm0 = sZ[om + 4 * kk], Zm1 = sZ[om + 8 * LD + 4 * kk];
           const double Pn0 = sPhi[on + 4 * kk], Pn1 = sPhi[on + 8 * LD + 4 * kk], Zn0 = sZ[on + 4 * kk], Zn1 = sZ[on + 8 * LD + 4 * kk];
           // the two DMMAs of one accumulator are kept apart (a dependent DMMA waits for the result of the one before)
@@ -862,7 +864,7 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
         }
       } else {
 #pragma unroll 4
-        for (int kk = 0; kk < T / 4; ++kk) {
+        for (int kk = 0; kk < kkn; ++kk) {
           const double ai = sA[4 * kk + t4];
           const double Pm0 = sPhi[om + 4 * kk], Pm1 = sPhi[om + 8 * LD + 4 * kk];
           const double Pn0 = sPhi[on + 4 * kk], Pn1 = sPhi[on + 8 * LD + 4 * kk];
