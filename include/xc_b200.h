@@ -73,7 +73,9 @@ typedef struct xc_plan xc_plan;   /* opaque: owns host + device copies of grid, 
 /* Step (b) of the hot path + all uploads: builds the atom-centred grid (O1-O3), batches the points into
  * cuboids of <= max_batch_pts points by recursive median bisection of the whole point cloud (the batching
  * scheme is free; it satisfies Eq. (11)), screens shells per batch with Alg. 1
- * on the batch's tight bounding box, and uploads everything to `device`.
+ * on the batch's tight bounding box, and uploads everything to `device`.  With device >= 0 the per-point stages (grid
+ * points, bisection, Morton order inside the batches, the permuted point arrays) run on that GPU and the arrays stay
+ * there ("could be implemented on GPU"); the plan is bit-identical to the one the host makes.
  *   atoms   [host] natoms entries;  shells [host] nshells entries;  exps, coefs [host] nprim_total each.
  * device = -1 builds a HOST-ONLY plan (no CUDA call is made): xc_plan_info / xc_plan_stats / xc_plan_export work on
  * it, every compute entry point returns XC_ECUDA.  It exists so that the planner can be validated without a GPU.
