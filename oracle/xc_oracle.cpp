@@ -17,6 +17,8 @@
 // spin-unrestricted path and tau (readings A20-A22; tests/test_oracle_uks.py): polarised functionals vs 40-digit mpmath,
 // ferromagnetic uniform gas, zeta = 0 and spin-scaling reductions to the pinned unpolarised forms, P_a = P_b limit,
 // tr(P_s S), dE/dP^s = V^s, int tau = (2L+3) alpha/2 for one primitive, tau against the einsum definition;
+// meta-GGA MS0x+PBEc (reading A23; tests/test_oracle_uks.py): mpmath golden, Slater limit at alpha = 1, alpha = 0 for one
+// orbital, dE/dP = V with the tau term;
 // pure d shells (reading A19): typed values, orthonormality with s and p on a fine grid, Unsold's theorem, tr(PS), dE/dP = V.
 // Parity UNPINNED against the paper itself: the paper prints no E_xc / V_xc / N_el value.
 //
@@ -395,6 +397,39 @@ inline void eval_point_pol(int kind, double ra, double rb, double saa, double sa
   D5 r = f_xc_pol(kind, var5(std::max(ra, rho_tol), 0), var5(std::max(rb, rho_tol), 1), var5(saa, 2), var5(sab, 3), var5(sbb, 4));
   *f = r.v;
   for (int k = 0; k < 5; ++k) v[k] = r.d[k];
+}
+
+
+// ---- meta-GGA (reading A23): f(rho, sigma, tau), restricted -----------------
+// Exchange "MS0" (Sun, Xiao, Ruzsinszky 2012): F_x = F1(p) + f(alpha) (F0(p) - F1(p)),
+//   F_int(p; c) = 1 + kappa - kappa / (1 + (mu_GE p + c)/kappa),  F1 = F_int(p; 0),  F0 = F_int(p; c),
+//   f(alpha) = (1 - alpha^2)^3 / (1 + alpha^3 + b alpha^6),  p = s^2 = sigma / (4 (3 pi^2)^(2/3) rho^(8/3)),
+//   alpha = (tau - tau_W) / tau_unif,  tau_W = sigma / (8 rho),  tau_unif = (3/10) (3 pi^2)^(2/3) rho^(5/3),
+//   kappa = 0.29, c = 0.28771, b = 1, mu_GE = 10/81;  f_x = -C_x rho^(4/3) F_x.
+// Correlation: PBE (the unpolarised limit of f_pbe_c_pol).  D5 slots: 0 = rho, 1 = sigma, 2 = tau.
+inline D5 f_ms0_x(D5 rho, D5 sigma, D5 tau) {
+  const double kappa = 0.29, c = 0.28771, b = 1.0, muGE = 10.0 / 81.0;
+  const double k23 = std::pow(3.0 * kPi * kPi, 2.0 / 3.0);
+  D5 p = sigma / (4.0 * k23 * dpow(rho, 8.0 / 3.0));
+  D5 tauW = sigma / (8.0 * rho);
+  D5 tauU = 0.3 * k23 * dpow(rho, 5.0 / 3.0);
+  D5 al = (tau - tauW) / tauU;
+  D5 F1 = 1.0 + kappa - kappa / (1.0 + muGE * p / kappa);
+  D5 F0 = 1.0 + kappa - kappa / (1.0 + (muGE * p + c) / kappa);
+  D5 a2 = al * al, a3 = a2 * al;
+  D5 om = 1.0 - a2;
+  D5 fa = om * om * om / (1.0 + a3 + b * a3 * a3);
+  return -kCx * rho * dcbrt(rho) * (F1 + fa * (F0 - F1));
+}
+// kind 7 = MS0 exchange + PBE correlation, 8 = MS0 exchange alone (pins)
+inline bool is_mgga(int kind) { return kind == 7 || kind == 8; }
+inline void eval_point_mgga(int kind, double rho, double sigma, double tau, double rho_tol, double* f, double* v3) {
+  *f = 0.0; v3[0] = v3[1] = v3[2] = 0.0;
+  if (!(rho > rho_tol)) return;
+  D5 r = var5(rho, 0), s = var5(sigma, 1), t = var5(tau, 2);
+  D5 e = f_ms0_x(r, s, t);
+  if (kind == 7) e = e + f_pbe_c_pol(r, mk5(0.0), s);
+  *f = e.v; v3[0] = e.d[0]; v3[1] = e.d[1]; v3[2] = e.d[2];
 }
 
 }  // namespace
@@ -1068,6 +1103,105 @@ void orc_eval_uks(int64_t nbatch, const int64_t* batch_off, const int64_t* shell
   for (int64_t job = 0; job < njobs; ++job) { E += Eb[job]; A += Na[job]; B += Nb[job]; }
   if (E_out) *E_out = (double)E;
   if (N_out) { N_out[0] = (double)A; N_out[1] = (double)B; }
+}
+
+// meta-GGA functional exposed (A23): f and d f / d (rho, sigma, tau) at n points, v3 [n][3].
+void orc_functional_mgga(int kind, int64_t n, const double* rho, const double* sigma, const double* tau, double rho_tol, double* f,
+                         double* v3) {
+  for (int64_t i = 0; i < n; ++i) eval_point_mgga(kind, rho[i], sigma[i], tau[i], rho_tol, f + i, v3 + 3 * i);
+}
+
+// Alg. 4, Mode A, for a restricted meta-GGA ("with the addition of only a few
+// intermediates"; reading A23).  Besides Eqs. (13)-(15):
+//   tau_i = 1/2 sum_mu grad Phi_mu,i . grad X_mu,i,   grad X = P^j grad Phi^j
+//   Z = 1/2 (w v_rho) Phi + 2 (w v_sigma) grad rho . grad Phi                                   (Eq. (20))
+//   V^j = Z Phi^T + Phi Z^T + sum_c 1/2 (w v_tau) (d_c Phi) (d_c Phi)^T                          (d tau / d P_mu,nu = 1/2 grad phi_mu . grad phi_nu)
+// Arguments as orc_eval; tau_out (may be null) [npts].
+void orc_eval_mgga(int64_t nbatch, const int64_t* batch_off, const int64_t* shell_off, const int32_t* shells,
+                   const int64_t* subset, int64_t nsub, const double* pts, const double* w, const int32_t* shell_atom,
+                   const int32_t* shell_L, const int32_t* shell_nprim, const int32_t* shell_prim_off,
+                   const int32_t* func_off, const double* exps, const double* coefs, const double* xyz, int nbasis,
+                   const double* P, int64_t ldp, int kind, double rho_tol, double* V, double* E_out, double* N_out,
+                   double* E_b, double* N_b_out, double* rho_out, double* grho_out, double* tau_out) {
+  int64_t njobs = subset ? nsub : nbatch;
+  std::vector<long double> Eb(njobs, 0.0L), Nb(njobs, 0.0L);
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int64_t job = 0; job < njobs; ++job) {
+    int64_t j = subset ? subset[job] : job;
+    int64_t q0 = batch_off[j], nq = batch_off[j + 1] - q0;
+    const int32_t* S = shells + shell_off[j];
+    int ns = (int)(shell_off[j + 1] - shell_off[j]);
+    std::vector<int> fidx;
+    for (int k = 0; k < ns; ++k)
+      for (int c = 0; c < nfun(shell_L[S[k]]); ++c) fidx.push_back(func_off[S[k]] + c);
+    size_t nb = fidx.size();
+    if (nb == 0 || nq == 0) continue;
+    std::vector<double> Phi(nb * nq), G[3];
+    for (int c = 0; c < 3; ++c) G[c].resize(nb * nq);
+    orc_collocation(ns, S, shell_atom, shell_L, shell_nprim, shell_prim_off, exps, coefs, xyz, nq, pts + 3 * q0, Phi.data(),
+                    G[0].data(), G[1].data(), G[2].data());
+    std::vector<double> Pj(nb * nb);
+    for (size_t m = 0; m < nb; ++m)
+      for (size_t n = 0; n < nb; ++n) Pj[m * nb + n] = P[(size_t)fidx[m] * ldp + fidx[n]];
+    std::vector<double> X(nb * nq, 0.0);
+    for (size_t m = 0; m < nb; ++m)
+      for (size_t n = 0; n < nb; ++n)
+        for (int64_t i = 0; i < nq; ++i) X[m * nq + i] += Pj[m * nb + n] * Phi[n * nq + i];
+    std::vector<double> rho(nq, 0.0), gr[3], tau(nq, 0.0);
+    for (int c = 0; c < 3; ++c) gr[c].assign(nq, 0.0);
+    for (size_t m = 0; m < nb; ++m)
+      for (int64_t i = 0; i < nq; ++i) {
+        rho[i] += Phi[m * nq + i] * X[m * nq + i];
+        for (int c = 0; c < 3; ++c) gr[c][i] += 2.0 * G[c][m * nq + i] * X[m * nq + i];
+      }
+    for (int c = 0; c < 3; ++c) {
+      std::vector<double> GX(nb * nq, 0.0);
+      for (size_t m = 0; m < nb; ++m)
+        for (size_t n = 0; n < nb; ++n)
+          for (int64_t i = 0; i < nq; ++i) GX[m * nq + i] += Pj[m * nb + n] * G[c][n * nq + i];
+      for (size_t m = 0; m < nb; ++m)
+        for (int64_t i = 0; i < nq; ++i) tau[i] += 0.5 * G[c][m * nq + i] * GX[m * nq + i];
+    }
+    std::vector<double> wvr(nq), wvs(nq), wvt(nq);
+    long double e = 0.0L, nel = 0.0L;
+    for (int64_t i = 0; i < nq; ++i) {
+      double sigma = gr[0][i] * gr[0][i] + gr[1][i] * gr[1][i] + gr[2][i] * gr[2][i];
+      double f, v[3];
+      eval_point_mgga(kind, rho[i], sigma, tau[i], rho_tol, &f, v);
+      wvr[i] = w[q0 + i] * v[0]; wvs[i] = w[q0 + i] * v[1]; wvt[i] = w[q0 + i] * v[2];
+      e += (long double)w[q0 + i] * (long double)f;
+      nel += (long double)w[q0 + i] * (long double)rho[i];
+      if (rho_out) rho_out[q0 + i] = rho[i];
+      if (grho_out) for (int c = 0; c < 3; ++c) grho_out[3 * (q0 + i) + c] = gr[c][i];
+      if (tau_out) tau_out[q0 + i] = tau[i];
+    }
+    Eb[job] = e; Nb[job] = nel;
+    if (E_b) E_b[j] = (double)e;
+    if (N_b_out) N_b_out[j] = (double)nel;
+    if (!V) continue;
+    std::vector<double> Z(nb * nq);
+    for (size_t m = 0; m < nb; ++m)
+      for (int64_t i = 0; i < nq; ++i)
+        Z[m * nq + i] = 0.5 * wvr[i] * Phi[m * nq + i] +
+                        2.0 * wvs[i] * (gr[0][i] * G[0][m * nq + i] + gr[1][i] * G[1][m * nq + i] + gr[2][i] * G[2][m * nq + i]);
+    std::vector<double> Vj(nb * nb, 0.0);
+    for (size_t m = 0; m < nb; ++m)
+      for (size_t n = 0; n < nb; ++n) {
+        double acc = 0.0;
+        for (int64_t i = 0; i < nq; ++i) {
+          acc += Z[m * nq + i] * Phi[n * nq + i] + Phi[m * nq + i] * Z[n * nq + i];
+          for (int c = 0; c < 3; ++c) acc += 0.5 * wvt[i] * G[c][m * nq + i] * G[c][n * nq + i];
+        }
+        Vj[m * nb + n] = acc;
+      }
+#pragma omp critical(orc_v_increment_mgga)
+    for (size_t m = 0; m < nb; ++m)
+      for (size_t n = 0; n < nb; ++n) V[(size_t)fidx[m] * nbasis + fidx[n]] += Vj[m * nb + n];
+  }
+  long double E = 0.0L, N = 0.0L;
+  for (int64_t job = 0; job < njobs; ++job) { E += Eb[job]; N += Nb[job]; }
+  if (E_out) *E_out = (double)E;
+  if (N_out) *N_out = (double)N;
 }
 
 }  // extern "C"

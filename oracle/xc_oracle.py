@@ -289,3 +289,44 @@ def evaluate_uks(plan: Plan, w, basis, xyz, Pa, Pb, kind, rho_tol=1e-15, subset=
                        C.c_int(nbf), _d(Pa), _d(Pb), C.c_int64(Pa.shape[1]), C.c_int(kind), C.c_double(rho_tol), _d(Va), _d(Vb),
                        C.byref(E), N, _d(rho), _d(gr), _d(tau))
     return ResultUks(E.value, N[0], N[1], Va, Vb, rho, gr, tau)
+
+
+def functional_mgga(kind, rho, sigma, tau, rho_tol=1e-15):
+    """meta-GGA functional (reading A23; kind 7 = MS0 exchange + PBE correlation, 8 = MS0 exchange): f and
+    d f / d (rho, sigma, tau), shape (n, 3)."""
+    rho, sigma, tau = _f64(np.atleast_1d(rho)), _f64(np.atleast_1d(sigma)), _f64(np.atleast_1d(tau))
+    f = np.empty_like(rho)
+    v = np.empty((len(rho), 3))
+    lib().orc_functional_mgga(C.c_int(kind), C.c_int64(len(rho)), _d(rho), _d(sigma), _d(tau), C.c_double(rho_tol), _d(f), _d(v))
+    return f, v
+
+
+@dataclasses.dataclass
+class ResultMgga(Result):
+    tau: np.ndarray | None = None
+
+
+def evaluate_mgga(plan: Plan, w, basis, xyz, P, kind=7, rho_tol=1e-15, subset=None, want_V=True, want_batch=False,
+                  want_rho=False) -> ResultMgga:
+    """Mode A evaluation of a restricted meta-GGA (tau = 1/2 sum grad Phi . grad X and its potential term)."""
+    sa, sL, sn, so, ex, co = basis
+    sa, sL, sn, so, ex, co = _i32(sa), _i32(sL), _i32(sn), _i32(so), _f64(ex), _f64(co)
+    foff, nbf = _func_off(sL)
+    xyz, P, w = _f64(xyz), _f64(P), _f64(w)
+    pts = _f64(plan.pts)
+    boff, soff, sh = _i64(plan.batch_off), _i64(plan.shell_off), _i32(plan.shells)
+    nbat = len(boff) - 1
+    sub = _i64(subset) if subset is not None else None
+    V = np.zeros((nbf, nbf)) if want_V else None
+    Eb = np.zeros(nbat) if want_batch else None
+    Nb = np.zeros(nbat) if want_batch else None
+    rho = np.zeros(len(pts)) if want_rho else None
+    gr = np.zeros((len(pts), 3)) if want_rho else None
+    tau = np.zeros(len(pts)) if want_rho else None
+    E = C.c_double(0.0)
+    N = C.c_double(0.0)
+    lib().orc_eval_mgga(C.c_int64(nbat), _l(boff), _l(soff), _i(sh), _l(sub), C.c_int64(0 if sub is None else len(sub)),
+                        _d(pts), _d(w), _i(sa), _i(sL), _i(sn), _i(so), _i(foff), _d(ex), _d(co), _d(xyz), C.c_int(nbf),
+                        _d(P), C.c_int64(P.shape[1]), C.c_int(kind), C.c_double(rho_tol), _d(V), C.byref(E), C.byref(N),
+                        _d(Eb), _d(Nb), _d(rho), _d(gr), _d(tau))
+    return ResultMgga(E.value, N.value, V, Eb, Nb, rho, gr, tau)

@@ -176,3 +176,76 @@ def test_tau_pointwise_definition(orc):
         tau = 0.5 * sum(np.einsum("mi,mn,ni->i", g, P, g) for g in (gx, gy, gz))
         assert np.max(np.abs(tau - u.tau[s][sel])) <= 1e-10 * np.max(np.abs(tau))
         assert np.all(u.tau[s] >= -1e-18)
+
+
+# ---- restricted meta-GGA (reading A23: MS0 exchange + PBE correlation), PAPER.md:L51 -----------------------------------
+def test_mgga_functional_vs_mpmath_golden(orc):
+    rows = []
+    with open(os.path.join(HERE, "golden", "functional_values_mgga.txt")) as fh:
+        for line in fh:
+            if not line.startswith("#"):
+                rows.append([float(x) for x in line.split()])
+    assert len(rows) == 16
+    for row in rows:
+        f, v = orc.functional_mgga(int(row[0]), [row[1]], [row[2]], [row[3]])
+        assert f[0] == pytest.approx(row[4], rel=2e-13)
+        for k in range(3):
+            assert v[0, k] == pytest.approx(row[5 + k], rel=5e-11, abs=1e-13 * abs(row[5])), (row[:4], k)
+
+
+def test_mgga_limits(orc):
+    """alpha = 1, sigma = 0 (uniform gas): MS0 exchange = Slater exactly (kind 2, pinned); tau = tau_W (one orbital, alpha = 0):
+    F_x = F_int(p; c), typed out; f(alpha) -> 0 like alpha^-... for large alpha: F_x -> F1(p) from above."""
+    rho = np.exp(np.random.default_rng(1).uniform(-9, 3, 50))
+    k23 = (3 * math.pi ** 2) ** (2.0 / 3.0)
+    tau_u = 0.3 * k23 * rho ** (5.0 / 3.0)
+    f, v = orc.functional_mgga(8, rho, np.zeros_like(rho), tau_u)
+    f0, _, _ = orc.functional(2, rho)
+    assert np.max(np.abs(f - f0) / np.abs(f0)) < 1e-14
+    sig = rho ** (8.0 / 3.0) * 3.0
+    f, _ = orc.functional_mgga(8, rho, sig, sig / (8 * rho))
+    p = sig / (4 * k23 * rho ** (8.0 / 3.0))
+    F0 = 1 + 0.29 - 0.29 / (1 + (10.0 / 81.0 * p + 0.28771) / 0.29)
+    assert np.max(np.abs(f / (f0 * F0) - 1.0)) < 1e-13
+    # correlation part of kind 7 = PBE correlation (kind 6, pinned)
+    f7, v7 = orc.functional_mgga(7, rho, sig, 1.7 * tau_u)
+    f8, v8 = orc.functional_mgga(8, rho, sig, 1.7 * tau_u)
+    fc, vrc, vsc = orc.functional(6, rho, sig)
+    assert np.max(np.abs(f7 - f8 - fc) / np.abs(fc)) < 1e-11
+    assert np.max(np.abs(v7[:, 2] - v8[:, 2])) == 0.0 and np.max(np.abs(v7[:, 1] - v8[:, 1] - vsc) / np.abs(vsc)) < 1e-9
+
+
+def test_mgga_tau_equals_weizsaecker_for_one_orbital(orc):
+    """One doubly occupied orbital: tau = |grad rho|^2 / (8 rho) at every point (alpha = 0), from the oracle's own tau and
+    grad rho on the monomer with P = 2 c c^T."""
+    w, plan, wts = _setup(orc, "c1")
+    S = overlap_matrix(w)
+    c = np.random.default_rng(4).normal(size=w.n_basis)
+    c /= math.sqrt(c @ S @ c)
+    P = 2.0 * np.outer(c, c)
+    r = orc.evaluate_mgga(plan, wts, _basis(w), w.atoms_xyz, P, 7, want_V=False, want_rho=True)
+    m = r.rho > 1e-8
+    sigma = np.sum(r.grad_rho ** 2, axis=1)
+    assert np.max(np.abs(r.tau[m] - sigma[m] / (8 * r.rho[m])) / r.tau[m]) < 1e-7   # (cancellation in sum c phi near the orbital nodes)
+
+
+def test_mgga_symmetry_and_finite_difference(orc):
+    """dE/dP = V for the meta-GGA on the product grid: pins the factor 1/2 of the tau term and the three partials."""
+    w, plan, wts = _setup(orc, "c1", 100, 1152, 1)
+    basis = _basis(w)
+    r = orc.evaluate_mgga(plan, wts, basis, w.atoms_xyz, w.P, 7, want_rho=True)
+    assert abs(r.N_el - 10.0) < 1e-5
+    vmax = np.max(np.abs(r.V))
+    assert np.max(np.abs(r.V - r.V.T)) <= 1e-15 * vmax
+    g = orc.evaluate(plan, wts, basis, w.atoms_xyz, w.P, 1)
+    assert np.max(np.abs(r.V - g.V)) > 1e-3 * vmax and r.N_el == pytest.approx(g.N_el, rel=1e-14)   # not PBE, same density
+    h = 2e-5
+    rng = np.random.default_rng(12)
+    pairs = [(int(a), int(b)) for a, b in rng.integers(0, w.n_basis, (10, 2))] + [(3, 3), (14, 14), (24, 24)]
+    for (m, n) in pairs:
+        D = np.zeros_like(w.P)
+        D[m, n] = D[n, m] = 1.0
+        ep = orc.evaluate_mgga(plan, wts, basis, w.atoms_xyz, w.P + h * D, 7, want_V=False).E_xc
+        em = orc.evaluate_mgga(plan, wts, basis, w.atoms_xyz, w.P - h * D, 7, want_V=False).E_xc
+        expect = r.V[m, m] if m == n else 2.0 * r.V[m, n]
+        assert abs((ep - em) / (2 * h) - expect) < 1e-7 * vmax, (m, n)
