@@ -403,6 +403,17 @@ def main():
             uplan.eval_tau(Ph, reuse_weights=True)
             ev1.record()
             torch.cuda.synchronize()
+            mplan = xc.Plan.from_workload(wu, spec=xc.grid_spec(wu.n_rad, wu.n_ang, 2), device=local_rank)
+            Pf = torch.from_numpy(wu.P).cuda()
+            mplan.eval(Pf, Va)
+            tm = []
+            for _ in range(3):
+                mplan.eval(Pf, Va)
+                tm.append(mplan.timings()["total_ms"])
+            mplan.close()
+            line["mgga"] = {"workload": "c3 shapes, MS0 exchange + PBE correlation (functional = 2)", "ms_per_step": statistics.median(tm),
+                            "points_per_s": uplan.n_points / (statistics.median(tm) * 1e-3)}
+            del Pf
             line["uks"] = {"workload": "c3 (P_a = P_b = P/2)", "ms_per_step": statistics.median(tu),
                            "points_per_s": uplan.n_points / (statistics.median(tu) * 1e-3), "tau_ms_cached_weights": ev0.elapsed_time(ev1)}
             uplan.close()

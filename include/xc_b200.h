@@ -55,7 +55,8 @@ typedef struct {
   int32_t radial;         /* 0 = Mura-Knowles, m = 3 (reading A3) */
   int32_t angular;        /* 0 = Fibonacci sphere; 1 = Gauss-Legendre(cos theta) x trapezoid(phi), n_ang = 2 n_theta^2 (reading A4) */
   int32_t partition;      /* 0 = SSF, a = 0.64; 1 = Becke-1988, 3 iterations, no size adjustment (reading A1/A2) */
-  int32_t functional;     /* 0 = LDA Slater+VWN5; 1 = GGA PBE */
+  int32_t functional;     /* 0 = LDA Slater+VWN5; 1 = GGA PBE; 2 = meta-GGA MS0 exchange + PBE correlation (reading A23;
+                             PAPER.md:L51): xc_eval runs it as passes of the same kernels (densities, tau, functional, potential) */
   int32_t max_batch_pts;  /* <= 512 */
   int32_t flags;          /* bit 0: reserved */
   double  eta;            /* Eq. (10) tolerance, 1e-10 */

@@ -153,6 +153,116 @@ static int run_weights(xc_plan* p, int32_t flags, cudaStream_t st, int& launches
   return XC_OK;
 }
 
+// Restricted meta-GGA build (grid_spec.functional = 2, reading A23): the stages of Alg. 4 as passes of the same
+// kernels -- densities (MODE 1, full P^j), tau (MODE 3, lower triangle of P^j), the functional over the grid
+// (k_functional_mgga) with the per-batch E / N sums, then the potential: Z Phi^T + Phi Z^T (MODE 2) and the tau term (MODE 4)
+// into one fixed-point accumulator.
+static int eval_mgga(xc_plan* p, const double* dP, int64_t ldp, double* dV, int64_t ldv, double* E_xc, double* N_el, int32_t flags,
+                     cudaStream_t st) {
+  HostPlan& hp = p->hp;
+  const int64_t npts = hp.npts;
+  const bool diag = (flags & XC_EVAL_DIAG) != 0;
+  int launches = 0;
+  if (!p->d_urho) {
+    const size_t n = std::max<size_t>((size_t)npts, 1);
+    CU(cudaMalloc((void**)&p->d_urho, 2 * n * 8));   // rho | tau
+    CU(cudaMalloc((void**)&p->d_ugrho, 6 * n * 8));  // grad rho | w f, w rho (per point)
+    CU(cudaMalloc((void**)&p->d_ucA, 2 * n * 8));    // a | t
+    CU(cudaMalloc((void**)&p->d_ucG, 6 * n * 8));    // g
+    CU(cudaMalloc((void**)&p->d_upart, std::max<size_t>((size_t)uks_functional_blocks(npts), 1) * 3 * 8));
+    CU(cudaMalloc((void**)&p->d_ures, 4 * 8));
+  }
+  if (diag && !p->d_rho) {
+    CU(cudaMalloc((void**)&p->d_rho, std::max<size_t>(npts * 8, 8)));
+    CU(cudaMalloc((void**)&p->d_grho, std::max<size_t>(npts * 24, 8)));
+  }
+  CU(cudaEventRecord(p->ev[0], st));
+  { const int rc = run_weights(p, flags, st, launches); if (rc != XC_OK) return rc; }
+  CU(cudaEventRecord(p->ev[1], st));
+  const size_t nb2 = (size_t)hp.nbasis * hp.nbasis;
+  BatchArgs ba;
+  ba.batches = p->d_batches; ba.bshells = p->d_bshells; ba.bsfoff = p->d_bsfoff; ba.bfidx = p->d_bfidx;
+  ba.shells = p->d_shells; ba.exps = p->d_exps; ba.coefs = p->d_coefs;
+  ba.px = p->d_px; ba.py = p->d_py; ba.pz = p->d_pz; ba.w = p->d_w;
+  ba.P = dP; ba.ldp = ldp; ba.ppk = p->d_ppk;
+  ba.Epart = p->d_Epart; ba.Npart = p->d_Npart; ba.vhi = p->d_vhi; ba.vlo = p->d_vlo; ba.nbasis = hp.nbasis;
+  ba.rho_tol = hp.spec.rho_tol; ba.vexp = p->vexp;
+  ba.vflags = (unsigned*)(p->d_result + 2);
+  ba.cA = nullptr; ba.cG = nullptr;
+  double* d_rho = p->d_urho; double* d_tau = p->d_urho + npts;
+  double* d_gr = p->d_ugrho; double* d_ef = p->d_ugrho + 3 * npts; double* d_en = d_ef + npts;
+  double* d_a = p->d_ucA; double* d_t = p->d_ucA + npts;
+  const int nl = (int)hp.ids_large.size(), nsm = (int)hp.ids_small.size();
+  // densities: full P^j
+  ba.rho_out = d_rho; ba.grho_out = d_gr;
+  if (nl) { CUK(launch_pack(ba, p->d_ids_large, nl, false, st), st); ++launches; }
+  if (nsm) { CUK(launch_pack(ba, p->d_ids_small, nsm, false, st), st); ++launches; }
+  if (nl) { CUK(launch_batch(1, true, 1, ba, p->d_ids_large, nl, hp.smem_large, st), st); ++launches; }
+  if (nsm) { CUK(launch_batch(0, true, 1, ba, p->d_ids_small, nsm, hp.smem_small, st), st); ++launches; }
+  // tau: lower triangle of P^j
+  ba.rho_out = d_tau; ba.grho_out = nullptr;
+  if (nl) { CUK(launch_pack(ba, p->d_ids_large, nl, true, st), st); ++launches; }
+  if (nsm) { CUK(launch_pack(ba, p->d_ids_small, nsm, true, st), st); ++launches; }
+  if (nl) { CUK(launch_batch(1, false, 3, ba, p->d_ids_large, nl, hp.smem_large, st), st); ++launches; }
+  if (nsm) { CUK(launch_batch(0, false, 3, ba, p->d_ids_small, nsm, hp.smem_small, st), st); ++launches; }
+  CU(cudaEventRecord(p->ev[2], st));
+  // functional, per-batch partial sums
+  CUK(launch_functional_mgga(npts, (int)hp.batches.size(), p->d_batches, p->d_w, d_rho, d_gr, d_tau, hp.spec.rho_tol, d_a, p->d_ucG, d_t, d_ef,
+                             d_en, p->d_Epart, p->d_Npart, st), st);
+  launches += 2;
+  if (diag) {
+    CU(cudaMemcpyAsync(p->d_rho, d_rho, (size_t)npts * 8, cudaMemcpyDeviceToDevice, st));
+    CU(cudaMemcpyAsync(p->d_grho, d_gr, (size_t)npts * 24, cudaMemcpyDeviceToDevice, st));
+  }
+  p->diag_valid = diag;
+  ba.rho_out = nullptr; ba.grho_out = nullptr;
+  for (int attempt = 0;; ++attempt) {
+    ba.vexp = p->vexp;
+    CU(cudaMemsetAsync(p->d_vhi, 0, nb2 * 8, st));
+    CU(cudaMemsetAsync(p->d_vlo, 0, nb2 * 8, st));
+    CU(cudaMemsetAsync(p->d_result + 2, 0, 16, st));
+    ba.cA = d_a; ba.cG = p->d_ucG;
+    if (nl) { CUK(launch_batch(1, true, 2, ba, p->d_ids_large, nl, hp.smem_large, st), st); ++launches; }
+    if (nsm) { CUK(launch_batch(0, true, 2, ba, p->d_ids_small, nsm, hp.smem_small, st), st); ++launches; }
+    ba.cA = d_t; ba.cG = nullptr;
+    if (nl) { CUK(launch_batch(1, false, 4, ba, p->d_ids_large, nl, hp.smem_large, st), st); ++launches; }
+    if (nsm) { CUK(launch_batch(0, false, 4, ba, p->d_ids_small, nsm, hp.smem_small, st), st); ++launches; }
+    CUK(launch_reduce((int64_t)hp.batches.size(), p->d_Epart, p->d_Npart, p->d_result, st), st);
+    CUK(launch_finalize(hp.nbasis, p->d_vhi, p->d_vlo, dV, ldv, p->vexp, false, st), st);
+    launches += 2;
+    CU(cudaMemcpyAsync(p->h_result, p->d_result, 32, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    unsigned vf[4];
+    std::memcpy(vf, p->h_result + 2, 16);
+    if (vf[1] != 0) {
+      CUK(launch_finalize(hp.nbasis, p->d_vhi, p->d_vlo, dV, ldv, p->vexp, true, st), st);
+      CU(cudaStreamSynchronize(st));
+      *E_xc = *N_el = std::nan("");
+      return fail(XC_EINVAL, "non-finite value met while accumulating V (NaN or Inf in P, or overflow); V is filled with NaN");
+    }
+    const int e = vf[0] ? (int)(vf[0] >> 20) - 1023 : p->vexp;
+    const bool fits = p->vexp >= e - 10 && p->vexp <= e + 14;
+    if (fits || attempt == 1) {
+      if (!fits) return fail(XC_EUNSUPPORTED, "V increments span more than the fixed-point accumulator covers");
+      break;
+    }
+    p->vexp = e - 8;
+  }
+  CU(cudaEventRecord(p->ev[3], st));
+  CU(cudaEventRecord(p->ev[4], st));
+  CU(cudaStreamSynchronize(st));
+  *E_xc = p->h_result[0];
+  *N_el = p->h_result[1];
+  float t;
+  CU(cudaEventElapsedTime(&t, p->ev[0], p->ev[1])); p->ms[0] = t;   // weights
+  CU(cudaEventElapsedTime(&t, p->ev[1], p->ev[2])); p->ms[1] = t;   // packs, densities, tau
+  CU(cudaEventElapsedTime(&t, p->ev[2], p->ev[3])); p->ms[2] = t;   // functional and potential passes
+  p->ms[3] = 0.f;
+  CU(cudaEventElapsedTime(&t, p->ev[0], p->ev[4])); p->ms[4] = t;
+  p->launches = launches;
+  return XC_OK;
+}
+
 extern "C" {
 
 const char* xc_strerror(int code) {
@@ -292,6 +402,10 @@ int xc_eval(xc_plan* p, const double* dP, int64_t ldp, double* dV, int64_t ldv, 
   if (ldp < hp.nbasis || ldv < hp.nbasis) return fail(XC_EINVAL, "leading dimension smaller than n_basis");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   DeviceGuard guard(p->device);
+  if (hp.spec.functional == 2) {
+    if (p->wait_P) { p->wait_P = false; CU(cudaStreamWaitEvent(st, p->ev_P, 0)); }
+    return eval_mgga(p, dP, ldp, dV, ldv, E_xc, N_el, flags, st);
+  }
   const bool gga = hp.spec.functional == 1;
   const bool diag = (flags & XC_EVAL_DIAG) != 0;
   int launches = 0;
@@ -382,6 +496,7 @@ int xc_eval_uks(xc_plan* p, const double* dPa, const double* dPb, int64_t ldp, d
   HostPlan& hp = p->hp;
   if (ldp < hp.nbasis || ldv < hp.nbasis) return fail(XC_EINVAL, "leading dimension smaller than n_basis");
   if (!(hp.spec.rho_tol > 0.0)) return fail(XC_EINVAL, "the spin-unrestricted build needs rho_tol > 0 (reading A20)");
+  if (hp.spec.functional > 1) return fail(XC_EUNSUPPORTED, "the spin-unrestricted build knows Slater+VWN5 and PBE only");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   DeviceGuard guard(p->device);
   const bool gga = hp.spec.functional == 1;

@@ -428,7 +428,9 @@ struct BatchCfg {
 // live points written to rho_out / grho_out; then k_functional_uks couples the spins; MODE 2 = stages 1, 4-6 with the
 // per-point coefficients of Z^s read from cA / cG instead of a functional evaluation.  MODE 3 (xc_eval_tau): the meta-GGA
 // intermediate tau = 1/2 sum_mu grad Phi_mu . grad X_mu: stages 1-2 once per gradient component with
-// d_c Phi in the Phi buffer, tau = sum_c (d_c Phi)^T L (d_c Phi) from the LDA epilogue, written to rho_out.
+// d_c Phi in the Phi buffer, tau = sum_c (d_c Phi)^T L (d_c Phi) from the LDA epilogue, written to rho_out.  MODE 4 (restricted
+// meta-GGA, reading A23): stages 1, 5, 6 once per gradient component, V^j += sum_i (1/2 w v_tau)_i d_c Phi_mu,i d_c Phi_nu,i
+// with the coefficient read from cA, accumulated in the same registers over the three components.
 template <int NT, int T, bool GGA, int NTW, int ROUNDS, int MINB, int MODE>
 __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_t* __restrict__ batch_ids) {
   using Cfg = BatchCfg<NT, T>;
@@ -542,9 +544,9 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
   PRing ring;
   ring.ppk = a.ppk + b.ppk_off; ring.buf = sRing; ring.full = sBar; ring.empty = sBar + kRingStages;
   ring.ntile = ntile; ring.nks = nks; ring.G = max(1, b.ring_g); ring.spp = (nks + ring.G - 1) / ring.G;
-  ring.total = (MODE == 2 || !GGA) ? 0u : (unsigned)(((nqe + T - 1) / T) * ring.spp);   // GGA X GEMM only
+  ring.total = (MODE == 2 || MODE == 4 || !GGA) ? 0u : (unsigned)(((nqe + T - 1) / T) * ring.spp);   // GGA X GEMM only
   ring.n = 0;
-  if (MODE != 2 && GGA && tid == 0) {
+  if (MODE != 2 && MODE != 4 && GGA && tid == 0) {
     for (int k = 0; k < kRingStages; ++k) { mbar_init(ring.full + k, 1); mbar_init(ring.empty + k, Cfg::NW); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -554,7 +556,8 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
   double Eacc = 0.0, Nacc = 0.0;
   PH_DECL
   PH(0);
-  for (int t0 = 0, it = 0; t0 < nqe; t0 += T, ++it) {
+  // MODE 4 visits every tile three times (c4 = gradient component), the other modes once
+  for (int t0 = 0, it = 0, c4 = 0; t0 < nqe; (MODE == 4 && c4 < 2) ? (void)++c4 : (void)(c4 = 0, t0 += T, ++it)) {
     const int npt = min(T, nqe - t0);          // valid points in this tile
     const double* sx = sPt + (size_t)(it & 1) * 4 * T;   // this tile's points (written one tile ahead)
     const double *sy = sx + T, *sz = sx + 2 * T, *sw = sx + 3 * T;
@@ -582,11 +585,12 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
       }
       if (GGA) *reinterpret_cast<double2*>(sR + ((size_t)slot * T + i) * 2) = make_double2(R0, R1);
       double* dst = sPhi + (size_t)sh._pad * LD + i;
-      if (MODE == 3) {
+      if (MODE == 3 || MODE == 4) {
         // d/dr_c of the shell's functions: d_c (m R0) = (d_c m) R0 + m (r - R)_c R1
-        const double dc = comp == 0 ? dx : (comp == 1 ? dy : dz);
+        const int dcomp = MODE == 4 ? c4 : comp;
+        const double dc = dcomp == 0 ? dx : (dcomp == 1 ? dy : dz);
         const double base = dc * R1;
-        const double ex = comp == 0 ? R0 : 0.0, ey = comp == 1 ? R0 : 0.0, ez = comp == 2 ? R0 : 0.0;   // R0 d(r - R)_k / dr_c
+        const double ex = dcomp == 0 ? R0 : 0.0, ey = dcomp == 1 ? R0 : 0.0, ez = dcomp == 2 ? R0 : 0.0;   // R0 d(r - R)_k / dr_c
         if (sh.L == 0) {
           dst[0] = base;
         } else if (sh.L == 1) {
@@ -621,7 +625,7 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
     PH(2);
 
     // ---- 2. X^T = Phi^T P^j and the density reductions ----
-    if (MODE != 2) {
+    if (MODE != 2 && MODE != 4) {
       double C[2][NTW][2];
 #pragma unroll
       for (int u = 0; u < 2; ++u)
@@ -687,12 +691,12 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
         }
       }
     }
-    if (MODE != 2) __syncthreads();
+    if (MODE != 2 && MODE != 4) __syncthreads();
     if (MODE == 3 && tid < T) {                  // (grad_c Phi)^T L (grad_c Phi) = 1/2 (grad_c Phi)^T P (grad_c Phi): tau's share
       for (int q = 0; q < Cfg::WM; ++q) tau_acc += sRed[(size_t)(q * 4) * T + tid];
     }
     }                                            // component loop (one pass unless MODE 3)
-    if (GGA && MODE != 2) {
+    if (GGA && MODE != 2 && MODE != 4) {
       // density pass per (shell, point): thread = (group, point); a group walks over the shells group, group + NG, ...
       const int i = tid % T, grp = tid / T;
       const double xi = sx[i], yi = sy[i], zi = sz[i];
@@ -746,14 +750,14 @@ __global__ void __launch_bounds__(NT, MINB) k_xc_batch(BatchArgs a, const int32_
       nx[li] = a.px[gi]; nx[T + li] = a.py[gi]; nx[2 * T + li] = a.pz[gi];
       nx[3 * T + li] = li < nn ? a.w[gi] : 0.0;
     }
-    if (tid < T && MODE == 2) {
+    if (tid < T && (MODE == 2 || MODE == 4)) {
       // per-point coefficients of Z^s from the functional kernel: a (LDA: w v_rho_s; GGA: 1/2 w v_rho_s), g (GGA)
       const int64_t gi = (int64_t)b.pt_off + sLive[t0 + min(tid, npt - 1)];
       const bool ok = tid < npt;
       sA[tid] = ok ? a.cA[gi] : 0.0;
       if (GGA) { sG0[tid] = ok ? a.cG[3 * gi] : 0.0; sG1[tid] = ok ? a.cG[3 * gi + 1] : 0.0; sG2[tid] = ok ? a.cG[3 * gi + 2] : 0.0; }
     }
-    if (tid < T && MODE != 2) {
+    if (tid < T && MODE != 2 && MODE != 4) {
       double rho = 0.0, gx = 0.0, gy = 0.0, gz = 0.0;
       for (int q = 0; q < (GGA ? Cfg::NG : Cfg::WM); ++q) {
         rho += sRed[(size_t)(q * 4 + 0) * T + tid];
@@ -998,6 +1002,10 @@ cudaError_t launch_batch(int cls, bool gga, int mode, const BatchArgs& a, const 
   if (nbatches <= 0) return cudaSuccess;
   if (mode == 1) return launch_batch_m<1>(cls, gga, a, batch_ids, nbatches, smem, st);
   if (mode == 2) return launch_batch_m<2>(cls, gga, a, batch_ids, nbatches, smem, st);
+  if (mode == 4) {   // tau term of a meta-GGA potential: V^j += sum_c (t d_c Phi)(d_c Phi)^T, the LDA (symmetric) V^j GEMM per component
+    return cls == 0 ? launch_batch_t<512, 64, false, 4, 2, 1, 4>(a, batch_ids, nbatches, smem, st)
+                    : launch_batch_t<512, 32, false, 3, 5, 1, 4>(a, batch_ids, nbatches, smem, st);
+  }
   if (mode == 3) {   // tau: gradient components through the LDA (lower-triangle) X GEMM, whatever the plan's functional
     return cls == 0 ? launch_batch_t<512, 64, false, 4, 2, 1, 3>(a, batch_ids, nbatches, smem, st)
                     : launch_batch_t<512, 32, false, 3, 5, 1, 3>(a, batch_ids, nbatches, smem, st);

@@ -53,6 +53,10 @@ cudaError_t launch_batch(int cls, bool gga, int mode, const BatchArgs& a, const 
 int64_t uks_functional_blocks(int64_t npts);
 cudaError_t launch_functional_uks(bool gga, int64_t npts, const double* w, const double* rho, const double* grho, double rho_tol,
                                   double* cA, double* cG, double* part, double* out3, cudaStream_t st);
+// restricted meta-GGA (reading A23): functional over the grid and per-batch E / N partials (xc_uks.cu)
+cudaError_t launch_functional_mgga(int64_t npts, int nbatches, const BatchRec* batches, const double* w, const double* rho, const double* grho,
+                                   const double* tau, double rho_tol, double* cA, double* cG, double* cT, double* ef, double* en, double* Epart,
+                                   double* Npart, cudaStream_t st);
 cudaError_t launch_finalize(int nbasis, const unsigned long long* vhi, const unsigned long long* vlo, double* V,
                             int64_t ldv, int vexp, bool poison, cudaStream_t st);
 cudaError_t launch_reduce(int64_t n, const double* ep, const double* np, double* out, cudaStream_t st);

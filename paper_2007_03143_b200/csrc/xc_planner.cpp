@@ -162,7 +162,7 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     err = "bad grid_spec sizes (need n_rad,n_ang >= 1 and 1 <= max_batch_pts <= 512)"; return XC_EINVAL;
   }
   if (spec->radial != 0 || spec->angular < 0 || spec->angular > 1 || spec->partition < 0 || spec->partition > 1 ||
-      spec->functional < 0 || spec->functional > 1) { err = "bad grid_spec enum"; return XC_EINVAL; }
+      spec->functional < 0 || spec->functional > 2) { err = "bad grid_spec enum"; return XC_EINVAL; }
   if (!(spec->eta > 0.0) || !(spec->mk_alpha > 0.0) || !(spec->rho_tol >= 0.0)) { err = "bad grid_spec reals"; return XC_EINVAL; }
   hp.natoms = natoms; hp.nshells = nshells; hp.nprim = nprim_total; hp.spec = *spec;
   hp.atoms.resize(3 * (size_t)natoms);
@@ -321,7 +321,7 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
     atom_shells[hp.shells[s].atom].push_back(s);
     atom_rmax[hp.shells[s].atom] = std::max(atom_rmax[hp.shells[s].atom], hp.rcut[s]);
   }
-  const bool gga = spec->functional == 1;
+  const bool gga = spec->functional >= 1;       // 2 = meta-GGA (reading A23): the GGA footprint covers its passes
   auto screen = [&](const Leaf& lf, std::vector<int32_t>& out, int& nb, const double* known_box = nullptr) {
     Box b;
     if (known_box) {

@@ -95,10 +95,9 @@ __device__ __forceinline__ T5 pbe_x_channel(const T5& r2, const T5& s4) {   // u
   const T5 F = (1.0 + kappa) - (kappa * kappa) / (kappa + mu * s2);
   return (-kCx) * r43 * F;
 }
-__device__ __forceinline__ T5 pbe_pol(const T5& ra, const T5& rb, const T5& saa, const T5& sab, const T5& sbb) {
+// PBE correlation at (rho, zeta, sigma = |grad rho|^2), per unit volume
+__device__ __forceinline__ T5 pbe_c_pol(const T5& rho, const T5& z, const T5& sigma) {
   const double gamma = 0.031090690869654895, beta = 0.06672455060314922;
-  const T5 rho = ra + rb, z = (ra - rb) / rho, sigma = saa + 2.0 * sab + sbb;
-  const T5 fx = 0.5 * (pbe_x_channel(2.0 * ra, 4.0 * saa) + pbe_x_channel(2.0 * rb, 4.0 * sbb));
   const T5 r13 = tcbrt(rho);
   const T5 rs = kRs / r13, srs = tsqrt(rs);
   const T5 e0 = pw92_fit(rs, srs, 0.0310907, 0.21370, 7.5957, 3.5876, 1.6382, 0.49294);
@@ -113,7 +112,28 @@ __device__ __forceinline__ T5 pbe_pol(const T5& ra, const T5& rb, const T5& saa,
   const T5 Ac = (beta / gamma) / texpm1((-1.0 / gamma) * eu / phi3);
   const T5 At = Ac * t2;
   const T5 H = gamma * phi3 * tlog1p((beta / gamma) * t2 * (1.0 + At) / (1.0 + At + At * At));
-  return fx + rho * (eu + H);
+  return rho * (eu + H);
+}
+__device__ __forceinline__ T5 pbe_pol(const T5& ra, const T5& rb, const T5& saa, const T5& sab, const T5& sbb) {
+  const T5 rho = ra + rb, z = (ra - rb) / rho, sigma = saa + 2.0 * sab + sbb;
+  const T5 fx = 0.5 * (pbe_x_channel(2.0 * ra, 4.0 * saa) + pbe_x_channel(2.0 * rb, 4.0 * sbb));
+  return fx + pbe_c_pol(rho, z, sigma);
+}
+// restricted meta-GGA of reading A23: MS0 exchange (Sun, Xiao, Ruzsinszky 2012) + PBE correlation; tangent slots 0 = rho,
+// 1 = sigma, 2 = tau.  F_x = F1 + f(alpha) (F0 - F1), F_int(p; c) = 1 + kappa - kappa^2 / (kappa + mu_GE p + c)
+__device__ __forceinline__ T5 mgga_ms0_pbe(const T5& rho, const T5& sigma, const T5& tau) {
+  const double kappa = 0.29, c = 0.28771, muGE = 10.0 / 81.0;
+  const double k23 = 9.5707800006273037;         // (3 pi^2)^(2/3)
+  const T5 r13 = tcbrt(rho), r23 = r13 * r13;
+  const T5 r43 = rho * r13, r53 = rho * r23;
+  const T5 p = sigma / ((4.0 * k23) * r43 * r43);
+  const T5 al = (tau - sigma / (8.0 * rho)) / ((0.3 * k23) * r53);
+  const T5 F1 = (1.0 + kappa) - (kappa * kappa) / (kappa + muGE * p);
+  const T5 F0 = (1.0 + kappa) - (kappa * kappa) / ((kappa + c) + muGE * p);
+  const T5 a2 = al * al, a3 = a2 * al, om = 1.0 - a2;
+  const T5 fa = om * om * om / (1.0 + a3 + a3 * a3);
+  const T5 fx = (-kCx) * r43 * (F1 + fa * (F0 - F1));
+  return fx + pbe_c_pol(rho, cst(0.0), sigma);
 }
 
 constexpr int kUksThreads = 256;
@@ -195,6 +215,61 @@ __global__ void __launch_bounds__(1024) k_reduce3(int64_t n, const double* __res
 }
 
 int64_t uks_functional_blocks(int64_t npts) { return (npts + kUksThreads - 1) / kUksThreads; }
+
+// restricted meta-GGA: per point f(rho, sigma, tau) and the coefficients of the potential: a = 1/2 w v_rho, g = 2 w v_sigma
+// grad rho (Eq. (20)), t = 1/2 w v_tau (the tau term of V^j); w f and w rho per point for the per-batch sums
+__global__ void __launch_bounds__(kUksThreads) k_functional_mgga(int64_t npts, const double* __restrict__ w, const double* __restrict__ rho,
+                                                                 const double* __restrict__ grho, const double* __restrict__ tau, double rho_tol,
+                                                                 double* __restrict__ cA, double* __restrict__ cG, double* __restrict__ cT,
+                                                                 double* __restrict__ ef, double* __restrict__ en) {
+  const int64_t i = (int64_t)blockIdx.x * kUksThreads + threadIdx.x;
+  if (i >= npts) return;
+  const double wi = w[i];
+  double a = 0.0, t = 0.0, g[3] = {0.0, 0.0, 0.0}, e = 0.0, n = 0.0;
+  if (wi != 0.0) {
+    const double r = rho[i], x[3] = {grho[3 * i], grho[3 * i + 1], grho[3 * i + 2]};
+    n = wi * r;
+    if (!(r <= rho_tol)) {                       // a NaN density is not skipped: it propagates
+      const double sigma = x[0] * x[0] + x[1] * x[1] + x[2] * x[2];
+      const T5 f = mgga_ms0_pbe(seed(r, 0), seed(sigma, 1), seed(tau[i], 2));
+      e = wi * f.v;
+      a = 0.5 * wi * f.t[0];
+      t = 0.5 * wi * f.t[2];
+      const double gs = 2.0 * wi * f.t[1];
+      for (int c = 0; c < 3; ++c) g[c] = gs * x[c];
+    }
+  }
+  cA[i] = a; cT[i] = t;
+  for (int c = 0; c < 3; ++c) cG[3 * i + c] = g[c];
+  ef[i] = e; en[i] = n;
+}
+// per-batch sums of w f and w rho (Eq. (16)): one block per batch, fixed order
+__global__ void __launch_bounds__(128) k_batch_sums(const BatchRec* __restrict__ batches, const double* __restrict__ ef,
+                                                    const double* __restrict__ en, double* __restrict__ Epart, double* __restrict__ Npart) {
+  __shared__ double se[128], sn[128];
+  const BatchRec b = batches[blockIdx.x];
+  double e = 0.0, n = 0.0;
+  for (int k = threadIdx.x; k < b.nq; k += 128) { e += ef[(int64_t)b.pt_off + k]; n += en[(int64_t)b.pt_off + k]; }
+  se[threadIdx.x] = e; sn[threadIdx.x] = n;
+  __syncthreads();
+  for (int s = 64; s >= 1; s >>= 1) {
+    if ((int)threadIdx.x < s) { se[threadIdx.x] += se[threadIdx.x + s]; sn[threadIdx.x] += sn[threadIdx.x + s]; }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) { Epart[blockIdx.x] = se[0]; Npart[blockIdx.x] = sn[0]; }
+}
+
+cudaError_t launch_functional_mgga(int64_t npts, int nbatches, const BatchRec* batches, const double* w, const double* rho, const double* grho,
+                                   const double* tau, double rho_tol, double* cA, double* cG, double* cT, double* ef, double* en, double* Epart,
+                                   double* Npart, cudaStream_t st) {
+  if (npts <= 0 || nbatches <= 0) return cudaSuccess;
+  k_functional_mgga<<<(unsigned)uks_functional_blocks(npts), kUksThreads, 0, st>>>(npts, w, rho, grho, tau, rho_tol, cA, cG, cT, ef, en);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  k_batch_sums<<<nbatches, 128, 0, st>>>(batches, ef, en, Epart, Npart);
+  return cudaGetLastError();
+}
+
 
 cudaError_t launch_functional_uks(bool gga, int64_t npts, const double* w, const double* rho, const double* grho, double rho_tol,
                                   double* cA, double* cG, double* part, double* out3, cudaStream_t st) {

@@ -546,3 +546,37 @@ def test_gpu_planner_equals_host_planner(xc, name, kw):
         assert np.array_equal(getattr(a, f), getattr(b, f)), f
     assert pd.stats() == ph.stats()
     pd.close(); ph.close()
+
+
+# ---- restricted meta-GGA, SURVEY 8(f) item 3 (reading A23: MS0 exchange + PBE correlation) -----------------
+@pytest.mark.parametrize("name", ["c1", "w8", "p8", "w27"])
+def test_mgga_parity(xc, orc, name):
+    """grid_spec.functional = 2: xc_eval runs the meta-GGA as passes of the batch kernel (densities, tau, functional, Z / V^j,
+    tau term of V^j).  Against the oracle's literal Alg. 4 with tau on the library's plan: V, E_xc, N_el at the north_star
+    tolerances, rho / grad rho and the per-batch sums point by point; bit-identical repeat."""
+    import torch
+    w = make_workload(name)
+    plan = xc.Plan.from_workload(w, spec=xc.grid_spec(w.n_rad, w.n_ang, 2))
+    P = torch.from_numpy(w.P).cuda()
+    E, N, V = plan.eval(P, diag=True)
+    d = plan.diagnostics(want_points=True, want_rho=True)
+    ex = plan.export()
+    op = oracle_plan(orc, ex)
+    wts = orc.partition_weights(w.atoms_xyz, op.pts, op.wq, op.parent, 0, True)
+    r = orc.evaluate_mgga(op, wts, basis_of(w), w.atoms_xyz, w.P, 7, want_batch=True, want_rho=True)
+    vmax = np.max(np.abs(r.V))
+    Vh = V.cpu().numpy()
+    assert np.max(np.abs(Vh - r.V)) <= TOL_V * vmax and np.array_equal(Vh, Vh.T)
+    assert abs(E - r.E_xc) <= TOL_S * abs(r.E_xc) and abs(N - r.N_el) <= TOL_S * r.N_el
+    assert np.max(np.abs(d["w"] - wts)) <= 1e-13 * np.max(wts)
+    m = d["w"] != 0.0
+    assert np.max(np.abs(d["rho"][m] - r.rho[m])) <= 1e-12 * np.max(np.abs(r.rho))
+    assert np.max(np.abs(d["grad_rho"][m] - r.grad_rho[m])) <= 1e-12 * np.max(np.abs(r.grad_rho))
+    assert np.max(np.abs(d["E_batch"] - r.E_batch)) <= 1e-12 * abs(r.E_xc)
+    assert np.max(np.abs(d["N_batch"] - r.N_batch)) <= 1e-12 * abs(r.N_el)
+    # it is not PBE: the tau-dependent exchange changes V
+    g = orc.evaluate(op, wts, basis_of(w), w.atoms_xyz, w.P, 1, want_V=True)
+    assert np.max(np.abs(Vh - g.V)) > 1e-3 * vmax
+    E2, N2, V2 = plan.eval(P, reuse_weights=True)
+    assert E2 == E and N2 == N and torch.equal(V, V2)
+    plan.close()
