@@ -79,7 +79,7 @@ def test_product_rule_and_bad_specs(xc):
     p = xc.Plan.from_workload(w, device=-1, spec=xc.grid_spec(10, 288, 0, angular=1))
     assert p.n_points == 3 * 10 * 288
     p.close()
-    for bad in (xc.grid_spec(10, 287, 0, angular=1), xc.grid_spec(0, 26, 0), xc.grid_spec(10, 26, 2),
+    for bad in (xc.grid_spec(10, 287, 0, angular=1), xc.grid_spec(0, 26, 0), xc.grid_spec(10, 26, 3),
                 xc.grid_spec(10, 26, 0, eta=0.0), xc.grid_spec(10, 26, 0, max_batch_pts=513)):
         with pytest.raises(xc.XcError) as e:
             xc.Plan.from_workload(w, device=-1, spec=bad)
