@@ -51,7 +51,7 @@ def _peaks():
 
 def _ncu_traffic(workload, kernel):
     """dram bytes per launch of `kernel` from the committed ncu --set full capture of this round (profiles/), or None."""
-    p = os.path.join(ROOT, "profiles", "r02_ncu_traffic.json")
+    p = os.path.join(ROOT, "profiles", "r02_ncu_traffic.txt")
     try:
         with open(p) as fh:
             return json.load(fh).get(workload, {}).get(kernel)
