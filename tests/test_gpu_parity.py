@@ -580,3 +580,50 @@ def test_mgga_parity(xc, orc, name):
     E2, N2, V2 = plan.eval(P, reuse_weights=True)
     assert E2 == E and N2 == N and torch.equal(V, V2)
     plan.close()
+
+
+def test_extensions_at_c3_size_sampled(xc, orc):
+    """The spin-unrestricted and meta-GGA builds on the 64-water PBE shapes (4.3 M points, 1600 functions): 60 random batches
+    against the oracle point by point (rho_s, grad rho_s, tau) and per batch (meta-GGA E / N sums); electron counts against
+    tr(P_s S) = n_s at the Fibonacci-grid accuracy; V symmetric and bit-identical on repeat."""
+    import torch
+    from workloads import spin_density_matrices
+    w = make_workload("c3")
+    Pa, Pb = spin_density_matrices(w, 330, 310)
+    plan = xc.Plan.from_workload(w, spec=xc.grid_spec(w.n_rad, w.n_ang, 1))
+    Pad, Pbd = torch.from_numpy(Pa).cuda(), torch.from_numpy(Pb).cuda()
+    E, (Na, Nb), Va, Vb = plan.eval_uks(Pad, Pbd)
+    assert abs(Na - 330.0) / 330.0 < 2e-4 and abs(Nb - 310.0) / 310.0 < 2e-4
+    assert torch.equal(Va, Va.T) and torch.equal(Vb, Vb.T)
+    rho, gr = plan.uks_densities()
+    ta = plan.eval_tau(Pad, reuse_weights=True).cpu().numpy()
+    ex = plan.export()
+    op = oracle_plan(orc, ex)
+    sub = np.sort(np.random.default_rng(21).choice(plan.n_batches, 60, replace=False))
+    pidx = np.concatenate([np.arange(ex.batch_off[j], ex.batch_off[j + 1]) for j in sub])
+    gw = plan.diagnostics()["w"]
+    wts = np.zeros(len(ex.wq))
+    wts[pidx] = orc.partition_weights(w.atoms_xyz, ex.pts[pidx], ex.wq[pidx], ex.parent[pidx], 0, True)
+    assert np.max(np.abs(gw[pidx] - wts[pidx])) <= 1e-13 * np.max(ex.wq)
+    r = orc.evaluate_uks(op, wts, basis_of(w), w.atoms_xyz, Pa, Pb, 1, subset=sub, want_V=False, want_rho=True, want_tau=True)
+    m = pidx[gw[pidx] != 0.0]
+    for s in range(2):
+        assert np.max(np.abs(rho[s][m] - r.rho[s][m])) <= 1e-12 * np.max(np.abs(r.rho))
+        assert np.max(np.abs(gr[s][m] - r.grad_rho[s][m])) <= 1e-12 * np.max(np.abs(r.grad_rho))
+    assert np.max(np.abs(ta[m] - r.tau[0][m])) <= 1e-12 * np.max(np.abs(r.tau))
+    E2, N2, Va2, Vb2 = plan.eval_uks(Pad, Pbd, reuse_weights=True)
+    assert E2 == E and torch.equal(Va, Va2) and torch.equal(Vb, Vb2)
+    plan.close()
+    # meta-GGA on the same cluster
+    mplan = xc.Plan.from_workload(w, spec=xc.grid_spec(w.n_rad, w.n_ang, 2))
+    P = torch.from_numpy(w.P).cuda()
+    Em, Nm, Vm = mplan.eval(P, diag=True)
+    assert abs(Nm - 640.0) / 640.0 < 2e-4 and torch.equal(Vm, Vm.T)
+    d = mplan.diagnostics(want_points=True, want_rho=True)
+    exm = mplan.export()
+    assert np.array_equal(exm.orig, ex.orig)                 # same plan (the functional only sizes the shared memory)
+    rm = orc.evaluate_mgga(op, wts, basis_of(w), w.atoms_xyz, w.P, 7, subset=sub, want_V=False, want_batch=True, want_rho=True)
+    assert np.max(np.abs(d["rho"][m] - rm.rho[m])) <= 1e-12 * np.max(np.abs(rm.rho))
+    assert np.max(np.abs(d["E_batch"][sub] - rm.E_batch[sub])) <= 1e-12 * abs(Em)
+    assert np.max(np.abs(d["N_batch"][sub] - rm.N_batch[sub])) <= 1e-12 * abs(Nm)
+    mplan.close()
