@@ -184,6 +184,27 @@ int xc_partition_weights(const xc_atom* atoms /*[host]*/, int32_t natoms, int32_
 int xc_functional(int32_t functional, int64_t n, const double* drho, const double* dsigma, double rho_tol,
                   double* df, double* dvrho, double* dvsigma, void* cuda_stream);
 
+/* The spin-coupling step of the spin-unrestricted build (Alg. 4 l.4.6-4.7 per spin; DESIGN.md readings
+ * A20-A21) as a call that ALLOCATES NOTHING -- for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * serving loops, harnesses that forbid it).  It is the kernel pair xc_eval_uks runs between its density and potential
+ * passes; the per-block partial sums go to a file-scope device array of the library instead of a plan's buffer.
+ *   functional  0 = Slater+VWN5, 1 = PBE (spin-polarised);  npts <= XC_STATIC_MAX_POINTS, else XC_EUNSUPPORTED
+ *   d_w    [device] npts           partition weights w_i (points with w_i = 0 are skipped: their densities are not read)
+ *   d_rho  [device] 2 x npts       rho_a | rho_b (spin-major);  d_grho [device] 2 x npts x 3  grad rho_s (PBE; may be NULL for 0)
+ *   rho_tol > 0                    as xc_grid_spec.rho_tol of a spin-unrestricted build
+ *   d_cA   [device] 2 x npts  out  a_s = w v_rho_s (LDA) | 1/2 w v_rho_s (PBE): coefficient of Phi in Z^s, Eq. (20)
+ *   d_cG   [device] 2 x npts x 3 out  g_s = w (2 v_ss grad rho_s + v_ab grad rho_s') (PBE; may be NULL for 0)
+ *   d_out3 [device] 3         out  E_xc, N_a, N_b (Eq. (16)), summed in a fixed order: bit-identical from call to call
+ * All pointers are device pointers of the CURRENT device, owned by the caller; the call is stream-ordered on cuda_stream
+ * and returns without synchronising.  The static array (768 KB) exists once per GPU that loads the library and is held until
+ * the process exits; every call on a GPU shares it and it keeps the last call's contents (nothing in it needs to start
+ * at zero: a call overwrites the partials it then reads).  Calls that OVERLAP on one GPU (two streams, two threads) race
+ * on it: serialise them.  No cudaMalloc, cudaFree or allocating library routine is called.
+ * Errors: XC_EINVAL (enum, null, npts < 0, rho_tol <= 0), XC_EUNSUPPORTED (npts beyond the maximum), XC_ECUDA. */
+#define XC_STATIC_MAX_POINTS 8388608
+int xc_functional_uks_static(int32_t functional, int64_t npts, const double* d_w, const double* d_rho, const double* d_grho,
+                             double rho_tol, double* d_cA, double* d_cG, double* d_out3, void* cuda_stream);
+
 /* FP64 pipe microbenchmark of `device` (no memory traffic, register-resident chains; CUDA events, best of `reps`
  * launches): kind 0 = DFMA chains, 1 = DMMA (mma.sync m8n8k4 f64, the instruction of the batch kernel's contractions).
  * MEASURED_PEAKS.json has no FP64 entry, so bench.py measures the denominator of the FP64 roofline with this call

@@ -68,6 +68,7 @@ def _load():
                                  C.POINTER(XcGridSpec), C.c_int32, vp, C.c_int64, vp, C.c_int64, dp, dp, vp]
     lib.xc_partition_weights.argtypes = [C.POINTER(XcAtom), C.c_int32, C.c_int32, C.c_int64, vp, vp, vp, vp, vp, vp, vp]
     lib.xc_functional.argtypes = [C.c_int32, C.c_int64, vp, vp, C.c_double, vp, vp, vp, vp]
+    lib.xc_functional_uks_static.argtypes = [C.c_int32, C.c_int64, vp, vp, vp, C.c_double, vp, vp, vp, vp]
     lib.xc_measure_fp64_peak.argtypes = [C.c_int32, C.c_int32, C.c_int32, dp, dp]
     for name in EXPORTED:
         getattr(lib, name)  # fail loudly if a declared symbol is missing
@@ -76,7 +77,7 @@ def _load():
 
 EXPORTED = ["xc_plan_create", "xc_plan_info", "xc_plan_export", "xc_eval", "xc_eval_host", "xc_eval_uks", "xc_eval_uks_densities", "xc_eval_tau", "xc_eval_diagnostics",
             "xc_eval_timings", "xc_eval_counters", "xc_plan_stats", "xc_plan_destroy", "xc_integrate", "xc_partition_weights",
-            "xc_functional", "xc_measure_fp64_peak", "xc_strerror", "xc_last_error"]
+            "xc_functional", "xc_functional_uks_static", "xc_measure_fp64_peak", "xc_strerror", "xc_last_error"]
 
 _lib = _load()
 
@@ -314,6 +315,20 @@ def functional(kind, rho, sigma, rho_tol=1e-15, stream=None):
                               C.c_void_p(f.data_ptr()), C.c_void_p(vr.data_ptr()), C.c_void_p(vs.data_ptr()),
                               _stream_ptr(stream)))
     return f, vr, vs
+
+
+XC_STATIC_MAX_POINTS = 1 << 23
+
+
+def functional_uks_static(kind, w, rho, grho, cA, cG, out3, rho_tol=1e-15, stream=None):
+    """xc_functional_uks_static: the spin-coupling step without any allocation (the scratch is a static device array).
+    Every tensor is a caller-owned torch CUDA float64 tensor of the current device: w (n), rho (2, n), grho (2, n, 3) or
+    None for kind 0, outputs cA (2, n), cG (2, n, 3) or None, out3 (3) = E_xc, N_a, N_b.  Stream-ordered, no sync."""
+    ptr = lambda t: C.c_void_p(t.data_ptr() if t is not None else 0)
+    for t in (w, rho, grho, cA, cG, out3):
+        assert t is None or (t.is_cuda and t.is_contiguous() and t.element_size() == 8)
+    _check(_lib.xc_functional_uks_static(kind, w.numel(), ptr(w), ptr(rho), ptr(grho), rho_tol, ptr(cA), ptr(cG), ptr(out3),
+                                         _stream_ptr(stream)))
 
 
 def measure_fp64_peak(kind=1, device=0, reps=5):

@@ -795,6 +795,23 @@ int xc_partition_weights(const xc_atom* atoms, int32_t natoms, int32_t partition
   return rc;
 }
 
+static_assert(kUksStaticMaxPoints == XC_STATIC_MAX_POINTS, "header and kernel agree on the static scratch size");
+int xc_functional_uks_static(int32_t functional, int64_t npts, const double* d_w, const double* d_rho, const double* d_grho,
+                             double rho_tol, double* d_cA, double* d_cG, double* d_out3, void* cuda_stream) {
+  if (functional < 0 || functional > 1) return fail(XC_EINVAL, "xc_functional_uks_static: functional must be 0 (Slater+VWN5) or 1 (PBE)");
+  if (npts < 0) return fail(XC_EINVAL, "xc_functional_uks_static: npts < 0");
+  if (npts > kUksStaticMaxPoints)
+    return fail(XC_EUNSUPPORTED, "xc_functional_uks_static: npts = " + std::to_string(npts) + " exceeds the static scratch (at most " +
+                                     std::to_string(kUksStaticMaxPoints) + " points); use xc_eval_uks, which allocates");
+  if (!(rho_tol > 0.0)) return fail(XC_EINVAL, "xc_functional_uks_static: rho_tol must be > 0 (reading A20)");
+  if (!d_out3 || (npts && (!d_w || !d_rho || !d_cA || (functional == 1 && (!d_grho || !d_cG)))))
+    return fail(XC_EINVAL, "xc_functional_uks_static: null argument");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (npts == 0) { CU(cudaMemsetAsync(d_out3, 0, 24, st)); return XC_OK; }
+  CU(functional_uks_static(functional == 1, npts, d_w, d_rho, d_grho, rho_tol, d_cA, d_cG, d_out3, st));
+  return XC_OK;
+}
+
 int xc_functional(int32_t functional, int64_t n, const double* drho, const double* dsigma, double rho_tol, double* df,
                   double* dvrho, double* dvsigma, void* cuda_stream) {
   if (functional < 0 || functional > 1 || n < 0 || (n && (!drho || !df || !dvrho || !dvsigma)) || (functional == 1 && n && !dsigma))

@@ -53,6 +53,11 @@ cudaError_t launch_batch(int cls, bool gga, int mode, const BatchArgs& a, const 
 int64_t uks_functional_blocks(int64_t npts);
 cudaError_t launch_functional_uks(bool gga, int64_t npts, const double* w, const double* rho, const double* grho, double rho_tol,
                                   double* cA, double* cG, double* part, double* out3, cudaStream_t st);
+// the same without any allocation: block partials in a file-scope device array (xc_uks.cu); npts <= kUksStaticMaxPoints;
+// works on the CURRENT device; calls that overlap on one GPU race on the array
+constexpr int64_t kUksStaticMaxPoints = (int64_t)1 << 23;   // 32768 blocks of 256 points: 768 KB of partials per GPU
+cudaError_t functional_uks_static(bool gga, int64_t npts, const double* w, const double* rho, const double* grho, double rho_tol,
+                                  double* cA, double* cG, double* out3, cudaStream_t st);
 // restricted meta-GGA (reading A23): functional over the grid and per-batch E / N partials (xc_uks.cu)
 cudaError_t launch_functional_mgga(int64_t npts, int nbatches, const BatchRec* batches, const double* w, const double* rho, const double* grho,
                                    const double* tau, double rho_tol, double* cA, double* cG, double* cT, double* ef, double* en, double* Epart,

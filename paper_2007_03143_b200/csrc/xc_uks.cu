@@ -12,6 +12,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdint>
+#include <mutex>
 
 #include "xc_internal.h"
 #include "xc_kernels.h"
@@ -270,6 +271,47 @@ cudaError_t launch_functional_mgga(int64_t npts, int nbatches, const BatchRec* b
   return cudaGetLastError();
 }
 
+
+// ------------------------------------------------------------------------------------------------
+// The same step with NO allocation (xc_functional_uks_static; for callers that cannot call cudaMalloc: CUDA graph capture,
+// serving loops): the block partials go to a file-scope array instead of a cudaMalloc'ed buffer.  The array exists once per
+// GPU that loads the library (768 KB, held until exit), every call on that GPU shares it, and it keeps the last call's
+// contents.  Nothing in it has to start at zero: a call writes the partials of its blocks [0, nblk) before k_reduce3 reads
+// exactly those.  Two calls that overlap on one GPU (different streams, or two host threads) race on it.
+// In host code the array's NAME is a host-side stand-in, not a device address: the address the kernels get comes from
+// cudaGetSymbolAddress, asked once per device with that device current.
+// ------------------------------------------------------------------------------------------------
+constexpr int64_t kStaticMaxBlocks = kUksStaticMaxPoints / kUksThreads;
+static_assert(kUksStaticMaxPoints % kUksThreads == 0, "kUksStaticMaxPoints is a whole number of blocks");
+static __device__ __align__(256) double g_uks_static_part[3 * kStaticMaxBlocks];
+
+namespace {
+constexpr int kMaxDevices = 64;
+std::mutex g_static_mu;
+double* g_static_part_addr[kMaxDevices] = {};   // device address of g_uks_static_part on device d (null: not asked yet)
+}  // namespace
+
+cudaError_t functional_uks_static(bool gga, int64_t npts, const double* w, const double* rho, const double* grho, double rho_tol,
+                                  double* cA, double* cG, double* out3, cudaStream_t st) {
+  if (npts <= 0) return cudaSuccess;
+  if (npts > kUksStaticMaxPoints) return cudaErrorInvalidValue;   // (the C entry point rejects it with its own message first)
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+  double* part = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_part_addr[dev]) {
+      void* ptr = nullptr;
+      e = cudaGetSymbolAddress(&ptr, g_uks_static_part);   // the current device's copy of the array
+      if (e != cudaSuccess) return e;
+      g_static_part_addr[dev] = (double*)ptr;
+    }
+    part = g_static_part_addr[dev];
+  }
+  return launch_functional_uks(gga, npts, w, rho, grho, rho_tol, cA, cG, part, out3, st);
+}
 
 cudaError_t launch_functional_uks(bool gga, int64_t npts, const double* w, const double* rho, const double* grho, double rho_tol,
                                   double* cA, double* cG, double* part, double* out3, cudaStream_t st) {
