@@ -162,7 +162,7 @@ static int eval_mgga(xc_plan* p, const double* dP, int64_t ldp, double* dV, int6
   HostPlan& hp = p->hp;
   const int64_t npts = hp.npts;
   const bool diag = (flags & XC_EVAL_DIAG) != 0;
-  int launches = 0;
+  int launches = 0, nk = 0;
   if (!p->d_urho) {
     const size_t n = std::max<size_t>((size_t)npts, 1);
     CU(cudaMalloc((void**)&p->d_urho, 2 * n * 8));   // rho | tau
@@ -197,13 +197,13 @@ static int eval_mgga(xc_plan* p, const double* dP, int64_t ldp, double* dV, int6
   ba.rho_out = d_rho; ba.grho_out = d_gr;
   if (nl) { CUK(launch_pack(ba, p->d_ids_large, nl, false, st), st); ++launches; }
   if (nsm) { CUK(launch_pack(ba, p->d_ids_small, nsm, false, st), st); ++launches; }
-  if (nl) { CUK(launch_batch(1, true, 1, ba, p->d_ids_large, nl, hp.smem_large, st), st); ++launches; }
+  if (nl) { CUK(launch_batch(1, true, 1, ba, p->d_ids_large, nl, hp.smem_large, st, hp.n_heavy, &nk), st); launches += nk; }
   if (nsm) { CUK(launch_batch(0, true, 1, ba, p->d_ids_small, nsm, hp.smem_small, st), st); ++launches; }
   // tau: lower triangle of P^j
   ba.rho_out = d_tau; ba.grho_out = nullptr;
   if (nl) { CUK(launch_pack(ba, p->d_ids_large, nl, true, st), st); ++launches; }
   if (nsm) { CUK(launch_pack(ba, p->d_ids_small, nsm, true, st), st); ++launches; }
-  if (nl) { CUK(launch_batch(1, false, 3, ba, p->d_ids_large, nl, hp.smem_large, st), st); ++launches; }
+  if (nl) { CUK(launch_batch(1, false, 3, ba, p->d_ids_large, nl, hp.smem_large, st, hp.n_heavy, &nk), st); launches += nk; }
   if (nsm) { CUK(launch_batch(0, false, 3, ba, p->d_ids_small, nsm, hp.smem_small, st), st); ++launches; }
   CU(cudaEventRecord(p->ev[2], st));
   // functional, per-batch partial sums
@@ -222,10 +222,10 @@ static int eval_mgga(xc_plan* p, const double* dP, int64_t ldp, double* dV, int6
     CU(cudaMemsetAsync(p->d_vlo, 0, nb2 * 8, st));
     CU(cudaMemsetAsync(p->d_result + 2, 0, 16, st));
     ba.cA = d_a; ba.cG = p->d_ucG;
-    if (nl) { CUK(launch_batch(1, true, 2, ba, p->d_ids_large, nl, hp.smem_large, st), st); ++launches; }
+    if (nl) { CUK(launch_batch(1, true, 2, ba, p->d_ids_large, nl, hp.smem_large, st, hp.n_heavy, &nk), st); launches += nk; }
     if (nsm) { CUK(launch_batch(0, true, 2, ba, p->d_ids_small, nsm, hp.smem_small, st), st); ++launches; }
     ba.cA = d_t; ba.cG = nullptr;
-    if (nl) { CUK(launch_batch(1, false, 4, ba, p->d_ids_large, nl, hp.smem_large, st), st); ++launches; }
+    if (nl) { CUK(launch_batch(1, false, 4, ba, p->d_ids_large, nl, hp.smem_large, st, hp.n_heavy, &nk), st); launches += nk; }
     if (nsm) { CUK(launch_batch(0, false, 4, ba, p->d_ids_small, nsm, hp.smem_small, st), st); ++launches; }
     CUK(launch_reduce((int64_t)hp.batches.size(), p->d_Epart, p->d_Npart, p->d_result, st), st);
     CUK(launch_finalize(hp.nbasis, p->d_vhi, p->d_vlo, dV, ldv, p->vexp, false, st), st);
@@ -408,7 +408,7 @@ int xc_eval(xc_plan* p, const double* dP, int64_t ldp, double* dV, int64_t ldv, 
   }
   const bool gga = hp.spec.functional == 1;
   const bool diag = (flags & XC_EVAL_DIAG) != 0;
-  int launches = 0;
+  int launches = 0, nk = 0;
   size_t ie = 0;
   if (diag && !p->d_rho) {
     CU(cudaMalloc((void**)&p->d_rho, std::max<size_t>(hp.npts * 8, 8)));
@@ -445,7 +445,7 @@ int xc_eval(xc_plan* p, const double* dP, int64_t ldp, double* dV, int64_t ldv, 
     CU(cudaMemsetAsync(p->d_vlo, 0, nb2 * 8, st));
     CU(cudaMemsetAsync(p->d_result + 2, 0, 16, st));
     if (attempt == 0) CU(cudaEventRecord(p->ev[ie++], st));
-    if (!hp.ids_large.empty()) { CUK(launch_batch(1, gga, 0, ba, p->d_ids_large, (int)hp.ids_large.size(), hp.smem_large, st), st); ++launches; }
+    if (!hp.ids_large.empty()) { CUK(launch_batch(1, gga, 0, ba, p->d_ids_large, (int)hp.ids_large.size(), hp.smem_large, st, hp.n_heavy, &nk), st); launches += nk; }
     if (!hp.ids_small.empty()) { CUK(launch_batch(0, gga, 0, ba, p->d_ids_small, (int)hp.ids_small.size(), hp.smem_small, st), st); ++launches; }
     if (attempt == 0) CU(cudaEventRecord(p->ev[ie++], st));
     CUK(launch_reduce((int64_t)hp.batches.size(), p->d_Epart, p->d_Npart, p->d_result, st), st);
@@ -501,7 +501,7 @@ int xc_eval_uks(xc_plan* p, const double* dPa, const double* dPb, int64_t ldp, d
   DeviceGuard guard(p->device);
   const bool gga = hp.spec.functional == 1;
   const int64_t npts = hp.npts;
-  int launches = 0;
+  int launches = 0, nk = 0;
   if (!p->d_urho) {
     const size_t n = std::max<size_t>((size_t)npts, 1);
     CU(cudaMalloc((void**)&p->d_urho, 2 * n * 8));
@@ -530,7 +530,7 @@ int xc_eval_uks(xc_plan* p, const double* dPa, const double* dPb, int64_t ldp, d
     ba.rho_out = p->d_urho + (size_t)s * npts; ba.grho_out = p->d_ugrho + (size_t)s * npts * 3;
     if (!hp.ids_large.empty()) { CUK(launch_pack(ba, p->d_ids_large, (int)hp.ids_large.size(), !gga, st), st); ++launches; }
     if (!hp.ids_small.empty()) { CUK(launch_pack(ba, p->d_ids_small, (int)hp.ids_small.size(), !gga, st), st); ++launches; }
-    if (!hp.ids_large.empty()) { CUK(launch_batch(1, gga, 1, ba, p->d_ids_large, (int)hp.ids_large.size(), hp.smem_large, st), st); ++launches; }
+    if (!hp.ids_large.empty()) { CUK(launch_batch(1, gga, 1, ba, p->d_ids_large, (int)hp.ids_large.size(), hp.smem_large, st, hp.n_heavy, &nk), st); launches += nk; }
     if (!hp.ids_small.empty()) { CUK(launch_batch(0, gga, 1, ba, p->d_ids_small, (int)hp.ids_small.size(), hp.smem_small, st), st); ++launches; }
   }
   CU(cudaEventRecord(p->ev[2], st));
@@ -547,7 +547,7 @@ int xc_eval_uks(xc_plan* p, const double* dPa, const double* dPb, int64_t ldp, d
       CU(cudaMemsetAsync(p->d_vhi, 0, nb2 * 8, st));
       CU(cudaMemsetAsync(p->d_vlo, 0, nb2 * 8, st));
       CU(cudaMemsetAsync(p->d_result + 2, 0, 16, st));
-      if (!hp.ids_large.empty()) { CUK(launch_batch(1, gga, 2, ba, p->d_ids_large, (int)hp.ids_large.size(), hp.smem_large, st), st); ++launches; }
+      if (!hp.ids_large.empty()) { CUK(launch_batch(1, gga, 2, ba, p->d_ids_large, (int)hp.ids_large.size(), hp.smem_large, st, hp.n_heavy, &nk), st); launches += nk; }
       if (!hp.ids_small.empty()) { CUK(launch_batch(0, gga, 2, ba, p->d_ids_small, (int)hp.ids_small.size(), hp.smem_small, st), st); ++launches; }
       CUK(launch_finalize(hp.nbasis, p->d_vhi, p->d_vlo, dV, ldv, p->vexp, false, st), st);
       ++launches;
@@ -608,7 +608,7 @@ int xc_eval_tau(xc_plan* p, const double* dP, int64_t ldp, double* d_tau, int32_
   if (ldp < hp.nbasis) return fail(XC_EINVAL, "leading dimension smaller than n_basis");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   DeviceGuard guard(p->device);
-  int launches = 0;
+  int launches = 0, nk = 0;
   { const int rc = run_weights(p, flags, st, launches); if (rc != XC_OK) return rc; }
   BatchArgs ba;
   ba.batches = p->d_batches; ba.bshells = p->d_bshells; ba.bsfoff = p->d_bsfoff; ba.bfidx = p->d_bfidx;
@@ -621,7 +621,7 @@ int xc_eval_tau(xc_plan* p, const double* dP, int64_t ldp, double* d_tau, int32_
   CU(cudaMemsetAsync(d_tau, 0, (size_t)hp.npts * 8, st));
   if (!hp.ids_large.empty()) { CUK(launch_pack(ba, p->d_ids_large, (int)hp.ids_large.size(), true, st), st); ++launches; }
   if (!hp.ids_small.empty()) { CUK(launch_pack(ba, p->d_ids_small, (int)hp.ids_small.size(), true, st), st); ++launches; }
-  if (!hp.ids_large.empty()) { CUK(launch_batch(1, false, 3, ba, p->d_ids_large, (int)hp.ids_large.size(), hp.smem_large, st), st); ++launches; }
+  if (!hp.ids_large.empty()) { CUK(launch_batch(1, false, 3, ba, p->d_ids_large, (int)hp.ids_large.size(), hp.smem_large, st, hp.n_heavy, &nk), st); launches += nk; }
   if (!hp.ids_small.empty()) { CUK(launch_batch(0, false, 3, ba, p->d_ids_small, (int)hp.ids_small.size(), hp.smem_small, st), st); ++launches; }
   CU(cudaStreamSynchronize(st));
   p->launches = launches;

@@ -14,6 +14,7 @@ constexpr int kMaxL = 2;
 constexpr int kMaxPrim = 16;
 constexpr int kBatchThreads = 512;  // 16 warps per batch CTA
 constexpr int kSmallNb = 112;   // N_b^j limit of the 64-point-tile instantiation (<= 28 lower-triangle 16x16 blocks = 2 per warp of 16)
+constexpr int kMidNb = 144;     // class 1 batches up to here (<= 45 blocks) run the three-round instantiation: its accumulators stay in registers
 constexpr int kMaxNb = 192;     // N_b^j limit of the batch kernel (<= 78 blocks = 5 per warp); the planner splits larger batches
 constexpr size_t kSmemLimit = 227 * 1024;
 constexpr size_t kBatchStaticSmem = 2048;   // static shared memory of k_xc_batch (live-point list, counters, ring barriers), rounded up
@@ -84,6 +85,7 @@ struct HostPlan {
   int64_t ppk_doubles = 0;              // size of the packed-P^j buffer
   double sum_nbnq = 0, sum_nb2 = 0, flops = 0;
   int max_nb = 0, max_ns = 0;
+  int n_heavy = 0;             // the first n_heavy entries of ids_large have N_b^j > kMidNb (five-round instantiation)
   size_t smem_small = 0, smem_large = 0;  // max dynamic smem over each work list
 };
 

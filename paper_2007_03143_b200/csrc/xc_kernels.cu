@@ -1012,30 +1012,45 @@ static cudaError_t launch_batch_t(const BatchArgs& a, const int32_t* batch_ids, 
   k_xc_batch<NT, T, GGA, NTW, ROUNDS, MINB, MODE><<<nbatches, NT, smem, st>>>(a, batch_ids);
   return cudaGetLastError();
 }
-template <int MODE>
-static cudaError_t launch_batch_m(int cls, bool gga, const BatchArgs& a, const int32_t* batch_ids, int nbatches, size_t smem, cudaStream_t st) {
-  if (cls == 0) return gga ? launch_batch_t<512, 64, true, 4, 2, 1, MODE>(a, batch_ids, nbatches, smem, st)
-                           : launch_batch_t<512, 64, false, 4, 2, 1, MODE>(a, batch_ids, nbatches, smem, st);
-  return gga ? launch_batch_t<512, 32, true, 3, 5, 1, MODE>(a, batch_ids, nbatches, smem, st)
-             : launch_batch_t<512, 32, false, 3, 5, 1, MODE>(a, batch_ids, nbatches, smem, st);
+// one class of batches; cls 0: T = 64, two rounds of V^j blocks; cls 1: T = 32, three rounds (N_b^j <= kMidNb); cls 2: T = 32, five
+template <int MODE, bool GGA>
+static cudaError_t launch_batch_c(int cls, const BatchArgs& a, const int32_t* batch_ids, int nbatches, size_t smem, cudaStream_t st) {
+  if (cls == 0) return launch_batch_t<512, 64, GGA, 4, 2, 1, MODE>(a, batch_ids, nbatches, smem, st);
+  if (cls == 1) return launch_batch_t<512, 32, GGA, 3, 3, 1, MODE>(a, batch_ids, nbatches, smem, st);
+  return launch_batch_t<512, 32, GGA, 3, 5, 1, MODE>(a, batch_ids, nbatches, smem, st);
+}
+static cudaError_t launch_batch_1(int cls, bool gga, int mode, const BatchArgs& a, const int32_t* batch_ids, int nbatches, size_t smem,
+                                  cudaStream_t st) {
+  switch (mode) {
+    case 1: return gga ? launch_batch_c<1, true>(cls, a, batch_ids, nbatches, smem, st) : launch_batch_c<1, false>(cls, a, batch_ids, nbatches, smem, st);
+    case 2: return gga ? launch_batch_c<2, true>(cls, a, batch_ids, nbatches, smem, st) : launch_batch_c<2, false>(cls, a, batch_ids, nbatches, smem, st);
+    // tau (3) and the tau term of a meta-GGA potential (4) run the LDA GEMMs per gradient component, whatever the plan's functional
+    case 3: return launch_batch_c<3, false>(cls, a, batch_ids, nbatches, smem, st);
+    case 4: return launch_batch_c<4, false>(cls, a, batch_ids, nbatches, smem, st);
+    default: return gga ? launch_batch_c<0, true>(cls, a, batch_ids, nbatches, smem, st) : launch_batch_c<0, false>(cls, a, batch_ids, nbatches, smem, st);
+  }
 }
 
-// cls 0: N_b^j <= kSmallNb, tiles of 64 points; cls 1: N_b^j <= kMaxNb, tiles of 32 points; 16 warps, one CTA per SM.
-// mode 0: fused restricted build; 1: densities of one spin; 2: potential of one spin from given coefficients (xc_eval_uks)
 cudaError_t launch_batch(int cls, bool gga, int mode, const BatchArgs& a, const int32_t* batch_ids, int nbatches, size_t smem,
-                         cudaStream_t st) {
+                         cudaStream_t st, int n_heavy, int* launched) {
+  if (launched) *launched = 0;
   if (nbatches <= 0) return cudaSuccess;
-  if (mode == 1) return launch_batch_m<1>(cls, gga, a, batch_ids, nbatches, smem, st);
-  if (mode == 2) return launch_batch_m<2>(cls, gga, a, batch_ids, nbatches, smem, st);
-  if (mode == 4) {   // tau term of a meta-GGA potential: V^j += sum_c (t d_c Phi)(d_c Phi)^T, the LDA (symmetric) V^j GEMM per component
-    return cls == 0 ? launch_batch_t<512, 64, false, 4, 2, 1, 4>(a, batch_ids, nbatches, smem, st)
-                    : launch_batch_t<512, 32, false, 3, 5, 1, 4>(a, batch_ids, nbatches, smem, st);
+  if (cls == 0) {
+    if (launched) *launched = 1;
+    return launch_batch_1(0, gga, mode, a, batch_ids, nbatches, smem, st);
   }
-  if (mode == 3) {   // tau: gradient components through the LDA (lower-triangle) X GEMM, whatever the plan's functional
-    return cls == 0 ? launch_batch_t<512, 64, false, 4, 2, 1, 3>(a, batch_ids, nbatches, smem, st)
-                    : launch_batch_t<512, 32, false, 3, 5, 1, 3>(a, batch_ids, nbatches, smem, st);
+  n_heavy = n_heavy < 0 ? 0 : (n_heavy > nbatches ? nbatches : n_heavy);
+  if (n_heavy > 0) {
+    const cudaError_t e = launch_batch_1(2, gga, mode, a, batch_ids, n_heavy, smem, st);
+    if (e != cudaSuccess) return e;
+    if (launched) ++*launched;
   }
-  return launch_batch_m<0>(cls, gga, a, batch_ids, nbatches, smem, st);
+  if (n_heavy < nbatches) {
+    const cudaError_t e = launch_batch_1(1, gga, mode, a, batch_ids + n_heavy, nbatches - n_heavy, smem, st);
+    if (e != cudaSuccess) return e;
+    if (launched) ++*launched;
+  }
+  return cudaSuccess;
 }
 
 cudaError_t launch_finalize(int nbasis, const unsigned long long* vhi, const unsigned long long* vlo, double* V,

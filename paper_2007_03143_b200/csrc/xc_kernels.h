@@ -46,8 +46,10 @@ cudaError_t launch_weights_becke(const WeightArgs& a, const int32_t* batch_ids, 
 cudaError_t launch_functional(int kind, int64_t n, const double* rho, const double* sigma, double rho_tol, double* f,
                               double* vr, double* vs, cudaStream_t st);
 cudaError_t launch_pack(const BatchArgs& a, const int32_t* batch_ids, int nbatches, bool tri, cudaStream_t st);
+// cls 1: the first n_heavy batches of the list have N_b^j > kMidNb (one launch of the five-round kernel), the others run the
+// three-round kernel; *launched (may be null) receives the number of kernels launched (1 or 2)
 cudaError_t launch_batch(int cls, bool gga, int mode, const BatchArgs& a, const int32_t* batch_ids, int nbatches, size_t smem,
-                         cudaStream_t st);
+                         cudaStream_t st, int n_heavy = 0, int* launched = nullptr);
 // spin-unrestricted build: functional over the grid (xc_uks.cu); rho [2][npts], grho [2][npts][3] in, cA [2][npts], cG [2][npts][3]
 // and out3 = (E_xc, N_a, N_b) out; part: scratch of 3 * uks_functional_blocks(npts) doubles
 int64_t uks_functional_blocks(int64_t npts);

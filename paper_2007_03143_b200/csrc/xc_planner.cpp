@@ -539,7 +539,16 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
   // heaviest batches first: the tail of each launch is made of cheap CTAs
   auto cost = [&](int32_t j) { const BatchRec& b = hp.batches[j]; return (double)b.nb * b.nb * b.nq + 200.0 * b.ns * b.nq; };
   std::stable_sort(hp.ids_small.begin(), hp.ids_small.end(), [&](int32_t x, int32_t y) { return cost(x) > cost(y); });
-  std::stable_sort(hp.ids_large.begin(), hp.ids_large.end(), [&](int32_t x, int32_t y) { return cost(x) > cost(y); });
+  // (class 1: the batches with N_b^j > kMidNb first: they run as a launch of their own)
+  std::stable_sort(hp.ids_large.begin(), hp.ids_large.end(), [&](int32_t x, int32_t y) {
+    const bool hx = hp.batches[x].nb > kMidNb, hy = hp.batches[y].nb > kMidNb;
+    return hx != hy ? hx : cost(x) > cost(y);
+  });
+  hp.n_heavy = 0;
+  for (int32_t j : hp.ids_large) hp.n_heavy += hp.batches[j].nb > kMidNb ? 1 : 0;
+  // a launch of its own costs the tail of one more kernel (about one CTA's time), the three-round kernel gains ~4 % on its
+  // batches: with fewer than 4096 of them (28 waves) the whole class runs the five-round kernel, as one launch
+  if ((int)hp.ids_large.size() - hp.n_heavy < 4096) hp.n_heavy = (int)hp.ids_large.size();
   // Becke-88 weights launch: warps per CTA such that the per-warp distance rows fit in shared memory
   // (the SSF kernel has a fixed footprint and reads list entries beyond its cache from global memory)
   hp.w_warps = 8;
