@@ -58,11 +58,16 @@ typedef struct {
   int32_t functional;     /* 0 = LDA Slater+VWN5; 1 = GGA PBE; 2 = meta-GGA MS0 exchange + PBE correlation (reading A23;
                              PAPER.md:L51): xc_eval runs it as passes of the same kernels (densities, tau, functional, potential) */
   int32_t max_batch_pts;  /* <= 512 */
-  int32_t flags;          /* bit 0: reserved */
+  int32_t flags;          /* bit 0: reserved; bit 1 = XC_SPEC_SPLIT_CLASS1 (a tuning knob, results unchanged bit for bit) */
   double  eta;            /* Eq. (10) tolerance, 1e-10 */
   double  mk_alpha;       /* Mura-Knowles scale, bohr (5.0) */
   double  rho_tol;        /* points with rho <= rho_tol contribute nothing (1e-15, reading A12) */
 } xc_grid_spec;
+
+/* xc_grid_spec.flags.  XC_SPEC_SPLIT_CLASS1: batches with 112 < N_b^j <= 144 always run the three-round instantiation of the
+ * batch kernel (its V^j accumulators stay in registers), the ones beyond 144 as a launch of their own; by default the planner
+ * does that only when at least 4096 batches profit (or none is beyond 144) and otherwise keeps the class one five-round launch. */
+#define XC_SPEC_SPLIT_CLASS1 2
 
 /* flags of xc_eval / xc_eval_host */
 #define XC_EVAL_REUSE_WEIGHTS 1   /* reuse the partition weights of the previous xc_eval on this plan (skip step (a); reading A16) */

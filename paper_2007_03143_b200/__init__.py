@@ -5,7 +5,7 @@ The binding is loaded on first use (so that `python -m paper_2007_03143_b200.bui
 library exists); any use of the API without the built CUDA library raises ImportError -- there is no
 CPU fallback."""
 
-_API = ("EXPORTED", "LIB_PATH", "Plan", "XC_STATIC_MAX_POINTS", "XcError", "XcGridSpec", "functional", "functional_uks_static", "grid_spec",
+_API = ("EXPORTED", "LIB_PATH", "Plan", "XC_SPEC_SPLIT_CLASS1", "XC_STATIC_MAX_POINTS", "XcError", "XcGridSpec", "functional", "functional_uks_static", "grid_spec",
         "measure_fp64_peak", "partition_weights", "xc_integrate")
 
 

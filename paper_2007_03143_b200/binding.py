@@ -30,9 +30,12 @@ class XcGridSpec(C.Structure):
                 ("eta", C.c_double), ("mk_alpha", C.c_double), ("rho_tol", C.c_double)]
 
 
+XC_SPEC_SPLIT_CLASS1 = 2
+
+
 def grid_spec(n_rad, n_ang, functional, angular=0, partition=0, max_batch_pts=512, eta=1e-10, mk_alpha=5.0,
-              rho_tol=1e-15) -> XcGridSpec:
-    return XcGridSpec(n_rad, n_ang, 0, angular, partition, functional, max_batch_pts, 0, eta, mk_alpha, rho_tol)
+              rho_tol=1e-15, flags=0) -> XcGridSpec:
+    return XcGridSpec(n_rad, n_ang, 0, angular, partition, functional, max_batch_pts, flags, eta, mk_alpha, rho_tol)
 
 
 class XcError(RuntimeError):

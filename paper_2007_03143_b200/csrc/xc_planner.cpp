@@ -549,7 +549,7 @@ int build_host_plan(const xc_atom* atoms, int natoms, const xc_shell* shells, in
   // a launch of its own costs the tail of one more kernel (about one CTA's time), the three-round kernel gains ~4 % on its
   // batches: with fewer than 4096 of them (28 waves) the whole class runs the five-round kernel, as one launch
   // (no batch beyond kMidNb at all: the whole class runs the three-round kernel, still as one launch)
-  if (hp.n_heavy > 0 && (int)hp.ids_large.size() - hp.n_heavy < 4096) hp.n_heavy = (int)hp.ids_large.size();
+  if (hp.n_heavy > 0 && (int)hp.ids_large.size() - hp.n_heavy < 4096 && !(spec->flags & XC_SPEC_SPLIT_CLASS1)) hp.n_heavy = (int)hp.ids_large.size();
   // Becke-88 weights launch: warps per CTA such that the per-warp distance rows fit in shared memory
   // (the SSF kernel has a fixed footprint and reads list entries beyond its cache from global memory)
   hp.w_warps = 8;

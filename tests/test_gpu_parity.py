@@ -582,6 +582,36 @@ def test_mgga_parity(xc, orc, name):
     plan.close()
 
 
+def test_three_round_class_matches_the_five_round_one(xc):
+    """27 waters have 169 batches with 113..144 functions and 5 beyond: by default one five-round launch.  With
+    XC_SPEC_SPLIT_CLASS1 the 169 run the three-round instantiation (the one the large configs use): every build type --
+    restricted LDA / PBE / meta-GGA, spin-unrestricted, tau -- must agree to rounding (same blocks, same order of the sums;
+    the two instantiations are compiled separately, so a product-sum may be contracted into another FMA: 1 ulp of an
+    element of Phi, seen as ~1e-16 max|V|)."""
+    import torch
+    from workloads import spin_density_matrices
+    w = make_workload("w27")
+    P = torch.from_numpy(w.P).cuda()
+    Pa, Pb = (torch.from_numpy(x).cuda() for x in spin_density_matrices(w, 139, 131))
+    for functional in (0, 1, 2):
+        res = []
+        for flags in (0, xc.XC_SPEC_SPLIT_CLASS1):
+            plan = xc.Plan.from_workload(w, spec=xc.grid_spec(w.n_rad, w.n_ang, functional, flags=flags))
+            E, N, V = plan.eval(P)
+            out = [E, N, V.clone(), plan.eval_tau(P, reuse_weights=True).clone()]
+            if functional < 2:
+                Eu, (Na, Nb), Va, Vb = plan.eval_uks(Pa, Pb, reuse_weights=True)
+                out += [Eu, Na, Nb, Va.clone(), Vb.clone()]
+            res.append(out)
+            plan.close()
+        for a, b in zip(*res):
+            if torch.is_tensor(a):
+                assert float((a - b).abs().max()) <= 1e-14 * float(a.abs().max()), functional
+            else:
+                assert abs(a - b) <= 1e-14 * abs(a), functional
+        assert float(res[0][2].abs().max()) > 0.1
+
+
 def test_extensions_at_c3_size_sampled(xc, orc):
     """The spin-unrestricted and meta-GGA builds on the 64-water PBE shapes (4.3 M points, 1600 functions): 60 random batches
     against the oracle point by point (rho_s, grad rho_s, tau) and per batch (meta-GGA E / N sums); electron counts against
