@@ -247,8 +247,8 @@ def oracle_sample(w, name, target_seconds=15.0, stride=None, fn=None):
     basis = (w.shell_atom, w.shell_L, w.shell_nprim, w.shell_prim_off, w.exps, w.coefs)
     na = len(w.atoms_Z)
     if stride is None:
-        # calibrated here: ~1.7 core-seconds per atom-centred grid at 64 waters (LDA, 75x302); the weights term grows with N_atoms
-        per_atom = 0.85 * (1 + na / 200.0) * (1.6 if fn == 1 else 1.0) * (w.n_rad * w.n_ang / 22650.0) / max(1, orc.num_threads())
+        # calibrated on the GPU box (16 threads): ~0.3 s wall per atom-centred grid at c5 (PBE, 100x302, 1536 atoms); the weights term grows with N_atoms
+        per_atom = 0.85 * (1 + na / 800.0) * (1.6 if fn == 1 else 1.0) * (w.n_rad * w.n_ang / 22650.0) / max(1, orc.num_threads())
         stride = max(1, int(round(na * per_atom / target_seconds)))
     atoms = np.arange(0, na, stride)
     t0 = time.perf_counter()
