@@ -241,19 +241,30 @@ __global__ void k_functional(int kind, int64_t n, const double* rho, const doubl
 // tri (LDA): rho = phi^T P phi = 2 phi^T L phi with L = strict lower triangle of P^j + half its diagonal, so only
 // L is packed (entries nu > mu are zero) and the X GEMM skips the k-steps above the diagonal.
 __global__ void __launch_bounds__(256) k_pack_P(BatchArgs a, const int32_t* __restrict__ batch_ids, int tri) {
+  __shared__ int64_t sRow[kMaxNb];             // row offsets fidx[mu] * ldp
+  __shared__ int sCol[kMaxNb];
   const BatchRec b = a.batches[batch_ids[blockIdx.x]];
   const int nb = b.nb, ntile = (nb + 7) >> 3, nks = (nb + 3) >> 2;
   const int32_t* fidx = a.bfidx + b.f_off;
+  for (int f = threadIdx.x; f < nb; f += 256) { const int g = fidx[f]; sCol[f] = g; sRow[f] = (int64_t)g * a.ldp; }
+  __syncthreads();
   double* out = a.ppk + b.ppk_off;
   const int total = nks * ntile * 32;
-  for (int e = threadIdx.x; e < total; e += 256) {
-    const int lane = e & 31, frag = e >> 5;
-    const int ks = frag / ntile, nt = frag - ks * ntile;
-    const int nu = 4 * ks + (lane & 3), mu = 8 * nt + (lane >> 2);
-    double v = 0.0;
-    if (nu < nb && mu < nb) v = __ldg(a.P + (size_t)fidx[mu] * a.ldp + fidx[nu]);   // P symmetric: row mu is read along nu
-    if (tri) v = nu < mu ? v : (nu == mu ? 0.5 * v : 0.0);
-    out[e] = v;
+  const int lane = threadIdx.x & 31, t4 = lane & 3, g4 = lane >> 2;
+  // four fragments in flight per thread (independent loads)
+  for (int e0 = threadIdx.x; e0 < total; e0 += 4 * 256) {
+    double v[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int e = e0 + u * 256, frag = e >> 5;
+      const int ks = frag / ntile, nt = frag - ks * ntile;
+      const int nu = 4 * ks + t4, mu = 8 * nt + g4;
+      v[u] = 0.0;
+      if (e < total && nu < nb && mu < nb && !(tri && nu > mu)) v[u] = __ldg(a.P + sRow[mu] + sCol[nu]);   // P symmetric: row mu is read along nu
+      if (tri && nu == mu) v[u] *= 0.5;
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) if (e0 + u * 256 < total) out[e0 + u * 256] = v[u];
   }
 }
 
